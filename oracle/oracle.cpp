@@ -1,0 +1,243 @@
+// CPU ORACLE — TEST INFRASTRUCTURE, NOT PRODUCT. See oracle.h for who may call this.
+//
+// Each function follows SURVEY.md §8(c) (the readings of PAPER.md this build binds itself to) in the
+// order and notation given there: no blocking, fusion or reordering, single thread, int64 ticks,
+// fp64 EMA with four separately rounded operations (build with -ffp-contract=off).
+//
+// Pin status (tests/test_oracle_*.py): characterize — pinned (Python bytes.split(), independent
+// per-byte reference, closed-form token/word ratio, hand cases). simulate — pinned to the hand-worked
+// traces H1-H6, closed forms (service time, M/M/1, M/D/1, EMA geometric form), invariants I1-I9 and
+// brute force; the absolute latencies of the synthetic server model are this build's reading of
+// BASELINE.json:configs[0] (DESIGN.md §4 A6-A10): "parity unpinned" beyond those pins.
+// tail_stats — pinned (hand values, numpy partition).
+#include "oracle.h"
+
+#include <algorithm>
+#include <cmath>
+#include <vector>
+
+namespace {
+
+// SURVEY.md §8(c) C.1 byte classes. WS = Python bytes.split() whitespace ("split()").
+inline bool is_ws(uint8_t c) { return c == 0x09 || c == 0x0A || c == 0x0B || c == 0x0C || c == 0x0D || c == 0x20; }
+// PUNCT = Python string.punctuation.
+inline bool is_punct(uint8_t c) {
+  return (c >= 0x21 && c <= 0x2F) || (c >= 0x3A && c <= 0x40) || (c >= 0x5B && c <= 0x60) || (c >= 0x7B && c <= 0x7E);
+}
+
+}  // namespace
+
+extern "C" int oracle_characterize(const uint8_t* bytes, int64_t n_bytes, const int64_t* offsets, int64_t n_prompts,
+                                   int32_t* words_out, int32_t* tokens_out) {
+  if (n_prompts < 0 || n_bytes < 0) return -1;
+  for (int64_t i = 0; i < n_prompts; ++i) {
+    int64_t a = offsets[i], b = offsets[i + 1];
+    if (a < 0 || b < a || b > n_bytes) return -1;
+    // words: number of maximal runs of non-WS bytes inside the prompt (isolated string).
+    // tokens: sum over maximal LETTER runs of ceil(len/4), plus the number of PUNCT bytes.
+    int32_t words = 0, tokens = 0;
+    bool in_word = false;
+    int64_t run = 0;  // current LETTER run length
+    for (int64_t k = a; k < b; ++k) {
+      uint8_t c = bytes[k];
+      bool ws = is_ws(c), pu = is_punct(c);
+      if (!ws) { if (!in_word) ++words; in_word = true; } else in_word = false;
+      if (!ws && !pu) ++run;
+      else { tokens += (int32_t)((run + 3) / 4); run = 0; if (pu) ++tokens; }
+    }
+    tokens += (int32_t)((run + 3) / 4);
+    words_out[i] = words;
+    tokens_out[i] = tokens;
+  }
+  return 0;
+}
+
+namespace {
+
+enum { FIFO = 0, PRIORITY = 1, WEIGHTED = 2, SJF = 3, AGING = 4 };
+enum { SPLIT = 0, EXACT = 1 };
+
+struct Sim {
+  // inputs for one instance (local request index r in [0,n))
+  const int64_t* arr; const uint8_t* tier; const int32_t* W; const int32_t* P; const int32_t* O;
+  int64_t n; const oracle_server* sv; int policy, estimator; double alpha;
+  // state (SURVEY.md §8(c) C.2 "State per instance")
+  int64_t now = 0, next = 0, kv_used = 0, done = 0;
+  double B[3] = {1.0, 1.0, 1.0};
+  int cur = 0;                       // Weighted slot cursor
+  std::vector<int64_t> queued;       // all queued requests, arrival (= index) order
+  std::vector<int64_t> R;            // running set, ascending request index
+  std::vector<int64_t> est, g;
+
+  int64_t base(int64_t r) const { return estimator == SPLIT ? (int64_t)W[r] : (int64_t)P[r]; }
+
+  // admit_to_queue(r): estimate frozen at arrival (A5), Eq. 1-2 reduced form (A1).
+  void admit_to_queue(int64_t r) {
+    int64_t b = base(r);
+    if (b > 0) est[r] = (int64_t)std::ceil(B[tier[r]] * (double)b); else est[r] = 0;
+    queued.push_back(r);
+  }
+  // ema_update(k,r): Eq. 5/6 with T_actual = tokens, T_base = base (A3); four separate roundings.
+  void ema_update(int k, int64_t r) {
+    int64_t b = base(r);
+    if (alpha > 0.0 && b > 0) {
+      double m = (double)P[r] / (double)b;
+      double t1 = 1.0 - alpha;
+      double t2 = t1 * B[k];
+      double t3 = alpha * m;
+      B[k] = t2 + t3;
+    }
+  }
+  // peek(policy, now): position in `queued` of the request the policy serves next. Lower key wins,
+  // ties -> lower request index. `queued` is in index order, so the first minimum is the answer.
+  size_t peek(int* weighted_pos) const {
+    size_t best = 0;
+    if (policy == WEIGHTED) {
+      // slot pattern: weight[0] Premium slots, weight[1] Standard, weight[2] Batch (A9); scan from cur.
+      int tot = sv->weight[0] + sv->weight[1] + sv->weight[2];
+      for (int s = 0; s < tot; ++s) {
+        int pos = (cur + s) % tot;
+        int t = pos < sv->weight[0] ? 0 : (pos < sv->weight[0] + sv->weight[1] ? 1 : 2);
+        for (size_t i = 0; i < queued.size(); ++i)
+          if (tier[queued[i]] == t) { *weighted_pos = pos; return i; }   // head of that tier's FIFO
+      }
+      return 0;  // unreachable when queued is non-empty
+    }
+    int64_t bk0 = 0, bk1 = 0;
+    for (size_t i = 0; i < queued.size(); ++i) {
+      int64_t r = queued[i], k0, k1 = r;
+      switch (policy) {
+        case FIFO: k0 = 0; break;                                   // key = seq
+        case PRIORITY: k0 = tier[r]; break;                         // (tier, seq)
+        case SJF: k0 = est[r]; break;                               // (est, seq)
+        default: {                                                  // AGING (A10)
+          int64_t lv = (now - arr[r]) / sv->aging_step;
+          int64_t eff = (int64_t)tier[r] - lv; if (eff < 0) eff = 0;
+          k0 = eff;
+        }
+      }
+      if (i == 0 || k0 < bk0 || (k0 == bk0 && k1 < bk1)) { best = i; bk0 = k0; bk1 = k1; }
+    }
+    return best;
+  }
+};
+
+}  // namespace
+
+extern "C" int oracle_simulate(const oracle_traces* tr, const oracle_server* sv, const oracle_instance* inst,
+                               int64_t n_inst, const int64_t* out_off, int64_t* start_tick, int64_t* done_tick,
+                               double* ema_final, const int64_t* traj_off, double* ema_traj) {
+  if (sv->max_batch < 1) return -1;
+  if (sv->weight[0] < 1 || sv->weight[1] < 1 || sv->weight[2] < 1) return -1;
+  if (sv->aging_step < 1) return -1;
+  for (int64_t ii = 0; ii < n_inst; ++ii) {
+    const oracle_instance& in = inst[ii];
+    if (in.trace < 0 || in.trace >= tr->n_traces || in.policy < 0 || in.policy > 4 || in.estimator < 0 ||
+        in.estimator > 1 || !(in.ema_alpha >= 0.0 && in.ema_alpha <= 1.0)) return -1;
+    int64_t lo = tr->trace_off[in.trace], n = tr->trace_off[in.trace + 1] - lo;
+    Sim s;
+    s.arr = tr->arrival_tick + lo; s.tier = tr->tier + lo; s.W = tr->words + lo; s.P = tr->tokens + lo;
+    s.O = tr->out_len + lo; s.n = n; s.sv = sv; s.policy = in.policy; s.estimator = in.estimator; s.alpha = in.ema_alpha;
+    s.est.assign(n, 0); s.g.assign(n, 0);
+    int64_t* st = start_tick + out_off[ii];
+    int64_t* dn = done_tick + out_off[ii];
+    // instance ii owns samples [traj_off[ii], traj_off[ii+1]) of ema_traj, floor(n/traj_every) of them, 3 doubles each
+    double* traj = (ema_traj && traj_off && sv->traj_every > 0) ? ema_traj + traj_off[ii] * 3 : nullptr;
+
+    bool skip_to_ingest_now = false;
+    for (;;) {
+      if (!skip_to_ingest_now) {
+        // 1. INGEST-EARLY: arrivals strictly before `now` use the factors before this tick's completions (R-ORD).
+        while (s.next < n && s.arr[s.next] < s.now) s.admit_to_queue(s.next++);
+        // 2. RETIRE: completions at `now`, ascending request index.
+        for (size_t i = 0; i < s.R.size();) {
+          int64_t r = s.R[i];
+          if (s.g[r] == s.O[r]) {
+            dn[r] = s.now;
+            s.kv_used -= (int64_t)s.P[r] + s.g[r];
+            s.R.erase(s.R.begin() + i);
+            s.ema_update(s.tier[r], r);
+            ++s.done;
+            if (traj && sv->traj_every > 0 && s.done % sv->traj_every == 0) {
+              double* q = traj + (s.done / sv->traj_every - 1) * 3;
+              q[0] = s.B[0]; q[1] = s.B[1]; q[2] = s.B[2];
+            }
+          } else ++i;
+        }
+      }
+      skip_to_ingest_now = false;
+      // 3. INGEST-NOW: arrivals at exactly `now` see the updated factors.
+      while (s.next < n && s.arr[s.next] <= s.now) s.admit_to_queue(s.next++);
+      // 4. ADMIT
+      int64_t prefill_new = 0;
+      while ((int64_t)s.R.size() < sv->max_batch && !s.queued.empty()) {
+        int wpos = 0;
+        size_t qi = s.peek(&wpos);
+        int64_t c = s.queued[qi];
+        if (!s.R.empty() && sv->kv_budget > 0 && s.kv_used + s.est[c] > sv->kv_budget) break;  // deferred (A8)
+        s.queued.erase(s.queued.begin() + qi);
+        if (s.policy == WEIGHTED) s.cur = (wpos + 1) % (sv->weight[0] + sv->weight[1] + sv->weight[2]);
+        st[c] = s.now; s.g[c] = 0;
+        s.R.insert(std::lower_bound(s.R.begin(), s.R.end(), c), c);
+        s.kv_used += s.P[c];
+        prefill_new += s.P[c];
+      }
+      // 5. IDLE / END
+      if (s.R.empty()) {
+        if (s.next == n) break;
+        s.now = s.arr[s.next];
+        skip_to_ingest_now = true;
+        continue;
+      }
+      // 6. STEP: one server iteration (A6, A7).
+      int64_t ctx = 0;
+      for (int64_t r : s.R) ctx += (int64_t)s.P[r] + s.g[r];
+      int64_t dt = sv->c_base + sv->c_batch * (int64_t)s.R.size() + sv->c_ctx * ctx + sv->c_prefill * prefill_new;
+      for (int64_t r : s.R) s.g[r] += 1;
+      s.kv_used += (int64_t)s.R.size();
+      s.now += dt;
+    }
+    ema_final[ii * 3 + 0] = s.B[0]; ema_final[ii * 3 + 1] = s.B[1]; ema_final[ii * 3 + 2] = s.B[2];
+  }
+  return 0;
+}
+
+extern "C" int oracle_latencies(const oracle_traces* tr, const oracle_instance* inst, int64_t n_inst,
+                                const int64_t* out_off, const int64_t* start_tick, const int64_t* done_tick,
+                                const int32_t* group, const int64_t* t_mid, int64_t* e2e, int64_t* qdelay,
+                                int32_t* seg_tier, int32_t* seg_all) {
+  for (int64_t ii = 0; ii < n_inst; ++ii) {
+    int64_t t = inst[ii].trace, lo = tr->trace_off[t], n = tr->trace_off[t + 1] - lo;
+    for (int64_t r = 0; r < n; ++r) {
+      int64_t o = out_off[ii] + r, a = tr->arrival_tick[lo + r];
+      e2e[o] = done_tick[o] - a;        // end-to-end latency
+      qdelay[o] = start_tick[o] - a;    // queue wait
+      int32_t gph = group ? group[ii] : 0;
+      if (t_mid) gph = gph * 2 + (a >= t_mid[t] ? 1 : 0);   // pre/post-drift phase (configs[4])
+      if (seg_tier) seg_tier[o] = gph * 3 + tr->tier[lo + r];
+      if (seg_all) seg_all[o] = gph;
+    }
+  }
+  return 0;
+}
+
+extern "C" int oracle_tail_stats(const int64_t* values, const int32_t* seg_id, int64_t n, int32_t n_segments,
+                                 const int32_t* pct, int32_t n_pct, int64_t* out, int64_t* count_out) {
+  // collect values[i] with seg_id[i]==s (ids outside [0,n_segments) are skipped), sort ascending
+  std::vector<std::vector<int64_t>> bucket((size_t)n_segments);
+  for (int64_t i = 0; i < n; ++i) if (seg_id[i] >= 0 && seg_id[i] < n_segments) bucket[seg_id[i]].push_back(values[i]);
+  for (int32_t s = 0; s < n_segments; ++s) {
+    std::vector<int64_t>& v = bucket[s];
+    std::sort(v.begin(), v.end());
+    if (count_out) count_out[s] = (int64_t)v.size();
+    for (int32_t q = 0; q < n_pct; ++q) {
+      if (v.empty()) { out[s * n_pct + q] = -1; continue; }
+      // nearest rank (A13): idx = max(1, ceil(p*n/100)) - 1
+      int64_t rank = ((int64_t)pct[q] * (int64_t)v.size() + 99) / 100;
+      if (rank < 1) rank = 1;
+      if (rank > (int64_t)v.size()) rank = (int64_t)v.size();
+      out[s * n_pct + q] = v[rank - 1];
+    }
+  }
+  return 0;
+}

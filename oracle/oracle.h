@@ -1,0 +1,63 @@
+/* CPU ORACLE — TEST INFRASTRUCTURE, NOT PRODUCT.
+ *
+ * Plain, slow, single-threaded restatement of what the DriftSched hot path computes, written from
+ * /root/reference/PAPER.md and SURVEY.md §8(c) (the binding readings of the paper; listed in
+ * DESIGN.md §4). Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+ * reference legs may build, load or call anything in this directory. It shares no code, header,
+ * table or constant generator with the CUDA path (paper_2606_02982_b200/csrc, include/): the
+ * structs below are re-declared here on purpose.
+ *
+ * All pointers are HOST pointers. All time is int64 microsecond ticks. Return 0 on success,
+ * -1 on a contract violation.
+ */
+#ifndef DRIFTSCHED_ORACLE_H
+#define DRIFTSCHED_ORACLE_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct {
+  int64_t n_traces;
+  const int64_t* trace_off;    /* [n_traces+1] */
+  const int64_t* arrival_tick; /* non-decreasing inside a trace */
+  const uint8_t* tier;         /* 0 Premium 1 Standard 2 Batch */
+  const int32_t* words;
+  const int32_t* tokens;
+  const int32_t* out_len;      /* >= 1 */
+} oracle_traces;
+
+typedef struct {
+  int32_t max_batch;
+  int64_t kv_budget;           /* <= 0: unlimited */
+  int64_t c_base, c_batch, c_ctx, c_prefill;
+  int32_t weight[3];
+  int64_t aging_step;
+  int32_t traj_every;
+} oracle_server;
+
+typedef struct { int32_t trace, policy, estimator, _pad; double ema_alpha; } oracle_instance;
+
+/* PAPER.md:35,114 (split() proxy vs tokenizer-aware count); SURVEY.md §8(c) C.1. */
+int oracle_characterize(const uint8_t* bytes, int64_t n_bytes, const int64_t* offsets, int64_t n_prompts,
+                        int32_t* words_out, int32_t* tokens_out);
+
+/* PAPER.md:171-181 (tier queues), 201-242 (policies), 278-286 (Eq. 5/6 EMA); SURVEY.md §8(c) C.2. */
+int oracle_simulate(const oracle_traces* tr, const oracle_server* sv, const oracle_instance* inst, int64_t n_inst,
+                    const int64_t* out_off, int64_t* start_tick, int64_t* done_tick,
+                    double* ema_final /*[n_inst*3]*/,
+                    const int64_t* traj_off /*nullable; [n_inst+1] sample ranges*/, double* ema_traj /*nullable; [samples][3]*/);
+
+/* PAPER.md:270 (queue wait vs end-to-end latency). seg outputs nullable. */
+int oracle_latencies(const oracle_traces* tr, const oracle_instance* inst, int64_t n_inst, const int64_t* out_off,
+                     const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, const int64_t* t_mid,
+                     int64_t* e2e, int64_t* qdelay, int32_t* seg_tier, int32_t* seg_all);
+
+/* PAPER.md:436 (P50/P95/P99 tables), reading A13 (nearest rank). */
+int oracle_tail_stats(const int64_t* values, const int32_t* seg_id, int64_t n, int32_t n_segments,
+                      const int32_t* pct, int32_t n_pct, int64_t* out, int64_t* count_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,206 @@
+"""Invariants I1-I9 and brute force over orderings for oracle.simulate (SURVEY.md §8(c) 'Pins')."""
+import itertools
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_02982_b200 import workload as wl
+from _simutil import run_oracle, server, service_time
+
+
+@pytest.fixture(scope="module")
+def small():
+    # 6 traces x 400 requests shaped like configs[1], all 5 policies x both estimators
+    return wl.config1(oracle.characterize, n_traces=6, n_req=400, seed=5)
+
+
+@pytest.fixture(scope="module")
+def small_out(small):
+    c = small
+    return oracle.simulate(c.trace_off, c.arrival, c.tier, c.words, c.tokens, c.out_len, c.server, c.instances)
+
+
+def _per_inst(c, arr):
+    return arr.reshape(c.n_inst, c.n_req)
+
+
+def test_i1_conservation_and_ordering(small, small_out):
+    c = small
+    st, dn, _ = small_out
+    assert (st >= 0).all() and (dn >= 0).all()          # every request started and finished exactly once
+    a = c.arrival.reshape(c.n_traces, c.n_req)[c.instances["trace"]]
+    S, D = _per_inst(c, st), _per_inst(c, dn)
+    assert (a <= S).all() and (S < D).all()
+    # a request holds a slot for exactly O iterations, each >= c_base + c_batch ticks
+    O = c.out_len.reshape(c.n_traces, c.n_req)[c.instances["trace"]]
+    assert (D - S >= O * (c.server.c_base + c.server.c_batch)).all()
+
+
+def test_i2_batch_limit(small, small_out):
+    c = small
+    st, dn, _ = small_out
+    S, D = _per_inst(c, st), _per_inst(c, dn)
+    for i in range(c.n_inst):
+        ev = np.concatenate([np.stack([S[i], np.ones_like(S[i])], 1), np.stack([D[i], -np.ones_like(D[i])], 1)])
+        ev = ev[np.lexsort((ev[:, 1], ev[:, 0]))]        # completions (-1) before starts (+1) at the same tick
+        assert np.cumsum(ev[:, 1]).max() <= c.server.max_batch
+
+
+def test_i3_i4_fifo_and_within_tier_order(small, small_out):
+    c = small
+    st, _, _ = small_out
+    S = _per_inst(c, st)
+    tier = c.tier.reshape(c.n_traces, c.n_req)
+    for i, ins in enumerate(c.instances):
+        if ins["policy"] == wl.FIFO:
+            assert (np.diff(S[i]) >= 0).all()            # I3 ("strictly in arrival order")
+        if ins["policy"] != wl.SJF:
+            for t in range(3):                           # I4 (PAPER.md:228-230 FIFO inside each tier)
+                assert (np.diff(S[i][tier[ins["trace"]] == t]) >= 0).all()
+
+
+def test_priority_tier_ordering_qualitative():
+    # PAPER.md Table VIII (507-525): under Priority queue wait Premium << Standard << Batch; FIFO about equal;
+    # Weighted in between. Needs real contention: overloaded server (rho 1.3), queue delay.
+    sv = wl.Server(max_batch=32, kv_budget=16384)
+    c = wl._trace_workload("x", 5, 6, 400, sv, [(p, wl.EXACT, 0.0) for p in wl.ALL_POLICIES], oracle.characterize, rho=1.3)
+    st, dn, _ = oracle.simulate(c.trace_off, c.arrival, c.tier, c.words, c.tokens, c.out_len, c.server, c.instances)
+    a = c.arrival.reshape(c.n_traces, c.n_req)[c.instances["trace"]]
+    qd = _per_inst(c, st) - a
+    tier = c.tier.reshape(c.n_traces, c.n_req)[c.instances["trace"]]
+    means = {pol: [qd[c.instances["policy"] == pol][tier[c.instances["policy"] == pol] == t].mean() for t in range(3)]
+             for pol in range(5)}
+    p = means[wl.PRIORITY]
+    assert p[0] * 3 < p[1] and p[1] * 3 < p[2]
+    f = means[wl.FIFO]
+    assert max(f) / min(f) < 1.15
+    w = means[wl.WEIGHTED]
+    assert p[0] < w[0] < f[0] and f[2] < w[2] < p[2]
+    # SJF lowers the aggregate queue wait when the key is informative
+    assert qd[c.instances["policy"] == wl.SJF].mean() < qd[c.instances["policy"] == wl.FIFO].mean()
+
+
+def test_i6_makespan_policy_independent_single_server():
+    rng = np.random.default_rng(2)
+    n = 40
+    req = np.stack([np.sort(rng.integers(0, 300_000, n)), rng.integers(0, 3, n), rng.integers(1, 50, n),
+                    rng.integers(1, 200, n), rng.integers(1, 40, n)], 1)
+    sv = server()
+    ends, busy = set(), []
+    for pol in range(5):
+        for est in (wl.SPLIT, wl.EXACT):
+            st, dn, _ = run_oracle(req, sv, pol, est, 0.1)
+            ends.add(int(dn.max()))
+            assert np.array_equal(dn - st, [service_time(int(p), int(o), sv) for p, o in req[:, 3:5]])
+            busy.append(sorted((dn - st).tolist()))
+    assert len(ends) == 1 and all(b == busy[0] for b in busy)
+
+
+def test_i8_tier_relabelling():
+    rng = np.random.default_rng(4)
+    n = 60
+    req = np.stack([np.sort(rng.integers(0, 100_000, n)), rng.integers(0, 3, n), rng.integers(1, 50, n),
+                    rng.integers(1, 200, n), rng.integers(1, 40, n)], 1)
+    req2 = req.copy()
+    req2[:, 1] = (req[:, 1] + 1) % 3
+    sv = server(max_batch=4, kv_budget=600)
+    for pol, est in ((wl.FIFO, wl.EXACT), (wl.SJF, wl.EXACT), (wl.FIFO, wl.SPLIT)):
+        a, b = run_oracle(req, sv, pol, est, 0.0), run_oracle(req2, sv, pol, est, 0.0)
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+def test_i9_degenerate_equivalences():
+    rng = np.random.default_rng(6)
+    n = 80
+    req = np.stack([np.sort(rng.integers(0, 200_000, n)), rng.integers(0, 3, n), rng.integers(1, 50, n),
+                    rng.integers(1, 200, n), rng.integers(1, 40, n)], 1)
+    sv = server(max_batch=3, aging_step=10**15)
+    a, p = run_oracle(req, sv, wl.AGING), run_oracle(req, sv, wl.PRIORITY)
+    assert np.array_equal(a[0], p[0]) and np.array_equal(a[1], p[1])     # huge aging step == PRIORITY
+    one = req.copy()
+    one[:, 1] = 1
+    f = run_oracle(one, sv, wl.FIFO)
+    for pol in (wl.WEIGHTED, wl.PRIORITY, wl.AGING):
+        x = run_oracle(one, sv, pol)
+        assert np.array_equal(x[0], f[0]) and np.array_equal(x[1], f[1])  # single-tier trace == FIFO
+
+
+def test_kv_budget_never_binds_equals_unlimited_and_tiny_budget_serialises():
+    rng = np.random.default_rng(8)
+    n = 50
+    req = np.stack([np.sort(rng.integers(0, 50_000, n)), rng.integers(0, 3, n), rng.integers(1, 50, n),
+                    rng.integers(1, 200, n), rng.integers(1, 40, n)], 1)
+    big, unl, tiny = server(max_batch=8, kv_budget=10**12), server(max_batch=8, kv_budget=0), server(max_batch=8, kv_budget=1)
+    for pol in range(5):
+        a, b = run_oracle(req, big, pol), run_oracle(req, unl, pol)
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+        st, dn, _ = run_oracle(req, tiny, pol)      # est>=1 never fits next to a running request: one at a time
+        order = np.argsort(st, kind="stable")
+        assert (st[order][1:] >= dn[order][:-1]).all()
+
+
+def _policy_order_direct(req, pol, sv, now):
+    idx = list(range(len(req)))
+    if pol == wl.FIFO:
+        return idx
+    if pol == wl.PRIORITY:
+        return sorted(idx, key=lambda r: (req[r][1], r))
+    if pol == wl.SJF:
+        return sorted(idx, key=lambda r: (req[r][3], r))
+    raise AssertionError
+
+
+@pytest.mark.parametrize("n", [2, 3, 4, 5, 6])
+def test_brute_force_orderings(n):
+    # all n requests queued behind a running head request; max_batch=1 (SURVEY.md 'Brute force (<=6 queued)')
+    rng = np.random.default_rng(100 + n)
+    sv = server(aging_step=10**12)
+    for trial in range(6):
+        q = np.stack([np.zeros(n, np.int64), rng.integers(0, 3, n), rng.integers(1, 9, n), rng.integers(1, 30, n),
+                      np.full(n, 3)], 1)
+        for pol in (wl.FIFO, wl.PRIORITY, wl.SJF):
+            st, dn, _ = run_oracle(q, sv, pol, wl.EXACT)
+            # request 0 is admitted first at tick 0 whatever the policy says about the others? No: all arrive at
+            # tick 0, so the policy orders all n.
+            assert np.argsort(st, kind="stable").tolist() == _policy_order_direct(q.tolist(), pol, sv, 0)
+        # WEIGHTED: direct simulation of the slot pattern PPPPSSB
+        st, _, _ = run_oracle(q, sv, wl.WEIGHTED, wl.EXACT)
+        pattern, cur, left, order = [0, 0, 0, 0, 1, 1, 2], 0, list(range(n)), []
+        while left:
+            for s in range(7):
+                pos = (cur + s) % 7
+                cand = [r for r in left if q[r][1] == pattern[pos]]
+                if cand:
+                    order.append(cand[0]); left.remove(cand[0]); cur = (pos + 1) % 7
+                    break
+        assert np.argsort(st, kind="stable").tolist() == order
+        # SJF + EXACT with equal O minimises sum(done) over all n! orders (closed form (i))
+        st, dn, _ = run_oracle(q, sv, wl.SJF, wl.EXACT)
+        S = [service_time(int(p), 3, sv) for p in q[:, 3]]
+        best = min(sum(itertools.accumulate(S[i] for i in perm)) for perm in itertools.permutations(range(n)))
+        assert int(dn.sum()) == best
+
+
+def test_aging_brute_force_against_direct_key():
+    # queued requests with different waits: AGING order = repeated argmin of (max(0,tier-floor(wait/step)), seq)
+    rng = np.random.default_rng(77)
+    sv = server(aging_step=3000)
+    for trial in range(20):
+        n = 6
+        head = [[0, 0, 1, int(rng.integers(500, 3000)), 1]]
+        arr = np.sort(rng.integers(1, 9000, n))
+        q = [[int(arr[i]), int(rng.integers(0, 3)), 1, int(rng.integers(1, 400)), 1] for i in range(n)]
+        req = head + q
+        st, dn, _ = run_oracle(req, sv, wl.AGING)
+        now, left, order = service_time(head[0][3], 1, sv), list(range(1, n + 1)), []
+        while left:
+            avail = [r for r in left if req[r][0] <= now]
+            if not avail:
+                now = min(req[r][0] for r in left)
+                continue
+            r = min(avail, key=lambda r: (max(0, req[r][1] - (now - req[r][0]) // 3000), r))
+            order.append(r); left.remove(r)
+            assert st[r] == now
+            now += service_time(req[r][3], 1, sv)
+        assert len(order) == n

@@ -1,0 +1,155 @@
+"""Pins for oracle.simulate: hand-worked traces H1-H6, EMA bit pattern H3, closed forms."""
+import json
+import math
+import os
+import struct
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_02982_b200 import workload as wl
+from _simutil import run_oracle, server, service_time
+
+
+def _golden(golden_dir):
+    return json.load(open(os.path.join(golden_dir, "hand_traces.json")))
+
+
+def test_hand_traces(golden_dir):
+    g = _golden(golden_dir)
+    assert len(g["cases"]) == 12
+    for c in g["cases"]:
+        sv = server(**c["server"])
+        if "weight" in c["server"]:
+            sv.weight = tuple(c["server"]["weight"])
+        st, dn, ema = run_oracle(c["req"], sv, c["policy"], c["estimator"], c["alpha"])
+        assert st.tolist() == c["start"], c["name"]
+        assert dn.tolist() == c["done"], c["name"]
+
+
+def test_h3_ema_bit_pattern(golden_dir):
+    g = _golden(golden_dir)
+    # the bit pattern is fixed by IEEE-754 arithmetic, independent of the oracle:
+    m = 4.0 / 3.0
+    b = (1.0 - 0.1) * 1.0 + 0.1 * m
+    assert hex(struct.unpack("<Q", struct.pack("<d", b))[0]).upper() == g["H3_ema"]["B_std_bits"].upper()
+    # one Standard request completes -> B[Std] is exactly that, others untouched
+    st, dn, ema = run_oracle([[0, 1, 3, 4, 2]], server(), wl.SJF, wl.SPLIT, 0.1)
+    bits = struct.unpack("<Q", struct.pack("<d", ema[0, 1]))[0]
+    assert bits == int(g["H3_ema"]["B_std_bits"], 16)
+    assert ema[0, 0] == 1.0 and ema[0, 2] == 1.0
+    # H2 with SPLIT: r1/r2 arrive before r0 completes -> est frozen at 8 and 2 (B=1.0), SJF picks r2 first
+    c = [x for x in g["cases"] if x["name"].startswith("H2/H3")][0]
+    st, dn, ema = run_oracle(c["req"], server(), wl.SJF, wl.SPLIT, 0.1)
+    assert st.tolist() == c["start"]
+    # after all three: Std saw m=4/3, Prem m=10/8, Batch m=3/2, one update each
+    assert ema[0].tolist() == [(1.0 - 0.1) * 1.0 + 0.1 * (10 / 8), b, (1.0 - 0.1) * 1.0 + 0.1 * (3 / 2)]
+
+
+def test_h4_round_robin_variant():
+    # weights {1,1,1}: r0 Prem running, then queued r1 Prem, r2 Std, r3 Batch -> WEIGHTED serves r2, r3, r1
+    req = [[0, 0, 1, 1, 1], [10, 0, 1, 1, 1], [20, 1, 1, 1, 1], [30, 2, 1, 1, 1]]
+    sv = server(weight=(1, 1, 1))
+    st, _, _ = run_oracle(req, sv, wl.WEIGHTED)
+    assert np.argsort(st).tolist() == [0, 2, 3, 1]
+    for pol in (wl.FIFO, wl.PRIORITY):
+        st, _, _ = run_oracle(req, sv, pol)
+        assert np.argsort(st).tolist() == [0, 1, 2, 3]
+
+
+def test_closed_form_service_time_single_request():
+    sv = server()
+    rng = np.random.default_rng(3)
+    for _ in range(50):
+        P, O = int(rng.integers(0, 500)), int(rng.integers(1, 300))
+        st, dn, _ = run_oracle([[17, 1, 5, P, O]], sv, wl.FIFO)
+        assert st[0] == 17 and dn[0] - st[0] == service_time(P, O, sv)
+    assert service_time(3, 2, sv) == 4322  # SURVEY.md check: 2168 + 2154
+
+
+def _queue_trace(n, mean_service, rho, seed, exponential):
+    rng = np.random.default_rng(seed)
+    P = np.maximum(0, np.rint(rng.exponential(mean_service, n))).astype(np.int64) if exponential \
+        else np.full(n, int(mean_service), np.int64)
+    ia = np.maximum(0, np.rint(rng.exponential(mean_service / rho, n))).astype(np.int64)
+    arr = np.cumsum(ia)
+    req = np.stack([arr, np.ones(n, np.int64), P, P, np.ones(n, np.int64)], axis=1)
+    return req
+
+
+@pytest.mark.parametrize("rho", [0.5, 0.8])
+def test_mm1_mean_wait(rho):
+    # M/M/1 FIFO: Wq = rho/(mu-lambda); degenerate server c_prefill=1, everything else 0, O=1 (closed form (ii))
+    n, mean_s = 1_000_000, 100_000.0
+    sv = server(c_base=0, c_batch=0, c_ctx=0, c_prefill=1)
+    req = _queue_trace(n, mean_s, rho, 5, True)
+    st, dn, _ = run_oracle(req, sv, wl.FIFO)
+    assert np.array_equal(dn - st, req[:, 3])           # service time = P ticks exactly
+    wq = (st - req[:, 0]).mean()
+    mu, lam = 1.0 / mean_s, rho / mean_s
+    assert abs(wq / (rho / (mu - lam)) - 1.0) < 0.02
+
+
+def test_md1_mean_wait():
+    # Pollaczek-Khinchine, constant service: Wq = rho/(2 mu (1-rho)) (closed form (iii))
+    n, mean_s, rho = 400_000, 50_000.0, 0.7
+    sv = server(c_base=0, c_batch=0, c_ctx=0, c_prefill=1)
+    req = _queue_trace(n, mean_s, rho, 9, False)
+    st, dn, _ = run_oracle(req, sv, wl.FIFO)
+    wq = (st - req[:, 0]).mean()
+    assert abs(wq / (rho * mean_s / (2 * (1 - rho))) - 1.0) < 0.02
+
+
+def test_sjf_beats_fifo_statistically_mg1():
+    # C-SJF (ii): O=1, S = c_prefill*P, Poisson arrivals, 1e5 requests, rho 0.8: mean wait SJF < FIFO
+    n, mean_s, rho = 100_000, 20_000.0, 0.8
+    sv = server(c_base=0, c_batch=0, c_ctx=0, c_prefill=1)
+    req = _queue_trace(n, mean_s, rho, 13, True)
+    w = {}
+    for pol in (wl.FIFO, wl.SJF):
+        st, dn, _ = run_oracle(req, sv, pol)
+        w[pol] = (st - req[:, 0]).mean()
+    assert w[wl.SJF] < 0.8 * w[wl.FIFO]
+
+
+@pytest.mark.parametrize("alpha", [0.05, 0.1, 0.5, 1.0])
+def test_ema_geometric_closed_form(alpha):
+    # constant ratio m=P/W: B_k = m + (1-m)(1-alpha)^k (closed form (iv)); trajectory sampled every completion
+    k = 60
+    req = [[i * 10_000_000, 1, 4, 6, 1] for i in range(k)]   # far apart: one completion at a time, m = 1.5
+    sv = server(traj_every=1)
+    st, dn, ema, traj = run_oracle(req, sv, wl.FIFO, wl.SPLIT, alpha, want_traj=True)
+    assert traj.shape == (k, 3)
+    for i in range(k):
+        expect = 1.5 + (1 - 1.5) * (1 - alpha) ** (i + 1)
+        assert abs(traj[i, 1] / expect - 1) < 1e-14
+        assert traj[i, 0] == 1.0 and traj[i, 2] == 1.0
+    assert ema[0, 1] == traj[-1, 1]
+
+
+def test_ema_exact_estimator_stays_one_and_alpha_zero():
+    cfg = wl.config0(oracle.characterize)
+    for alpha in (0.0, 0.05, 0.1, 0.3, 0.7, 1.0):
+        inst = np.zeros(1, wl.INSTANCE_DTYPE)
+        inst[0] = (0, wl.SJF, wl.EXACT, 0, alpha)
+        _, _, ema = oracle.simulate(cfg.trace_off, cfg.arrival, cfg.tier, cfg.words, cfg.tokens, cfg.out_len,
+                                    cfg.server, inst)
+        assert (ema == 1.0).all()          # (v) EXACT => B == 1.0 bit-exactly (A4)
+    inst[0] = (0, wl.SJF, wl.SPLIT, 0, 0.0)   # I7: alpha=0 => BIAS OFF
+    _, _, ema = oracle.simulate(cfg.trace_off, cfg.arrival, cfg.tier, cfg.words, cfg.tokens, cfg.out_len, cfg.server, inst)
+    assert (ema == 1.0).all()
+
+
+def test_ema_converges_to_token_word_ratio():
+    # stationary drift: time-average of B -> E[P/W] = 1.3977 (north_star invariant; Fig. 5 shows the
+    # same convergence of the bias factor on the real testbed)
+    cfg = wl.config1(oracle.characterize, n_traces=1, n_req=4000, seed=21)
+    cfg.server.traj_every = 1
+    inst = np.zeros(1, wl.INSTANCE_DTYPE)
+    inst[0] = (0, wl.FIFO, wl.SPLIT, 0, 0.05)
+    _, _, ema, traj = oracle.simulate(cfg.trace_off, cfg.arrival, cfg.tier, cfg.words, cfg.tokens, cfg.out_len,
+                                      cfg.server, inst, want_traj=True)
+    assert traj.shape == (4000, 3)
+    assert np.abs(traj[1000:].mean(axis=0) - 1.3977).max() < 0.02
+    assert np.abs(ema[0] - 1.3977).max() < 0.08
