@@ -1,0 +1,158 @@
+/* driftsched.h — C ABI of the B200-native DriftSched evaluation hot path (libdriftsched.so).
+ *
+ * The library evaluates LLM-serving scheduling policies in bulk, following the problem statement of
+ * "DriftSched" (arxiv/paper_2606_02982; text in /root/reference/PAPER.md) as instantiated by
+ * BASELINE.json and SURVEY.md §8:
+ *   (a) ds_characterize : admission-time workload characterization of packed prompt text,
+ *   (b) ds_simulate     : tick-exact simulation of tier queues x scheduling policy x continuous-batching
+ *                         server model x per-tier EMA calibration, one instance per warp,
+ *   (c) ds_latencies + ds_tail_stats : queue wait / end-to-end latency and their percentiles.
+ *
+ * Conventions (all entry points)
+ *  - extern "C"; plain pointers and sizes; no C++/torch types.
+ *  - Every function returns int: DS_OK (0) or a negative DS_E* code. No exception or abort crosses the ABI.
+ *  - Unless a parameter says "host", every data pointer is a DEVICE pointer owned by the caller
+ *    (allocate with cudaMalloc / torch). The library never frees or retains caller memory.
+ *  - Descriptor structs (ds_traces, ds_server) are passed by HOST pointer and read during the call;
+ *    the arrays they point to are device arrays.
+ *  - Work is enqueued on the caller's stream (`stream` is a cudaStream_t passed as void*; NULL = default
+ *    stream). Calls do not synchronise. Host-checkable arguments fail immediately with DS_EINVAL;
+ *    device-side contract violations (non-monotone offsets, tier > 2, out_len < 1, decreasing arrivals,
+ *    key overflow) set a sticky device status word, read (with a stream sync) by ds_device_status().
+ *  - Scratch memory comes from a caller-supplied workspace; query its size with ds_workspace_bytes().
+ *    Workspace contents are undefined on entry and exit; two calls in flight need two workspaces.
+ *  - There is no CPU fallback: every function fails with DS_ECUDA if no CUDA device is usable.
+ */
+#ifndef DRIFTSCHED_H
+#define DRIFTSCHED_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DS_OK 0
+#define DS_EINVAL (-1) /* bad argument / host-checkable contract violation */
+#define DS_ECUDA (-2)  /* CUDA runtime error (see ds_last_cuda_error) */
+#define DS_ENOMEM (-3) /* workspace too small */
+
+/* bits of the device status word (ds_device_status) */
+#define DS_DEV_BAD_OFFSETS 1u  /* ds_characterize: offsets not in [0,n_bytes] or decreasing */
+#define DS_DEV_BAD_TRACE 2u    /* ds_simulate: tier > 2, out_len < 1, words/tokens < 0 or arrivals decreasing */
+#define DS_DEV_KEY_RANGE 4u    /* ds_simulate: SJF key overflow (est >= 2^39 or trace longer than 2^24) */
+#define DS_DEV_BAD_INSTANCE 8u /* ds_simulate: instance field out of range */
+
+/* ---------------------------------------------------------------------------------------------- (a)
+ * Workload characterization ("whitespace-delimited word counts" vs
+ * "tokenizer-aware" accounting; Table III). Definition: SURVEY.md §8(c) C.1.
+ *   WS     = {0x09,0x0A,0x0B,0x0C,0x0D,0x20}  (Python bytes.split())
+ *   PUNCT  = 0x21-0x2F, 0x3A-0x40, 0x5B-0x60, 0x7B-0x7E
+ *   LETTER = every other byte value
+ * For prompt i = bytes[offsets[i], offsets[i+1]) taken as an isolated string:
+ *   words_out[i]  = number of maximal runs of non-WS bytes                      (the split() proxy)
+ *   tokens_out[i] = sum over maximal LETTER runs of ceil(len/4) + number of PUNCT bytes
+ *                   (BASELINE.json:configs[0] pseudo-token rule standing in for the model tokenizer)
+ * bytes   [n_bytes]      device, any alignment (16-byte alignment is fastest)
+ * offsets [n_prompts+1]  device, 0 <= offsets[0], non-decreasing, offsets[n_prompts] <= n_bytes
+ * words_out, tokens_out [n_prompts] device, overwritten.
+ * workspace: ds_workspace_bytes(DS_WS_CHARACTERIZE, n_bytes, n_prompts).
+ * Launches: 1 memset + 1 kernel. */
+int ds_characterize(const uint8_t* bytes, int64_t n_bytes, const int64_t* offsets, int64_t n_prompts,
+                    int32_t* words_out, int32_t* tokens_out, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------------------- (b) */
+typedef struct {              /* SoA request records, traces concatenated; HOST struct, DEVICE arrays */
+  int64_t n_traces;
+  const int64_t* trace_off;    /* [n_traces+1] request index range of each trace */
+  const int64_t* arrival_tick; /* microsecond ticks, >= 0, non-decreasing inside a trace */
+  const uint8_t* tier;         /* 0 Premium, 1 Standard, 2 Batch */
+  const int32_t* words;        /* split() count, >= 0 */
+  const int32_t* tokens;       /* pseudo-token count = true prompt length, >= 0 */
+  const int32_t* out_len;      /* decode length, >= 1 */
+} ds_traces;
+
+typedef struct {              /* continuous-batching server model, BASELINE.json:configs[0] */
+  int32_t max_batch;           /* 1..256 */
+  int64_t kv_budget;           /* tokens; <= 0 means unlimited */
+  int64_t c_base, c_batch, c_ctx, c_prefill; /* iteration cost = c_base + c_batch*b + c_ctx*sum(ctx) + c_prefill*sum(P_new) */
+  int32_t weight[3];           /* Weighted policy slots per tier, each >= 1: {4,2,1} configs, {5,3,2} PAPER.md:234 */
+  int64_t aging_step;          /* ticks waited per promoted tier level, >= 1 */
+  int32_t traj_every;          /* 0 = no EMA trajectory; k = sample B[0..2] every k completions */
+} ds_server;
+
+#define DS_FIFO 0
+#define DS_PRIORITY 1
+#define DS_WEIGHTED 2
+#define DS_SJF 3
+#define DS_AGING 4
+#define DS_SPLIT 0    /* estimate base = words  (split() proxy) */
+#define DS_EXACT 1    /* estimate base = tokens (tokenizer-aware) */
+
+typedef struct {
+  int32_t trace;     /* index into ds_traces */
+  int32_t policy;    /* DS_FIFO .. DS_AGING */
+  int32_t estimator; /* DS_SPLIT / DS_EXACT */
+  int32_t _pad;
+  double ema_alpha;  /* EMA learning rate in [0,1] (Eq. 5); 0 = BIAS OFF */
+} ds_instance;
+
+/* Simulate n_inst independent (trace, policy, estimator, alpha) instances, one warp each.
+ * Algorithm: SURVEY.md §8(c) C.2 (LOOP steps 1-6, readings A1-A14, R-ORD), summarised in DESIGN.md §3.
+ *   est = ceil(B[tier]*base) frozen at arrival (Eq. 1-2 reduced);
+ *   EMA on completion: m=P/base; B = (1-a)*B + a*m in fp64, four separately rounded operations.
+ * inst        [n_inst]            device
+ * out_off     [n_inst+1]          device; instance i writes start/done at out_off[i] + local request index
+ * start_tick, done_tick           device, int64, sized out_off[n_inst]; done_tick is also used as scratch
+ *                                 for the frozen estimates while a request is queued
+ * ema_final   [n_inst*3]          device, fp64 B[tier] at the end of the run
+ * traj_off    [n_inst+1] nullable device; instance i owns trajectory samples [traj_off[i], traj_off[i+1]),
+ *                                 floor(n_req_i / traj_every) of them
+ * ema_traj    [traj_off[n_inst]*3] nullable device fp64
+ * workspace: ds_workspace_bytes(DS_WS_SIMULATE, total_requests_over_instances, n_inst).
+ * Launches: 1 memset (work counter + status) + 1 kernel. */
+int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
+                const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
+                const int64_t* traj_off, double* ema_traj, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------------------- (c)
+ * Latency derivation (worker timestamps separate queueing from inference):
+ *   e2e = done - arrival, qdelay = start - arrival, per simulated request (same indexing as start/done).
+ * Segment ids for ds_tail_stats, with g = group[i] (nullable -> 0) and, if t_mid != NULL,
+ *   g = 2*g + (arrival >= t_mid[trace]) (pre/post-drift phase, BASELINE.json:configs[4]):
+ *   seg_tier = 3*g + tier (per-tier statistics), seg_all = g (overall). Either seg output may be NULL.
+ * n_total = out_off[n_inst] must be passed by the caller (host value). Launches: 1 kernel. */
+int ds_latencies(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t n_total,
+                 const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, const int64_t* t_mid,
+                 int64_t* e2e, int64_t* qdelay, int32_t* seg_tier, int32_t* seg_all, void* stream);
+
+/* Segmented percentiles by MSB-first radix select (PAPER.md:436 P50/P95/P99; Tables VI-VIII).
+ * For each segment s in [0,n_segments): the values[i] with seg_id[i]==s, sorted ascending; for each pct p the
+ * nearest-rank element, rank = max(1, ceil(p*n_s/100)). seg_id outside [0,n_segments)
+ * (e.g. -1) is skipped. out[s*n_pct+q] = -1 for an empty segment. count_out (nullable) [n_segments].
+ * pct is a HOST array of n_pct values in [0,100], n_pct <= 8.
+ * workspace: ds_workspace_bytes(DS_WS_TAIL_STATS, n_segments, n_pct). Launches: 1 memset + up to 9 x 2 kernels. */
+int ds_tail_stats(const int64_t* values, const int32_t* seg_id, int64_t n, int32_t n_segments, const int32_t* pct,
+                  int32_t n_pct, int64_t* out, int64_t* count_out, void* workspace, size_t workspace_bytes, void* stream);
+
+#define DS_WS_CHARACTERIZE 0
+#define DS_WS_SIMULATE 1
+#define DS_WS_TAIL_STATS 2
+/* Workspace size in bytes for call `which` with the two size arguments named at that call. Never 0. */
+size_t ds_workspace_bytes(int which, int64_t n, int64_t m);
+
+/* Synchronises `stream`, returns the sticky device status word (0 = all contracts held) and clears it.
+ * Negative on CUDA error. */
+int ds_device_status(void* stream);
+
+const char* ds_strerror(int code);
+/* Text of the last CUDA error seen by this thread inside the library ("" if none). */
+const char* ds_last_cuda_error(void);
+/* Number of kernel launches (memsets not counted) issued by the library in this process since load. */
+int64_t ds_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DRIFTSCHED_H */

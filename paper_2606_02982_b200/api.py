@@ -1,0 +1,137 @@
+"""Same-name Python wrappers of the C ABI (include/driftsched.h): argument marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+import torch
+
+from . import _lib
+from ._lib import DsServer, DsTraces, check, lib
+
+INSTANCE_BYTES = 24
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _need_cuda(*ts):
+    for t in ts:
+        if t is not None and (not t.is_cuda or not t.is_contiguous()):
+            raise ValueError("driftsched: tensors must be contiguous CUDA tensors (no CPU fallback)")
+
+
+def workspace_bytes(which, n, m):
+    return int(lib().ds_workspace_bytes(which, int(n), int(m)))
+
+
+def _workspace(which, n, m, device):
+    return torch.empty(workspace_bytes(which, n, m), dtype=torch.uint8, device=device)
+
+
+def launch_count():
+    return int(lib().ds_launch_count())
+
+
+def device_status():
+    rc = lib().ds_device_status(_stream())
+    if rc < 0:
+        check("ds_device_status", rc)
+    return rc
+
+
+def characterize(text, offsets, words_out=None, tokens_out=None, workspace=None):
+    """ds_characterize: text uint8[N], offsets int64[n+1] (CUDA) -> (words int32[n], tokens int32[n])."""
+    _need_cuda(text, offsets, words_out, tokens_out)
+    assert text.dtype == torch.uint8 and offsets.dtype == torch.int64
+    n = offsets.numel() - 1
+    if words_out is None:
+        words_out = torch.empty(n, dtype=torch.int32, device=text.device)
+    if tokens_out is None:
+        tokens_out = torch.empty(n, dtype=torch.int32, device=text.device)
+    if workspace is None:
+        workspace = _workspace(_lib.WS_CHARACTERIZE, text.numel(), n, text.device)
+    check("ds_characterize", lib().ds_characterize(_ptr(text), text.numel(), _ptr(offsets), n, _ptr(words_out), _ptr(tokens_out),
+                                                   _ptr(workspace), workspace.numel(), _stream()))
+    return words_out, tokens_out
+
+
+def _traces(trace_off, arrival, tier, words, tokens, out_len):
+    _need_cuda(trace_off, arrival, tier, words, tokens, out_len)
+    assert trace_off.dtype == torch.int64 and arrival.dtype == torch.int64 and tier.dtype == torch.uint8
+    assert words.dtype == torch.int32 and tokens.dtype == torch.int32 and out_len.dtype == torch.int32
+    return DsTraces(trace_off.numel() - 1, trace_off.data_ptr(), arrival.data_ptr(), tier.data_ptr(), words.data_ptr(),
+                    tokens.data_ptr(), out_len.data_ptr())
+
+
+def _server(sv):
+    return DsServer(sv.max_batch, sv.kv_budget, sv.c_base, sv.c_batch, sv.c_ctx, sv.c_prefill, (C.c_int32 * 3)(*sv.weight),
+                    sv.aging_step, sv.traj_every)
+
+
+def instances_to_device(instances: np.ndarray, device):
+    """numpy structured ds_instance array -> uint8 CUDA tensor with the same bytes."""
+    assert instances.dtype.itemsize == INSTANCE_BYTES
+    return torch.from_numpy(np.ascontiguousarray(instances).view(np.uint8).copy()).to(device)
+
+
+def simulate(trace_off, arrival, tier, words, tokens, out_len, server, inst, out_off, n_total, start=None, done=None,
+             ema_final=None, traj_off=None, ema_traj=None, workspace=None):
+    """ds_simulate. inst: uint8 CUDA tensor holding ds_instance[n_inst]; out_off int64[n_inst+1] (CUDA);
+    n_total = out_off[-1] (host int). Returns (start_tick, done_tick, ema_final[n_inst,3])."""
+    tr = _traces(trace_off, arrival, tier, words, tokens, out_len)
+    sv = _server(server)
+    _need_cuda(inst, out_off, start, done, ema_final, traj_off, ema_traj)
+    n_inst = inst.numel() // INSTANCE_BYTES
+    dev = arrival.device
+    if start is None:
+        start = torch.empty(n_total, dtype=torch.int64, device=dev)
+    if done is None:
+        done = torch.empty(n_total, dtype=torch.int64, device=dev)
+    if ema_final is None:
+        ema_final = torch.empty((n_inst, 3), dtype=torch.float64, device=dev)
+    if workspace is None:
+        workspace = _workspace(_lib.WS_SIMULATE, n_total, n_inst, dev)
+    check("ds_simulate", lib().ds_simulate(C.byref(tr), C.byref(sv), _ptr(inst), n_inst, _ptr(out_off), _ptr(start), _ptr(done),
+                                           _ptr(ema_final), _ptr(traj_off), _ptr(ema_traj), _ptr(workspace), workspace.numel(),
+                                           _stream()))
+    return start, done, ema_final
+
+
+def latencies(trace_off, arrival, tier, words, tokens, out_len, inst, out_off, n_total, start, done, group=None, t_mid=None,
+              want_seg_tier=True, want_seg_all=True):
+    """ds_latencies -> (e2e, qdelay, seg_tier, seg_all)."""
+    tr = _traces(trace_off, arrival, tier, words, tokens, out_len)
+    _need_cuda(inst, out_off, start, done, group, t_mid)
+    n_inst = inst.numel() // INSTANCE_BYTES
+    dev = start.device
+    e2e = torch.empty(n_total, dtype=torch.int64, device=dev)
+    qd = torch.empty(n_total, dtype=torch.int64, device=dev)
+    st = torch.empty(n_total, dtype=torch.int32, device=dev) if want_seg_tier else None
+    sa = torch.empty(n_total, dtype=torch.int32, device=dev) if want_seg_all else None
+    check("ds_latencies", lib().ds_latencies(C.byref(tr), _ptr(inst), n_inst, _ptr(out_off), n_total, _ptr(start), _ptr(done),
+                                             _ptr(group), _ptr(t_mid), _ptr(e2e), _ptr(qd), _ptr(st), _ptr(sa), _stream()))
+    return e2e, qd, st, sa
+
+
+def tail_stats(values, seg_id, n_segments, pct=(50, 99), out=None, count_out=None, workspace=None):
+    """ds_tail_stats -> (out int64[n_segments, n_pct], count int64[n_segments])."""
+    _need_cuda(values, seg_id, out, count_out)
+    assert values.dtype == torch.int64 and seg_id.dtype == torch.int32
+    dev = values.device
+    n_pct = len(pct)
+    if out is None:
+        out = torch.empty((n_segments, n_pct), dtype=torch.int64, device=dev)
+    if count_out is None:
+        count_out = torch.empty(n_segments, dtype=torch.int64, device=dev)
+    if workspace is None:
+        workspace = _workspace(_lib.WS_TAIL_STATS, n_segments, n_pct, dev)
+    arr = (C.c_int32 * n_pct)(*[int(x) for x in pct])
+    check("ds_tail_stats", lib().ds_tail_stats(_ptr(values), _ptr(seg_id), values.numel(), n_segments, arr, n_pct, _ptr(out),
+                                               _ptr(count_out), _ptr(workspace), workspace.numel(), _stream()))
+    return out, count_out

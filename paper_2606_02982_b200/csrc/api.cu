@@ -1,0 +1,81 @@
+// libdriftsched.so: error handling, status word, workspace sizes (include/driftsched.h).
+#include <atomic>
+#include <cstdio>
+#include <cstring>
+
+#include "common.cuh"
+
+namespace ds {
+
+__device__ unsigned int g_status_word = 0;
+
+static thread_local char t_cuda_err[256] = "";
+static std::atomic<long long> g_launches{0};
+
+unsigned int* status_ptr() {
+  static unsigned int* p = nullptr;
+  if (!p) {
+    void* q = nullptr;
+    if (cudaGetSymbolAddress(&q, g_status_word) != cudaSuccess) return nullptr;
+    p = (unsigned int*)q;
+  }
+  return p;
+}
+
+void note_launch(int n) { g_launches += n; }
+
+int cuda_fail(cudaError_t e) {
+  snprintf(t_cuda_err, sizeof(t_cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
+  cudaGetLastError();  // clear non-sticky error state
+  return DS_ECUDA;
+}
+
+// sizes shared with the kernels' own layouts (kept in one place: each .cu exposes its need)
+size_t ws_characterize(int64_t n_bytes, int64_t n_prompts);
+size_t ws_simulate(int64_t total_requests, int64_t n_inst);
+size_t ws_tail_stats(int64_t n_segments, int64_t n_pct);
+
+}  // namespace ds
+
+extern "C" {
+
+size_t ds_workspace_bytes(int which, int64_t n, int64_t m) {
+  size_t b = 0;
+  if (n < 0) n = 0;
+  if (m < 0) m = 0;
+  switch (which) {
+    case DS_WS_CHARACTERIZE: b = ds::ws_characterize(n, m); break;
+    case DS_WS_SIMULATE: b = ds::ws_simulate(n, m); break;
+    case DS_WS_TAIL_STATS: b = ds::ws_tail_stats(n, m); break;
+    default: b = 0;
+  }
+  return b < 256 ? 256 : b;
+}
+
+int ds_device_status(void* stream) {
+  unsigned int* p = ds::status_ptr();
+  if (!p) return ds::cuda_fail(cudaGetLastError());
+  unsigned int h = 0, zero = 0;
+  cudaStream_t s = (cudaStream_t)stream;
+  DS_CUDA(cudaStreamSynchronize(s));
+  DS_CUDA(cudaMemcpyAsync(&h, p, sizeof(h), cudaMemcpyDeviceToHost, s));
+  DS_CUDA(cudaMemcpyAsync(p, &zero, sizeof(zero), cudaMemcpyHostToDevice, s));
+  DS_CUDA(cudaStreamSynchronize(s));
+  return (int)h;
+}
+
+const char* ds_strerror(int code) {
+  switch (code) {
+    case DS_OK: return "ok";
+    case DS_EINVAL: return "invalid argument";
+    case DS_ECUDA: return "CUDA runtime error";
+    case DS_ENOMEM: return "workspace too small";
+    default: return "unknown error";
+  }
+}
+
+const char* ds_last_cuda_error(void) { return ds::t_cuda_err; }
+
+int64_t ds_launch_count(void) { return ds::g_launches.load(); }
+
+}  // extern "C"

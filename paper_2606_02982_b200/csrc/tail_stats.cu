@@ -1,0 +1,198 @@
+// K3 — ds_latencies + ds_tail_stats (Tables VI-VIII).
+//
+// ds_tail_stats: segmented nearest-rank percentiles by MSB-first radix select on 8-bit digits. Keys are the
+// values with the sign bit flipped (unsigned order == signed order). Pass 0 counts each segment and reduces
+// AND / OR of all keys: a digit on which every key agrees is skipped (latencies < 2^40 ticks skip 3 of 8).
+// Per digit: histogram kernel (shared-memory privatised when (segments x percentiles x 256) fits, global
+// atomics otherwise) -> select kernel (one thread per (segment, percentile) walks 256 bins, fixes the digit,
+// reduces the rank). Traffic: 12 B per value per non-skipped digit; only keys matching the prefix are counted.
+#include "common.cuh"
+
+namespace ds {
+namespace k3 {
+
+constexpr int kMaxPct = 8;
+constexpr unsigned long long kSign = 0x8000000000000000ull;
+
+struct Ws {               // header at the start of the workspace
+  unsigned long long and_bits, or_bits;
+  unsigned int any;
+};
+// layout: Ws | counts[n_seg] u64 | prefix[n_seg*n_pct] u64 | rank[n_seg*n_pct] u64 | hist[n_seg*n_pct*256] u32
+struct Layout {
+  Ws* hdr; unsigned long long* counts; unsigned long long* prefix; unsigned long long* rank; unsigned int* hist;
+  size_t total;
+};
+inline Layout make_layout(void* base, int64_t n_seg, int64_t n_pct) {
+  Layout L; char* p = (char*)base; size_t o = 0;
+  L.hdr = (Ws*)(p + o); o += 256;
+  L.counts = (unsigned long long*)(p + o); o += align_up(8 * (size_t)n_seg, 256);
+  L.prefix = (unsigned long long*)(p + o); o += align_up(8 * (size_t)(n_seg * n_pct), 256);
+  L.rank = (unsigned long long*)(p + o); o += align_up(8 * (size_t)(n_seg * n_pct), 256);
+  L.hist = (unsigned int*)(p + o); o += align_up(4 * 256 * (size_t)(n_seg * n_pct), 256);
+  L.total = o;
+  return L;
+}
+
+__global__ void latencies_kernel(const int64_t* __restrict__ trace_off, const int64_t* __restrict__ arrival,
+                                 const uint8_t* __restrict__ tier, const ds_instance* __restrict__ inst,
+                                 const int64_t* __restrict__ out_off, const int64_t* __restrict__ start,
+                                 const int64_t* __restrict__ done, const int32_t* __restrict__ group,
+                                 const int64_t* __restrict__ t_mid, int64_t* __restrict__ e2e, int64_t* __restrict__ qd,
+                                 int32_t* __restrict__ seg_tier, int32_t* __restrict__ seg_all) {
+  const long long ii = blockIdx.x;
+  const int t = inst[ii].trace;
+  const long long lo = trace_off[t], n = trace_off[t + 1] - lo, oo = out_off[ii];
+  const int g0 = group ? group[ii] : 0;
+  const bool ph = t_mid != nullptr;
+  const long long tm = ph ? t_mid[t] : 0;
+  for (long long r = threadIdx.x; r < n; r += blockDim.x) {
+    const long long a = arrival[lo + r];
+    e2e[oo + r] = done[oo + r] - a;
+    qd[oo + r] = start[oo + r] - a;
+    const int g = ph ? g0 * 2 + (a >= tm ? 1 : 0) : g0;
+    if (seg_tier) seg_tier[oo + r] = g * 3 + tier[lo + r];
+    if (seg_all) seg_all[oo + r] = g;
+  }
+}
+
+__global__ void count_kernel(const int64_t* __restrict__ v, const int32_t* __restrict__ seg, long long n, int n_seg,
+                             Ws* hdr, unsigned long long* counts) {
+  extern __shared__ unsigned int sc[];   // per-block segment counts when n_seg is small
+  const bool priv = n_seg <= 4096;
+  if (priv) { for (int i = threadIdx.x; i < n_seg; i += blockDim.x) sc[i] = 0; __syncthreads(); }
+  unsigned long long a = ~0ull, o = 0ull; bool any = false;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    const int s = seg[i];
+    if (s < 0 || s >= n_seg) continue;
+    const unsigned long long k = (unsigned long long)v[i] ^ kSign;
+    a &= k; o |= k; any = true;
+    if (priv) atomicAdd(&sc[s], 1u); else atomicAdd(&counts[s], 1ull);
+  }
+  for (int d = 16; d > 0; d >>= 1) { a &= __shfl_xor_sync(0xffffffffu, a, d); o |= __shfl_xor_sync(0xffffffffu, o, d); }
+  const unsigned anym = __ballot_sync(0xffffffffu, any);
+  if ((threadIdx.x & 31) == 0 && anym) { atomicAnd(&hdr->and_bits, a); atomicOr(&hdr->or_bits, o); atomicOr(&hdr->any, 1u); }
+  if (priv) { __syncthreads(); for (int i = threadIdx.x; i < n_seg; i += blockDim.x) if (sc[i]) atomicAdd(&counts[i], (unsigned long long)sc[i]); }
+}
+
+struct Pcts { int p[kMaxPct]; };
+
+__global__ void init_kernel(const unsigned long long* counts, int n_seg, int n_pct, Pcts pc, unsigned long long* prefix,
+                            unsigned long long* rank, int64_t* count_out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_seg * n_pct) return;
+  const int s = i / n_pct, q = i % n_pct;
+  const unsigned long long c = counts[s];
+  unsigned long long r = ((unsigned long long)pc.p[q] * c + 99ull) / 100ull;   // nearest rank (A13)
+  if (r < 1) r = 1;
+  if (r > c) r = c;
+  prefix[i] = 0; rank[i] = r;
+  if (q == 0 && count_out) count_out[s] = (int64_t)c;
+}
+
+// digit d (7 = most significant). Keys whose bits above digit d equal prefix[s,q] are counted in hist[s,q][digit].
+template <bool kPriv>
+__global__ void hist_kernel(const int64_t* __restrict__ v, const int32_t* __restrict__ seg, long long n, int n_seg, int n_pct,
+                            int d, const Ws* hdr, const unsigned long long* __restrict__ prefix, unsigned int* hist) {
+  const unsigned long long diff = hdr->and_bits ^ hdr->or_bits;
+  if (!hdr->any || ((diff >> (8 * d)) & 0xffull) == 0) return;   // every key has the same digit here: skipped
+  extern __shared__ unsigned int sh[];
+  const int nb = n_seg * n_pct * 256;
+  if (kPriv) { for (int i = threadIdx.x; i < nb; i += blockDim.x) sh[i] = 0; __syncthreads(); }
+  const int shift = 8 * d;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    const int s = seg[i];
+    if (s < 0 || s >= n_seg) continue;
+    const unsigned long long k = (unsigned long long)v[i] ^ kSign;
+    const unsigned long long hi = d == 7 ? 0ull : (k >> (shift + 8));
+    const unsigned dig = (unsigned)(k >> shift) & 0xffu;
+    for (int q = 0; q < n_pct; ++q) {
+      if (hi == prefix[s * n_pct + q]) {
+        const int bin = (s * n_pct + q) * 256 + dig;
+        if (kPriv) atomicAdd(&sh[bin], 1u); else atomicAdd(&hist[bin], 1u);
+      }
+    }
+  }
+  if (kPriv) { __syncthreads(); for (int i = threadIdx.x; i < nb; i += blockDim.x) if (sh[i]) atomicAdd(&hist[i], sh[i]); }
+}
+
+__global__ void select_kernel(int n_seg, int n_pct, int d, const Ws* hdr, const unsigned long long* counts,
+                              unsigned long long* prefix, unsigned long long* rank, unsigned int* hist, int64_t* out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_seg * n_pct) return;
+  const unsigned long long diff = hdr->and_bits ^ hdr->or_bits;
+  const bool skip = !hdr->any || ((diff >> (8 * d)) & 0xffull) == 0;
+  unsigned long long pf = prefix[i];
+  if (skip) pf = (pf << 8) | ((hdr->and_bits >> (8 * d)) & 0xffull);
+  else {
+    unsigned int* h = hist + (size_t)i * 256;
+    unsigned long long r = rank[i], cum = 0; int dig = 255;
+    for (int k = 0; k < 256; ++k) { const unsigned c = h[k]; if (cum + c >= r) { dig = k; break; } cum += c; }
+    for (int k = 0; k < 256; ++k) h[k] = 0;   // ready for the next digit
+    rank[i] = r - cum;
+    pf = (pf << 8) | (unsigned long long)dig;
+  }
+  prefix[i] = pf;
+  if (d == 0) out[i] = counts[i / n_pct] ? (int64_t)(pf ^ kSign) : -1;
+}
+
+}  // namespace k3
+
+size_t ws_tail_stats(int64_t n_seg, int64_t n_pct) { return k3::make_layout(nullptr, n_seg, n_pct).total; }
+
+}  // namespace ds
+
+extern "C" int ds_latencies(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t n_total,
+                            const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, const int64_t* t_mid,
+                            int64_t* e2e, int64_t* qdelay, int32_t* seg_tier, int32_t* seg_all, void* stream) {
+  using namespace ds;
+  if (!tr || n_inst < 0 || n_total < 0) return DS_EINVAL;
+  if (n_inst == 0 || n_total == 0) return DS_OK;
+  if (!inst || !out_off || !start_tick || !done_tick || !e2e || !qdelay || n_inst > 0x7fffffff) return DS_EINVAL;
+  k3::latencies_kernel<<<(unsigned)n_inst, 256, 0, (cudaStream_t)stream>>>(tr->trace_off, tr->arrival_tick, tr->tier, inst, out_off,
+                                                                        start_tick, done_tick, group, t_mid, e2e, qdelay, seg_tier, seg_all);
+  note_launch();
+  DS_CUDA(cudaGetLastError());
+  return DS_OK;
+}
+
+extern "C" int ds_tail_stats(const int64_t* values, const int32_t* seg_id, int64_t n, int32_t n_segments, const int32_t* pct,
+                             int32_t n_pct, int64_t* out, int64_t* count_out, void* workspace, size_t workspace_bytes, void* stream) {
+  using namespace ds;
+  if (n < 0 || n_segments < 1 || n_pct < 1 || n_pct > k3::kMaxPct || !pct || !out || !workspace) return DS_EINVAL;
+  if (n > 0 && (!values || !seg_id)) return DS_EINVAL;
+  if (n >= (1ll << 32) || (long long)n_segments * n_pct > (1 << 22)) return DS_EINVAL;
+  k3::Pcts pc;
+  for (int q = 0; q < n_pct; ++q) { if (pct[q] < 0 || pct[q] > 100) return DS_EINVAL; pc.p[q] = pct[q]; }
+  k3::Layout L = k3::make_layout(workspace, n_segments, n_pct);
+  if (workspace_bytes < L.total) return DS_ENOMEM;
+  cudaStream_t s = (cudaStream_t)stream;
+  DS_CUDA(cudaMemsetAsync(workspace, 0, L.total, s));
+  DS_CUDA(cudaMemsetAsync(&L.hdr->and_bits, 0xff, 8, s));
+  const int nsq = n_segments * n_pct;
+  const int threads = 256;
+  long long blocks = (n + threads * 8 - 1) / (threads * 8);
+  if (blocks > kNumSMs * 8) blocks = kNumSMs * 8;
+  if (blocks < 1) blocks = 1;
+  const size_t csm = n_segments <= 4096 ? sizeof(unsigned) * (size_t)n_segments : 0;
+  k3::count_kernel<<<(unsigned)blocks, threads, csm, s>>>(values, seg_id, n, n_segments, L.hdr, L.counts);
+  k3::init_kernel<<<(nsq + 255) / 256, 256, 0, s>>>(L.counts, n_segments, n_pct, pc, L.prefix, L.rank, count_out);
+  note_launch(2);
+  const size_t hsm = sizeof(unsigned) * 256 * (size_t)nsq;
+  const bool priv = hsm <= 160 * 1024;
+  static bool attr_set = false;
+  if (priv && !attr_set) {
+    DS_CUDA(cudaFuncSetAttribute(k3::hist_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
+    attr_set = true;
+  }
+  long long hblocks = priv ? (long long)kNumSMs * (hsm <= 64 * 1024 ? 2 : 1) : blocks;
+  if (hblocks > blocks) hblocks = blocks;
+  for (int d = 7; d >= 0; --d) {
+    if (priv) k3::hist_kernel<true><<<(unsigned)hblocks, threads, hsm, s>>>(values, seg_id, n, n_segments, n_pct, d, L.hdr, L.prefix, L.hist);
+    else k3::hist_kernel<false><<<(unsigned)blocks, threads, 0, s>>>(values, seg_id, n, n_segments, n_pct, d, L.hdr, L.prefix, L.hist);
+    k3::select_kernel<<<(nsq + 127) / 128, 128, 0, s>>>(n_segments, n_pct, d, L.hdr, L.counts, L.prefix, L.rank, L.hist, out);
+    note_launch(2);
+  }
+  DS_CUDA(cudaGetLastError());
+  return DS_OK;
+}

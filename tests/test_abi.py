@@ -1,0 +1,43 @@
+"""CPU: the C-ABI library loads and exports every symbol include/driftsched.h declares (no compute calls)."""
+import ctypes
+import os
+import re
+
+from paper_2606_02982_b200 import _lib, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_header_symbols_exported():
+    build.build()
+    hdr = open(os.path.join(ROOT, "include", "driftsched.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = sorted(set(re.findall(r"\b(ds_[a-z_]+)\s*\(", hdr)))
+    assert declared == sorted(_lib.EXPORTS)
+    L = ctypes.CDLL(_lib.LIB_PATH)
+    for name in declared:
+        assert hasattr(L, name), name
+
+
+def test_host_only_entry_points():
+    L = _lib.lib()
+    assert L.ds_strerror(0) == b"ok" and L.ds_strerror(-3) == b"workspace too small"
+    assert L.ds_workspace_bytes(_lib.WS_TAIL_STATS, 4, 2) >= 4 * 2 * 256 * 4
+    assert L.ds_workspace_bytes(_lib.WS_SIMULATE, 1000, 10) >= 8000
+    assert L.ds_workspace_bytes(99, 1, 1) >= 256
+    assert L.ds_launch_count() == 0
+
+
+def test_struct_layouts_match_header():
+    assert ctypes.sizeof(_lib.DsTraces) == 56 and ctypes.sizeof(_lib.DsServer) == 80
+    from paper_2606_02982_b200 import workload as wl
+    assert wl.INSTANCE_DTYPE.itemsize == 24
+
+
+def test_no_oracle_in_product_path():
+    pkg = os.path.join(ROOT, "paper_2606_02982_b200")
+    for dp, _, fs in os.walk(pkg):
+        for f in fs:
+            if f.endswith((".py", ".cu", ".cuh", ".cpp", ".h")):
+                src = open(os.path.join(dp, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "oracle/" not in src.replace("the oracle", ""), f
