@@ -104,16 +104,20 @@ def simulate(trace_off, arrival, tier, words, tokens, out_len, server, inst, out
 
 
 def latencies(trace_off, arrival, tier, words, tokens, out_len, inst, out_off, n_total, start, done, group=None, t_mid=None,
-              want_seg_tier=True, want_seg_all=True):
+              want_seg_tier=True, want_seg_all=True, out=None):
     """ds_latencies -> (e2e, qdelay, seg_tier, seg_all)."""
     tr = _traces(trace_off, arrival, tier, words, tokens, out_len)
     _need_cuda(inst, out_off, start, done, group, t_mid)
     n_inst = inst.numel() // INSTANCE_BYTES
     dev = start.device
-    e2e = torch.empty(n_total, dtype=torch.int64, device=dev)
-    qd = torch.empty(n_total, dtype=torch.int64, device=dev)
-    st = torch.empty(n_total, dtype=torch.int32, device=dev) if want_seg_tier else None
-    sa = torch.empty(n_total, dtype=torch.int32, device=dev) if want_seg_all else None
+    if out is not None:
+        e2e, qd, st, sa = out
+        _need_cuda(e2e, qd, st, sa)
+    else:
+        e2e = torch.empty(n_total, dtype=torch.int64, device=dev)
+        qd = torch.empty(n_total, dtype=torch.int64, device=dev)
+        st = torch.empty(n_total, dtype=torch.int32, device=dev) if want_seg_tier else None
+        sa = torch.empty(n_total, dtype=torch.int32, device=dev) if want_seg_all else None
     check("ds_latencies", lib().ds_latencies(C.byref(tr), _ptr(inst), n_inst, _ptr(out_off), n_total, _ptr(start), _ptr(done),
                                              _ptr(group), _ptr(t_mid), _ptr(e2e), _ptr(qd), _ptr(st), _ptr(sa), _stream()))
     return e2e, qd, st, sa

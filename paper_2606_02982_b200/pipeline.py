@@ -1,0 +1,83 @@
+"""One pass of the whole hot path over a resident workload:
+ds_characterize -> ds_simulate -> ds_latencies -> 4 x ds_tail_stats. Orchestration and buffer ownership only;
+every computation happens inside libdriftsched.so."""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from . import _lib, api
+
+
+class HotPath:
+    """Device-resident buffers for one workload (see workload.Workload) and the step that runs the path."""
+
+    def __init__(self, wl_obj, device="cuda:0", pct=(50, 99)):
+        c = wl_obj
+        self.c = c
+        self.dev = torch.device(device)
+        self.pct = tuple(pct)
+        up = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(self.dev)
+        self.text = up(c.text) if c.text is not None else None
+        self.offsets = up(c.offsets) if c.offsets is not None else None
+        self.trace_off = up(c.trace_off)
+        self.arrival = up(c.arrival)
+        self.tier = up(c.tier)
+        self.out_len = up(c.out_len)
+        self.words = up(c.words)     # overwritten by ds_characterize every step when text is present
+        self.tokens = up(c.tokens)
+        self.inst = api.instances_to_device(c.instances, self.dev)
+        self.out_off = up(c.out_off)
+        self.group = up(c.group)
+        self.t_mid = up(c.t_mid) if c.t_mid is not None else None
+        self.n_total = int(c.out_off[-1])
+        self.n_inst = c.n_inst
+        self.n_groups = c.n_groups * (2 if c.t_mid is not None else 1)
+        n, dev = self.n_total, self.dev
+        self.start = torch.empty(n, dtype=torch.int64, device=dev)
+        self.done = torch.empty(n, dtype=torch.int64, device=dev)
+        self.ema_final = torch.empty((self.n_inst, 3), dtype=torch.float64, device=dev)
+        self.traj_off = self.ema_traj = None
+        if c.server.traj_every > 0:
+            k = (np.diff(c.trace_off)[c.instances["trace"]] // c.server.traj_every).astype(np.int64)
+            toff = np.concatenate([[0], np.cumsum(k)]).astype(np.int64)
+            self.traj_off = up(toff)
+            self.ema_traj = torch.zeros((int(toff[-1]), 3), dtype=torch.float64, device=dev)
+        ws = lambda which, a, b: torch.empty(api.workspace_bytes(which, a, b), dtype=torch.uint8, device=dev)
+        self.ws_char = ws(_lib.WS_CHARACTERIZE, 0 if self.text is None else self.text.numel(), c.n_traces * c.n_req)
+        self.ws_sim = ws(_lib.WS_SIMULATE, n, self.n_inst)
+        self.ws_tail = ws(_lib.WS_TAIL_STATS, 3 * self.n_groups, len(self.pct))
+        self.stats = {k: torch.empty((ns, len(self.pct)), dtype=torch.int64, device=dev)
+                      for k, ns in (("e2e_tier", 3 * self.n_groups), ("e2e_all", self.n_groups),
+                                    ("qdelay_tier", 3 * self.n_groups), ("qdelay_all", self.n_groups))}
+        self.counts = {k: torch.empty(v.shape[0], dtype=torch.int64, device=dev) for k, v in self.stats.items()}
+        self.e2e = torch.empty(n, dtype=torch.int64, device=dev)
+        self.qdelay = torch.empty(n, dtype=torch.int64, device=dev)
+        self.seg_tier = torch.empty(n, dtype=torch.int32, device=dev)
+        self.seg_all = torch.empty(n, dtype=torch.int32, device=dev)
+
+    def step(self, timed_events=False):
+        """Run the path once on the current stream. With timed_events, returns CUDA events bracketing each stage."""
+        ev = []
+        mark = (lambda: ev.append(self._rec())) if timed_events else (lambda: None)
+        mark()
+        if self.text is not None:
+            api.characterize(self.text, self.offsets, self.words, self.tokens, self.ws_char)
+        mark()
+        api.simulate(self.trace_off, self.arrival, self.tier, self.words, self.tokens, self.out_len, self.c.server, self.inst,
+                     self.out_off, self.n_total, self.start, self.done, self.ema_final, self.traj_off, self.ema_traj, self.ws_sim)
+        mark()
+        e2e, qd, seg_t, seg_a = api.latencies(self.trace_off, self.arrival, self.tier, self.words, self.tokens, self.out_len,
+                                              self.inst, self.out_off, self.n_total, self.start, self.done, self.group, self.t_mid,
+                                              out=(self.e2e, self.qdelay, self.seg_tier, self.seg_all))
+        for name, vals, seg in (("e2e_tier", e2e, seg_t), ("e2e_all", e2e, seg_a), ("qdelay_tier", qd, seg_t),
+                                ("qdelay_all", qd, seg_a)):
+            api.tail_stats(vals, seg, self.stats[name].shape[0], self.pct, self.stats[name], self.counts[name], self.ws_tail)
+        mark()
+        return ev
+
+    @staticmethod
+    def _rec():
+        e = torch.cuda.Event(enable_timing=True)
+        e.record()
+        return e
