@@ -27,7 +27,7 @@ constexpr int kThreads = kWarps * 32;
 constexpr int kSeg = 64;                      // bytes per lane per chunk
 constexpr int kChunk = 32 * kSeg;             // 2 KiB per warp per step
 constexpr int kStages = 4;
-constexpr int kCtasPerSM = 2;
+constexpr int kCtasPerSM = 3;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr long long kInfOff = 0x7fffffffffffffffLL;
 
@@ -68,15 +68,33 @@ __device__ __forceinline__ void tma_load_1d(void* dst, const void* src, unsigned
 // z = x|0x80808080 keeps every byte >= 0x80 so the per-byte subtractions never borrow across bytes; bit 7 of
 // (z - n*0x01010101) is (low7(x) >= n). Intervals are XORs of nested thresholds. m = ~x & 0x80808080 both drops
 // bytes >= 0x80 (LETTER) and clears the 7 low garbage bits, so the results are exactly 0x80 / 0x00 per byte.
-__device__ __forceinline__ void classify4(uint32_t x, uint32_t& ws7, uint32_t& d7) {
+// The threshold adds are issued as IMAD (z * one + (-n)) with a run-time `one` == 1 so that they execute on the FMA
+// pipe: the ALU pipe (LOP3/SHF/ISETP, half rate) is the limiter of this kernel, not HBM.
+__device__ __forceinline__ uint32_t thr(uint32_t z, uint32_t one, uint32_t n) {
+  uint32_t t;
+  asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(t) : "r"(z), "r"(one), "r"(0u - n * 0x01010101u));
+  return t;
+}
+__device__ __forceinline__ uint32_t lop3_xor3(uint32_t a, uint32_t b, uint32_t c) {
+  uint32_t r;
+  asm("lop3.b32 %0, %1, %2, %3, 0x96;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+  return r;
+}
+__device__ __forceinline__ uint32_t lop3_xor_and(uint32_t a, uint32_t b, uint32_t c) {   // (a ^ b) & c
+  uint32_t r;
+  asm("lop3.b32 %0, %1, %2, %3, 0x28;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+  return r;
+}
+__device__ __forceinline__ void classify4(uint32_t x, uint32_t one, uint32_t& ws7, uint32_t& d7) {
   const uint32_t z = x | 0x80808080u;
   const uint32_t m = ~x & 0x80808080u;
-  const uint32_t t9 = z - 0x09090909u, t14 = z - 0x0E0E0E0Eu, t32 = z - 0x20202020u, t33 = z - 0x21212121u;
-  const uint32_t t48 = z - 0x30303030u, t58 = z - 0x3A3A3A3Au, t65 = z - 0x41414141u, t91 = z - 0x5B5B5B5Bu;
-  const uint32_t t97 = z - 0x61616161u, t123 = z - 0x7B7B7B7Bu, t127 = z - 0x7F7F7F7Fu;
-  const uint32_t s1 = t9 ^ t14 ^ t32;                       // [9,13] u [32,..)
-  ws7 = (s1 ^ t33) & m;                                     // WS = [9,13] u {32}
-  d7 = (s1 ^ (t48 ^ t58 ^ t65) ^ (t91 ^ t97 ^ t123) ^ t127) & m;  // non-LETTER = WS u PUNCT
+  const uint32_t t9 = thr(z, one, 9), t14 = thr(z, one, 14), t32 = thr(z, one, 32), t33 = thr(z, one, 33);
+  const uint32_t t48 = thr(z, one, 48), t58 = thr(z, one, 58), t65 = thr(z, one, 65), t91 = thr(z, one, 91);
+  const uint32_t t97 = thr(z, one, 97), t123 = thr(z, one, 123), t127 = thr(z, one, 127);
+  const uint32_t s1 = lop3_xor3(t9, t14, t32);              // [9,13] u [32,..)
+  ws7 = lop3_xor_and(s1, t33, m);                           // WS = [9,13] u {32}
+  const uint32_t a = lop3_xor3(t48, t58, t65), b = lop3_xor3(t91, t97, t123);
+  d7 = lop3_xor_and(lop3_xor3(s1, a, b), t127, m);          // non-LETTER = WS u PUNCT
 }
 
 // 8 bytes holding 0x80/0x00 -> 128 * (8-bit mask): two IDP4A with weights 1,2,4,8 | 16,32,64,128
@@ -126,7 +144,7 @@ __device__ __forceinline__ long long warp_count_lt(const int64_t* __restrict__ o
 
 __global__ void __launch_bounds__(kThreads, kCtasPerSM)
 characterize_kernel(const uint8_t* __restrict__ bytes, long long n_bytes, const int64_t* __restrict__ off, long long n_prompts,
-                    int32_t* __restrict__ words, int32_t* __restrict__ tokens, long long n_chunks, unsigned int* status) {
+                    int32_t* __restrict__ words, int32_t* __restrict__ tokens, long long n_chunks, unsigned int* status, unsigned int one) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
 
@@ -150,16 +168,17 @@ characterize_kernel(const uint8_t* __restrict__ bytes, long long n_bytes, const 
   sb[lane] = 0u; sb[lane + 32] = 0u;
   __syncwarp();
 
-  auto issue = [&](long long c) {  // lane 0 only: chunk c -> stage (c - c_begin) % kStages
-    const int s = (int)((c - c_begin) % kStages);
-    const long long a0 = c * (long long)kChunk;
+  auto issue = [&](unsigned it) {  // lane 0 only: chunk c_begin + it -> stage it % kStages
+    const int s = (int)(it & (kStages - 1));
+    const long long a0 = (c_begin + it) * (long long)kChunk;
     long long len = load_end - a0;
     if (len > kChunk) len = kChunk;
     mbar_expect_tx(&mbar[s], (unsigned)len);
     tma_load_1d(stage[s], abase + a0, (unsigned)len, &mbar[s]);
   };
+  const unsigned n_it = (unsigned)(c_end - c_begin);
   if (lane == 0)
-    for (long long c = c_begin; c < c_end && c < c_begin + kStages; ++c) issue(c);
+    for (unsigned it = 0; it < n_it && it < (unsigned)kStages; ++it) issue(it);
 
   // ---- span prologue: boundary cursor and the carries at the span's first byte ----
   const long long nb_total = n_prompts + 1;                   // boundaries off[0..n_prompts]
@@ -195,11 +214,12 @@ characterize_kernel(const uint8_t* __restrict__ bytes, long long n_bytes, const 
   load_window();
 
   const int rot = (lane >> 1) & 3;    // 16-byte pieces are read in rotated order: conflict-free LDS.128 at a 64-byte lane stride
-  for (long long c = c_begin; c < c_end; ++c) {
-    const long long it = c - c_begin;
-    const int s = (int)(it % kStages);
-    const unsigned parity = (unsigned)((it / kStages) & 1);
-    const long long cs = c * (long long)kChunk - mis, ce = cs + kChunk;   // chunk = positions [cs,ce) relative to bytes
+  static_assert((kStages & (kStages - 1)) == 0, "kStages must be a power of two");
+  long long cs = pos0;
+  for (unsigned it = 0; it < n_it; ++it, cs += kChunk) {
+    const int s = (int)(it & (kStages - 1));
+    const unsigned parity = (it / kStages) & 1u;
+    const long long ce = cs + kChunk;   // chunk = positions [cs,ce) relative to bytes
 
     // (a) prompt boundaries inside this chunk -> start bits (lanes 0..nb-1 of the window hold them)
     bool inb = o >= cs && o < ce;
@@ -224,12 +244,12 @@ characterize_kernel(const uint8_t* __restrict__ bytes, long long n_bytes, const 
       const int r = (j + rot) & 3;
       const uint4 v = *reinterpret_cast<const uint4*>(seg + r * 16);
       uint32_t w0, w1, w2, w3, e0, e1, e2, e3;
-      classify4(v.x, w0, e0); classify4(v.y, w1, e1); classify4(v.z, w2, e2); classify4(v.w, w3, e3);
+      classify4(v.x, one, w0, e0); classify4(v.y, one, w1, e1); classify4(v.z, one, w2, e2); classify4(v.w, one, w3, e3);
       wf[j] = mask8x128(w2, w3) * 256u + mask8x128(w0, w1);
       df[j] = mask8x128(e2, e3) * 256u + mask8x128(e0, e1);
     }
     __syncwarp();
-    if (lane == 0 && c + kStages < c_end) issue(c + kStages);   // the stage's bytes are all in registers now
+    if (lane == 0 && it + kStages < n_it) issue(it + kStages);   // the stage's bytes are all in registers now
     unsigned long long ws = rotl16(wf[1] * 512u + (wf[0] >> 7), wf[3] * 512u + (wf[2] >> 7), rot);
     unsigned long long d = rotl16(df[1] * 512u + (df[0] >> 7), df[3] * 512u + (df[2] >> 7), rot);
     if (cs < 0 || ce > n_bytes) {                        // bytes outside [0,n_bytes) count as whitespace
@@ -365,7 +385,7 @@ extern "C" int ds_characterize(const uint8_t* bytes, int64_t n_bytes, const int6
   const long long need = (n_chunks + k1::kWarps - 1) / k1::kWarps;
   if (grid > need) grid = need;
   k1::characterize_kernel<<<(unsigned)grid, k1::kThreads, sizeof(k1::Smem), st>>>(bytes, n_bytes, offsets, n_prompts, words_out,
-                                                                               tokens_out, n_chunks, status);
+                                                                               tokens_out, n_chunks, status, 1u);
   note_launch();
   DS_CUDA(cudaGetLastError());
   return DS_OK;
