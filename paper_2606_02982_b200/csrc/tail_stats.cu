@@ -56,18 +56,37 @@ __global__ void latencies_kernel(const int64_t* __restrict__ trace_off, const in
   }
 }
 
-__global__ void count_kernel(const int64_t* __restrict__ v, const int32_t* __restrict__ seg, long long n, int n_seg,
+// Warp-aggregated shared-memory add: lanes of the warp that target the same bin are merged with MATCH.ANY so a hot
+// bin (latencies share their high digits) costs one atomic per warp instead of 32 serialised ones.
+__device__ __forceinline__ void agg_add(unsigned int* bins, bool pred, unsigned bin) {
+  const unsigned m = __match_any_sync(0xffffffffu, pred ? bin : 0xffffffffu);
+  if (pred && (threadIdx.x & 31) == (unsigned)(__ffs(m) - 1)) atomicAdd(&bins[bin], (unsigned)__popc(m));
+}
+
+constexpr int kUnroll = 4;   // independent 12-byte loads in flight per thread
+
+__global__ void __launch_bounds__(512) count_kernel(const int64_t* __restrict__ v, const int32_t* __restrict__ seg, long long n, int n_seg,
                              Ws* hdr, unsigned long long* counts) {
   extern __shared__ unsigned int sc[];   // per-block segment counts when n_seg is small
   const bool priv = n_seg <= 4096;
   if (priv) { for (int i = threadIdx.x; i < n_seg; i += blockDim.x) sc[i] = 0; __syncthreads(); }
   unsigned long long a = ~0ull, o = 0ull; bool any = false;
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-    const int s = seg[i];
-    if (s < 0 || s >= n_seg) continue;
-    const unsigned long long k = (unsigned long long)v[i] ^ kSign;
-    a &= k; o |= k; any = true;
-    if (priv) atomicAdd(&sc[s], 1u); else atomicAdd(&counts[s], 1ull);
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long base = blockIdx.x * (long long)blockDim.x; base < n; base += stride * kUnroll) {   // block-uniform trip count
+    int sv[kUnroll]; unsigned long long kv[kUnroll];
+#pragma unroll
+    for (int u = 0; u < kUnroll; ++u) {
+      const long long i = base + u * stride + threadIdx.x;
+      sv[u] = i < n ? seg[i] : -1;
+      kv[u] = i < n ? (unsigned long long)v[i] ^ kSign : 0ull;
+    }
+#pragma unroll
+    for (int u = 0; u < kUnroll; ++u) {
+      const bool ok = sv[u] >= 0 && sv[u] < n_seg;
+      if (ok) { a &= kv[u]; o |= kv[u]; any = true; }
+      if (priv) agg_add(sc, ok, (unsigned)sv[u]);
+      else if (ok) atomicAdd(&counts[sv[u]], 1ull);
+    }
   }
   for (int d = 16; d > 0; d >>= 1) { a &= __shfl_xor_sync(0xffffffffu, a, d); o |= __shfl_xor_sync(0xffffffffu, o, d); }
   const unsigned anym = __ballot_sync(0xffffffffu, any);
@@ -92,48 +111,83 @@ __global__ void init_kernel(const unsigned long long* counts, int n_seg, int n_p
 
 // digit d (7 = most significant). Keys whose bits above digit d equal prefix[s,q] are counted in hist[s,q][digit].
 template <bool kPriv>
-__global__ void hist_kernel(const int64_t* __restrict__ v, const int32_t* __restrict__ seg, long long n, int n_seg, int n_pct,
-                            int d, const Ws* hdr, const unsigned long long* __restrict__ prefix, unsigned int* hist) {
+__global__ void __launch_bounds__(512) hist_kernel(const int64_t* __restrict__ v, const int32_t* __restrict__ seg, long long n, int n_seg,
+                            int n_pct, int d, const Ws* hdr, const unsigned long long* __restrict__ prefix, unsigned int* hist) {
   const unsigned long long diff = hdr->and_bits ^ hdr->or_bits;
   if (!hdr->any || ((diff >> (8 * d)) & 0xffull) == 0) return;   // every key has the same digit here: skipped
   extern __shared__ unsigned int sh[];
   const int nb = n_seg * n_pct * 256;
   if (kPriv) { for (int i = threadIdx.x; i < nb; i += blockDim.x) sh[i] = 0; __syncthreads(); }
+  unsigned int* bins = kPriv ? sh : hist;
   const int shift = 8 * d;
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-    const int s = seg[i];
-    if (s < 0 || s >= n_seg) continue;
-    const unsigned long long k = (unsigned long long)v[i] ^ kSign;
-    const unsigned long long hi = d == 7 ? 0ull : (k >> (shift + 8));
-    const unsigned dig = (unsigned)(k >> shift) & 0xffu;
-    for (int q = 0; q < n_pct; ++q) {
-      if (hi == prefix[s * n_pct + q]) {
-        const int bin = (s * n_pct + q) * 256 + dig;
-        if (kPriv) atomicAdd(&sh[bin], 1u); else atomicAdd(&hist[bin], 1u);
-      }
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long base = blockIdx.x * (long long)blockDim.x; base < n; base += stride * kUnroll) {   // block-uniform trip count
+    int sv[kUnroll]; unsigned long long kv[kUnroll];
+#pragma unroll
+    for (int u = 0; u < kUnroll; ++u) {
+      const long long i = base + u * stride + threadIdx.x;
+      sv[u] = i < n ? seg[i] : -1;
+      kv[u] = i < n ? (unsigned long long)v[i] ^ kSign : 0ull;
+    }
+#pragma unroll
+    for (int u = 0; u < kUnroll; ++u) {
+      const bool ok = sv[u] >= 0 && sv[u] < n_seg;
+      const int s = ok ? sv[u] : 0;
+      const unsigned long long hi = d == 7 ? 0ull : (kv[u] >> (shift + 8));
+      const unsigned dig = (unsigned)(kv[u] >> shift) & 0xffu;
+      for (int q = 0; q < n_pct; ++q)
+        agg_add(bins, ok && hi == prefix[s * n_pct + q], (unsigned)((s * n_pct + q) * 256) + dig);
     }
   }
   if (kPriv) { __syncthreads(); for (int i = threadIdx.x; i < nb; i += blockDim.x) if (sh[i]) atomicAdd(&hist[i], sh[i]); }
 }
 
+// one warp per (segment, percentile): lane l owns bins 8l..8l+7; warp prefix scan finds the digit that holds the rank
 __global__ void select_kernel(int n_seg, int n_pct, int d, const Ws* hdr, const unsigned long long* counts,
                               unsigned long long* prefix, unsigned long long* rank, unsigned int* hist, int64_t* out) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (i >= n_seg * n_pct) return;
   const unsigned long long diff = hdr->and_bits ^ hdr->or_bits;
   const bool skip = !hdr->any || ((diff >> (8 * d)) & 0xffull) == 0;
   unsigned long long pf = prefix[i];
   if (skip) pf = (pf << 8) | ((hdr->and_bits >> (8 * d)) & 0xffull);
   else {
-    unsigned int* h = hist + (size_t)i * 256;
-    unsigned long long r = rank[i], cum = 0; int dig = 255;
-    for (int k = 0; k < 256; ++k) { const unsigned c = h[k]; if (cum + c >= r) { dig = k; break; } cum += c; }
-    for (int k = 0; k < 256; ++k) h[k] = 0;   // ready for the next digit
-    rank[i] = r - cum;
-    pf = (pf << 8) | (unsigned long long)dig;
+    uint4* h4 = reinterpret_cast<uint4*>(hist + (size_t)i * 256 + lane * 8);
+    const uint4 x = h4[0], y = h4[1];
+    h4[0] = make_uint4(0, 0, 0, 0); h4[1] = make_uint4(0, 0, 0, 0);   // ready for the next digit
+    const unsigned c[8] = {x.x, x.y, x.z, x.w, y.x, y.y, y.z, y.w};
+    unsigned long long own = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) own += c[k];
+    unsigned long long incl = own;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned long long t = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += t;
+    }
+    const unsigned long long r = rank[i];
+    const unsigned hit = __ballot_sync(0xffffffffu, incl >= r);   // first lane whose inclusive count reaches the rank
+    const int src = hit ? __ffs(hit) - 1 : 31;
+    unsigned long long cum = incl - own;
+    int dig = 7;
+#pragma unroll
+    for (int k = 7; k >= 0; --k) {                                // first k with cum + c[0..k] >= r
+      unsigned long long pre = cum;
+#pragma unroll
+      for (int j = 0; j < k; ++j) pre += c[j];
+      if (pre + c[k] >= r) dig = k;
+    }
+    unsigned long long before = cum;
+    for (int j = 0; j < dig; ++j) before += c[j];
+    const int digit = __shfl_sync(0xffffffffu, lane * 8 + dig, src);
+    const unsigned long long bef = __shfl_sync(0xffffffffu, before, src);
+    if (lane == 0) rank[i] = r - bef;
+    pf = (pf << 8) | (unsigned long long)digit;
   }
-  prefix[i] = pf;
-  if (d == 0) out[i] = counts[i / n_pct] ? (int64_t)(pf ^ kSign) : -1;
+  if (lane == 0) {
+    prefix[i] = pf;
+    if (d == 0) out[i] = counts[i / n_pct] ? (int64_t)(pf ^ kSign) : -1;
+  }
 }
 
 }  // namespace k3
@@ -170,9 +224,9 @@ extern "C" int ds_tail_stats(const int64_t* values, const int32_t* seg_id, int64
   DS_CUDA(cudaMemsetAsync(workspace, 0, L.total, s));
   DS_CUDA(cudaMemsetAsync(&L.hdr->and_bits, 0xff, 8, s));
   const int nsq = n_segments * n_pct;
-  const int threads = 256;
-  long long blocks = (n + threads * 8 - 1) / (threads * 8);
-  if (blocks > kNumSMs * 8) blocks = kNumSMs * 8;
+  const int threads = 512;
+  long long blocks = (n + threads * k3::kUnroll - 1) / (threads * k3::kUnroll);
+  if (blocks > kNumSMs * 4) blocks = kNumSMs * 4;
   if (blocks < 1) blocks = 1;
   const size_t csm = n_segments <= 4096 ? sizeof(unsigned) * (size_t)n_segments : 0;
   k3::count_kernel<<<(unsigned)blocks, threads, csm, s>>>(values, seg_id, n, n_segments, L.hdr, L.counts);
@@ -185,12 +239,15 @@ extern "C" int ds_tail_stats(const int64_t* values, const int32_t* seg_id, int64
     DS_CUDA(cudaFuncSetAttribute(k3::hist_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
     attr_set = true;
   }
-  long long hblocks = priv ? (long long)kNumSMs * (hsm <= 64 * 1024 ? 2 : 1) : blocks;
+  long long per_sm = priv ? (long long)(200 * 1024) / (long long)(hsm + 1024) : 4;   // resident blocks by shared memory
+  if (per_sm > 4) per_sm = 4;
+  if (per_sm < 1) per_sm = 1;
+  long long hblocks = priv ? (long long)kNumSMs * per_sm : blocks;
   if (hblocks > blocks) hblocks = blocks;
   for (int d = 7; d >= 0; --d) {
     if (priv) k3::hist_kernel<true><<<(unsigned)hblocks, threads, hsm, s>>>(values, seg_id, n, n_segments, n_pct, d, L.hdr, L.prefix, L.hist);
     else k3::hist_kernel<false><<<(unsigned)blocks, threads, 0, s>>>(values, seg_id, n, n_segments, n_pct, d, L.hdr, L.prefix, L.hist);
-    k3::select_kernel<<<(nsq + 127) / 128, 128, 0, s>>>(n_segments, n_pct, d, L.hdr, L.counts, L.prefix, L.rank, L.hist, out);
+    k3::select_kernel<<<(nsq + 3) / 4, 128, 0, s>>>(n_segments, n_pct, d, L.hdr, L.counts, L.prefix, L.rank, L.hist, out);
     note_launch(2);
   }
   DS_CUDA(cudaGetLastError());
