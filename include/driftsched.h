@@ -111,7 +111,7 @@ typedef struct {
  *                                 floor(n_req_i / traj_every) of them
  * ema_traj    [traj_off[n_inst]*3] nullable device fp64
  * workspace: ds_workspace_bytes(DS_WS_SIMULATE, total_requests_over_instances, n_inst).
- * Launches: 1 memset (work counter + status) + 1 kernel. */
+ * Launches: 1 memset (work counter) + 2 kernels (policy-major ordering of the instances, simulation). */
 int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
                 const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
                 const int64_t* traj_off, double* ema_traj, void* workspace, size_t workspace_bytes, void* stream);

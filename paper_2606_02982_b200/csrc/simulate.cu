@@ -5,18 +5,25 @@
 // (t1=1-a; t2=t1*B; t3=a*m; B=t2+t3) and must match the oracle at 0 ulp; the _rn intrinsics below are never
 // contracted either way.
 //
-// Mapping to the warp (B200: 148 SMs, persistent warps pulling instances from an atomic counter):
-//  - warp-uniform scalars: clock `now`, cursor `next`, batch size b, kv_used, iteration cost dt, B[3];
+// Mapping to the warp (B200: 148 SMs, persistent warps pulling instances from an atomic counter). The per-instance
+// body is compiled once per (slots, policy) so that each policy's queue logic is straight-line code:
+//  - warp-uniform scalars: clock `now`, cursor `next`, next arrival tick `an`, batch size b, kv_used, B[3] (held by
+//    lanes 0..2);
 //  - running set: kSlots slots per lane (max_batch <= 32*kSlots), each {request index, finishing iteration};
-//    completions are found with one REDUX min over (fin - iter); between events the clock advances with a
-//    3-instruction recurrence (now += dt; dt += c_ctx*b) that is exactly the per-iteration cost of §8(c) step 6;
+//    completions are found with one REDUX min over (fin - iter);
+//  - between events the batch is constant, so j iterations cost exactly j*dt + c_ctx*b*j(j-1)/2 ticks (§8(c) step 6
+//    with a constant running set): the kernel jumps to the next event (completion, or arrival when an arrival can
+//    matter) with that closed form; a float estimate gives a provably safe lower bound on j, exact integer arithmetic
+//    does the jump, the last one or two iterations are stepped. The oracle steps one iteration at a time;
 //  - arrivals: a 32-request register window of (arrival, tier, base) per lane, ingested 32 at a time with one
-//    ballot; the estimate est=ceil(B[tier]*base) is computed by 32 lanes in parallel (B is constant within a step);
+//    ballot; est=ceil(B[tier]*base) is computed by 32 lanes in parallel. Arrivals cannot matter while the batch is
+//    full (or FIFO's head is KV-deferred): they are then ingested lazily, in bulk, at the next completion, which is
+//    exact because B only changes at completions and INGEST-EARLY uses the pre-completion B (R-ORD);
 //  - FIFO/PRIORITY/WEIGHTED/AGING queues need no storage: requests arrive in index order, so each tier's FIFO is a
 //    cursor (32-request block + ballot bitmask of that tier) and every policy picks among <= 3 heads; the frozen
 //    estimates of queued requests live in done_tick[] until the request completes;
-//  - SJF: warp-cooperative 32-ary min-heap of (est<<24 | index) keys, first 256 entries in shared memory, rest in
-//    the global workspace; sift-down compares 32 children per level with one REDUX-style shuffle min.
+//  - SJF: warp-cooperative 32-ary min-heap of (est<<24 | index) keys, first 256 entries in shared memory, rest in the
+//    global workspace; sift-down compares 32 children per level with one shuffle min.
 #include "common.cuh"
 
 namespace ds {
@@ -34,7 +41,7 @@ struct Params {
   int32_t traj_every;
   const ds_instance* inst; int64_t n_inst; const int64_t* out_off; int64_t* start_tick; int64_t* done_tick;
   double* ema_final; const int64_t* traj_off; double* ema_traj;
-  unsigned long long* heap_ws; unsigned int* counter; unsigned int* status;
+  unsigned long long* heap_ws; unsigned int* counter; unsigned int* status; const unsigned int* perm;
 };
 
 // 64-bit warp min (keys are unique, so the min identifies its lane)
@@ -46,6 +53,8 @@ __device__ __forceinline__ unsigned long long warp_min_u64(unsigned long long v)
   }
   return v;
 }
+__device__ __forceinline__ long long shfl_i64(long long v, int src) { return __shfl_sync(kFull, v, src); }
+__device__ __forceinline__ double shfl_f64(double v, int src) { return __shfl_sync(kFull, v, src); }
 
 // ---- SJF heap: implicit 32-ary min-heap, node i has children 32i+1 .. 32i+32 ----
 struct Heap {
@@ -89,279 +98,373 @@ struct Heap {
   }
 };
 
-
 // per-tier FIFO cursor for PRIORITY / WEIGHTED / AGING: head = first request of tier t at or after the cursor
 struct TierCursor {
   int blk;          // 32-request block holding the head
   unsigned mask;    // requests of this tier in that block at or after the head
   int head;         // local request index of the head, INT_MAX when the trace has no more of this tier
-  long long est;    // frozen estimate of the head (valid once it has arrived)
-  long long arr;    // arrival tick of the head
+  long long est;    // frozen estimate of the head (valid once it has arrived; only kept when the KV budget is on)
+  long long arr;    // arrival tick of the head (AGING only)
 };
 
+template <int kSlots, int kPolicy>
+__device__ __forceinline__ void run_instance(const Params& p, const unsigned inst_id, const int trace, const bool split, const double alpha,
+                                          unsigned long long* heap_sm, const int lane) {
+  constexpr bool kCursor = kPolicy == DS_PRIORITY || kPolicy == DS_WEIGHTED || kPolicy == DS_AGING;
+  const long long lo = p.trace_off[trace];
+  const long long n64 = p.trace_off[trace + 1] - lo;
+  if (n64 < 0 || n64 > 0x7ffffff0ll || (kPolicy == DS_SJF && n64 > (1 << 24))) {   // local indices are 32-bit (SJF keys: 24-bit)
+    if (lane == 0) atomicOr(p.status, n64 > (1 << 24) ? DS_DEV_KEY_RANGE : DS_DEV_BAD_TRACE);
+    return;
+  }
+  const int n = (int)n64;
+  const int64_t* __restrict__ arr = p.arrival + lo;
+  const uint8_t* __restrict__ tier = p.tier + lo;
+  const int32_t* __restrict__ W = p.words + lo;
+  const int32_t* __restrict__ P = p.tokens + lo;
+  const int32_t* __restrict__ O = p.out_len + lo;
+  const long long oo = p.out_off[inst_id];
+  int64_t* __restrict__ st = p.start_tick + oo;
+  int64_t* dn = p.done_tick + oo;
+  const int32_t* __restrict__ BASE = split ? W : P;
+  const bool use_kv = p.kv_budget > 0;
+  const bool need_est = use_kv || kPolicy == DS_SJF;
+  // EXACT estimator: m = P/P = 1.0, and (1-a)*1 + a*1 rounds to exactly 1.0 for every a in [0,1] (DESIGN.md §4 A4),
+  // so B stays 1.0 and est = base: no fp64 work at all on that path.
+  const bool ema_on = split && alpha > 0.0;
+  double* traj = (p.ema_traj && p.traj_off && p.traj_every > 0) ? p.ema_traj + 3 * p.traj_off[inst_id] : nullptr;
+  const int max_batch = p.max_batch;
+
+  // ---- state (warp-uniform unless noted) ----
+  long long now = 0, kv_used = 0, prefill_new = 0, an = kInf;
+  int next = 0, b = 0, cur = 0, fifo_head = 0, done = 0;
+  long long fifo_est = 0;
+  unsigned iter = 0, dist = 0xffffffffu;
+  bool blocked = false;
+  double Bl = 1.0;                       // lane t < 3 holds B[t]
+  int s_idx[kSlots]; unsigned s_fin[kSlots];   // per lane: running requests
+#pragma unroll
+  for (int s = 0; s < kSlots; ++s) { s_idx[s] = -1; s_fin[s] = 0; }
+  Heap heap; heap.sm = heap_sm; heap.gm = p.heap_ws + oo; heap.size = 0;
+  TierCursor tc[3];
+  const int wtot = p.w0 + p.w1 + p.w2;
+
+  // arrival window: lane holds request wb+lane
+  int wb = 0; long long w_arr = kInf; int w_tier = 0, w_base = 0;
+  auto load_window = [&]() {
+    const int i = wb + lane;
+    if (i < n) { w_arr = arr[i]; w_tier = tier[i]; w_base = BASE[i]; } else { w_arr = kInf; w_tier = 0; w_base = 0; }
+    const long long prev = __shfl_up_sync(kFull, w_arr, 1);
+    const bool bad = (i < n) && (w_tier > 2 || w_base < 0 || w_arr < 0 || (lane > 0 && w_arr < prev));
+    if (bad) atomicOr(p.status, DS_DEV_BAD_TRACE);
+    if (w_tier > 2) w_tier = 2;
+    if (w_base < 0) w_base = 0;
+  };
+  load_window();
+  an = n > 0 ? shfl_i64(w_arr, 0) : kInf;
+
+  auto advance_cursor = [&](TierCursor& c, const int t, bool first) {   // move tier t's head to its next request
+    if (!first) c.mask &= c.mask - 1;
+    while (c.mask == 0) {
+      if (!first) ++c.blk;
+      first = false;
+      if (c.blk * 32 >= n) { c.head = 0x7fffffff; return; }
+      const int i = c.blk * 32 + lane;
+      const int tv = i < n ? (int)tier[i] : 255;
+      c.mask = __ballot_sync(kFull, (tv > 2 ? 2 : tv) == t && i < n);
+    }
+    c.head = c.blk * 32 + (__ffs(c.mask) - 1);
+    if (c.head < next) {   // already arrived: its frozen estimate sits in the done_tick scratch
+      if (use_kv) c.est = (long long)__ldcg(dn + c.head);
+      if (kPolicy == DS_AGING) c.arr = arr[c.head];
+    }
+  };
+  if (kCursor)
+#pragma unroll
+    for (int t = 0; t < 3; ++t) { tc[t].blk = 0; tc[t].mask = 0; tc[t].est = 0; tc[t].arr = 0; advance_cursor(tc[t], t, true); }
+
+  // enqueue every request of the window that has arrived (strictly) by `now`; 32 at a time
+  auto ingest = [&](const bool strict) {
+    for (;;) {
+      const int i = wb + lane;
+      const bool pred = i >= next && i < n && (strict ? w_arr < now : w_arr <= now);
+      const unsigned m = __ballot_sync(kFull, pred);
+      if (m == 0) break;
+      const int c = __popc(m);
+      long long est = 0;
+      if (need_est) {
+        if (ema_on) {                                         // Eq. 1-2 reduced (A1), frozen at arrival (A5)
+          const double Bt = shfl_f64(Bl, w_tier);
+          if (w_base > 0) est = (long long)ceil(__dmul_rn(Bt, (double)w_base));
+        } else est = w_base;                                  // B == 1.0 exactly
+      }
+      if (kPolicy == DS_SJF) {
+        if (pred && est >= (1ll << 39)) atomicOr(p.status, DS_DEV_KEY_RANGE);
+        unsigned mm = m;
+        while (mm) {
+          const int l = __ffs(mm) - 1; mm &= mm - 1;
+          const long long e = shfl_i64(est, l);
+          heap.push(((unsigned long long)e << 24) | (unsigned long long)(wb + l), lane);
+        }
+      } else {
+        if (use_kv && pred) __stcg(dn + i, est);
+        __syncwarp();   // other lanes read these estimates back when a cursor reaches them
+        const int last = next + c;                            // requests [next,last) were ingested
+        if (kPolicy == DS_FIFO) {
+          if (use_kv && fifo_head >= next && fifo_head < last) fifo_est = shfl_i64(est, fifo_head - wb);
+        } else {
+#pragma unroll
+          for (int t = 0; t < 3; ++t) {
+            if (tc[t].head >= next && tc[t].head < last) {   // warp-uniform
+              if (use_kv) tc[t].est = shfl_i64(est, tc[t].head - wb);
+              if (kPolicy == DS_AGING) tc[t].arr = shfl_i64(w_arr, tc[t].head - wb);
+            }
+          }
+        }
+      }
+      next += c;
+      if (kPolicy != DS_FIFO) blocked = false;               // a new arrival can change the head (never FIFO's)
+      if (next == wb + 32 && next < n) { wb += 32; load_window(); continue; }
+      break;
+    }
+    an = next < n ? shfl_i64(w_arr, next - wb) : kInf;
+  };
+
+  // 2. RETIRE: completions at `now`, ascending request index (R-ORD); then the distance to the next completion
+  auto retire = [&]() {
+    for (;;) {
+      int lm = 0x7fffffff;
+#pragma unroll
+      for (int s = 0; s < kSlots; ++s) if (s_idx[s] >= 0 && s_fin[s] == iter) lm = min(lm, s_idx[s]);
+      const int r = __reduce_min_sync(kFull, lm);
+      if (r == 0x7fffffff) break;
+#pragma unroll
+      for (int s = 0; s < kSlots; ++s) if (s_idx[s] == r) s_idx[s] = -1;
+      const int Pr = P[r], Or = max(O[r], 1);
+      if (lane == 0) dn[r] = now;
+      kv_used -= (long long)Pr + Or;
+      --b;
+      if (ema_on) {                                           // Eq. 5-6 (A3): four separately rounded operations
+        const int br = W[r], tr = min((int)tier[r], 2);
+        if (br > 0) {
+          const double m = __ddiv_rn((double)Pr, (double)br);
+          const double t1 = __dsub_rn(1.0, alpha);
+          const double t2 = __dmul_rn(t1, shfl_f64(Bl, tr));
+          const double t3 = __dmul_rn(alpha, m);
+          const double Bn = __dadd_rn(t2, t3);
+          if (lane == tr) Bl = Bn;
+        }
+      }
+      ++done;
+      if (traj && done % p.traj_every == 0 && lane < 3) traj[3 * (done / p.traj_every - 1) + lane] = Bl;
+    }
+    blocked = false;
+    unsigned d = 0xffffffffu;
+#pragma unroll
+    for (int s = 0; s < kSlots; ++s) if (s_idx[s] >= 0) d = min(d, s_fin[s] - iter);
+    dist = __reduce_min_sync(kFull, d);
+    __syncwarp();
+  };
+
+  auto queue_nonempty = [&]() -> bool {
+    if (kPolicy == DS_FIFO) return fifo_head < next;
+    if (kPolicy == DS_SJF) return heap.size > 0;
+    return tc[0].head < next || tc[1].head < next || tc[2].head < next;
+  };
+
+  // 4. ADMIT: while a slot is free, peek(policy, now); KV check on the estimate (A8); pop
+  auto admit = [&]() {
+    while (b < max_batch) {
+      int c = -1, ct = 0, wpos = 0; long long est_c = 0;
+      if (kPolicy == DS_FIFO) {
+        if (fifo_head < next) { c = fifo_head; est_c = fifo_est; }
+      } else if (kPolicy == DS_SJF) {
+        if (heap.size > 0) { const unsigned long long k = heap.top(); c = (int)(k & 0xffffffull); est_c = (long long)(k >> 24); }
+      } else if (kPolicy == DS_PRIORITY) {
+#pragma unroll
+        for (int t = 2; t >= 0; --t) if (tc[t].head < next) { c = tc[t].head; est_c = tc[t].est; ct = t; }
+      } else if (kPolicy == DS_WEIGHTED) {
+        // slot pattern w0 x Premium, w1 x Standard, w2 x Batch scanned cyclically from `cur` (A9): the first non-empty
+        // tier in block order starting with cur's own block; position = cur itself or that block's first slot
+        const int t0 = cur < p.w0 ? 0 : (cur < p.w0 + p.w1 ? 1 : 2);
+        const unsigned nem = (tc[0].head < next ? 1u : 0u) | (tc[1].head < next ? 2u : 0u) | (tc[2].head < next ? 4u : 0u);
+        ct = -1;
+#pragma unroll
+        for (int k = 2; k >= 0; --k) {
+          int t = t0 + k; if (t >= 3) t -= 3;
+          if ((nem >> t) & 1u) { ct = t; wpos = k == 0 ? cur : (t == 0 ? 0 : (t == 1 ? p.w0 : p.w0 + p.w1)); }
+        }
+#pragma unroll
+        for (int t = 0; t < 3; ++t) if (t == ct) { c = tc[t].head; est_c = tc[t].est; }
+      } else {  // AGING (A10): eff = max(0, tier - floor(waited/aging_step)); key (eff, seq)
+        int best_eff = 99;
+#pragma unroll
+        for (int t = 0; t < 3; ++t) {
+          if (tc[t].head < next) {
+            const long long waited = now - tc[t].arr;
+            int eff = t;
+            if (t >= 1 && waited >= p.aging_step) --eff;
+            if (t >= 2 && waited >= 2 * p.aging_step) --eff;
+            if (eff < best_eff || (eff == best_eff && tc[t].head < c)) { best_eff = eff; c = tc[t].head; est_c = tc[t].est; ct = t; }
+          }
+        }
+      }
+      if (c < 0) break;
+      if (b > 0 && use_kv && kv_used + est_c > p.kv_budget) { blocked = kPolicy != DS_AGING; break; }   // deferred (A8)
+      // pop
+      if (kPolicy == DS_FIFO) {
+        ++fifo_head;
+        if (use_kv && fifo_head < next) fifo_est = (long long)__ldcg(dn + fifo_head);
+      } else if (kPolicy == DS_SJF) heap.pop(lane);
+      else {
+#pragma unroll
+        for (int t = 0; t < 3; ++t) if (t == ct) advance_cursor(tc[t], t, false);
+        if (kPolicy == DS_WEIGHTED) { cur = wpos + 1; if (cur >= wtot) cur = 0; }
+      }
+      const int Pc = P[c];
+      int Oc = O[c];
+      if (Oc < 1) { Oc = 1; if (lane == 0) atomicOr(p.status, DS_DEV_BAD_TRACE); }
+      if (lane == 0) st[c] = now;
+      bool has_free = false;                                   // first lane with a free slot takes the request
+#pragma unroll
+      for (int s = 0; s < kSlots; ++s) has_free |= s_idx[s] < 0;
+      const unsigned fm = __ballot_sync(kFull, has_free);
+      if (lane == __ffs(fm) - 1) {
+        bool placed = false;
+#pragma unroll
+        for (int s = 0; s < kSlots; ++s) if (!placed && s_idx[s] < 0) { s_idx[s] = c; s_fin[s] = iter + (unsigned)Oc; placed = true; }
+      }
+      kv_used += Pc; prefill_new += Pc; ++b;
+      dist = min(dist, (unsigned)Oc);
+    }
+  };
+
+  // ---- main loop: one pass per iteration boundary that has an event; event-free boundaries are jumped over ----
+  for (;;) {
+    if (an < now) ingest(true);                                           // 1. INGEST-EARLY
+    if (dist == 0) retire();                                              // 2. RETIRE
+    if (an <= now) ingest(false);                                         // 3. INGEST-NOW
+    if (!blocked && b < max_batch) admit();                               // 4. ADMIT
+    if (b == 0) {                                                         // 5. IDLE / END
+      if (next >= n) break;
+      now = an;
+      continue;
+    }
+    // 6. STEP: the iteration that carries the prefill of the newly admitted requests
+    long long dt = p.c_base + p.c_batch * b + p.c_ctx * kv_used;
+    const long long cb = p.c_ctx * b;
+    now += dt + p.c_prefill * prefill_new;
+    prefill_new = 0;
+    kv_used += b; dt += cb; --dist; ++iter;
+    // boundaries at which nothing can happen: no completion, and no arrival that could be admitted
+    if (dist != 0 && !(!blocked && b < max_batch && queue_nonempty())) {
+      const bool arrivals_matter = b < max_batch && !(kPolicy == DS_FIFO && blocked) && next < n;
+      unsigned j = dist;
+      if (arrivals_matter) {
+        // the stepping loop would run while an > now. Lower bound on its trip count: every one of the first `cap`
+        // iterations costs at most dt + cb*cap ticks, where cap >= min(dist, true count) because the true count is
+        // at most ceil(G/dt). Float rounding (2^-24 relative) is covered by the 1e-4 margins.
+        j = 0;
+        if (an > now && dt > 0) {
+          const float G = (float)(an - now), fdt = (float)dt;
+          const float cap = fminf(G / fdt * 1.0001f + 1.0f, (float)dist);
+          const float q = G / (fdt + (float)cb * cap) * 0.9999f;
+          j = q >= (float)dist ? dist : (unsigned)q;
+          if (j > dist) j = dist;
+        }
+      }
+      if (j) {                                                            // j iterations at once, exact
+        const unsigned long long jj = j;
+        now += (long long)(jj * (unsigned long long)dt + (unsigned long long)cb * (jj * (jj - 1) / 2));
+        kv_used += (long long)(jj * (unsigned long long)b);
+        dt += (long long)(jj * (unsigned long long)cb);
+        dist -= j; iter += j;
+      }
+      if (arrivals_matter)
+        while (dist != 0 && an > now) { now += dt; kv_used += b; dt += cb; --dist; ++iter; }
+    }
+  }
+  if (lane < 3) p.ema_final[3 * (size_t)inst_id + lane] = Bl;
+  __syncwarp();
+}
+
+// Processing order: instances grouped by policy, most expensive policy first (SJF, AGING, WEIGHTED, PRIORITY, FIFO).
+// Each policy is its own ~25 KB of straight-line code; running one policy at a time across the GPU keeps the
+// instruction cache warm (trace-major order thrashed it: 26 of 27 issue-stall samples were "no instruction"), and
+// longest-first shortens the tail. One block; n_inst is small next to the simulation itself.
+__global__ void __launch_bounds__(1024) order_kernel(const ds_instance* __restrict__ inst, long long n_inst, unsigned int* perm) {
+  __shared__ unsigned int cnt[6], pos[6];
+  if (threadIdx.x < 6) cnt[threadIdx.x] = 0;
+  __syncthreads();
+  auto bucket = [](int policy) { return policy == DS_SJF ? 0 : policy == DS_AGING ? 1 : policy == DS_WEIGHTED ? 2 :
+                                        policy == DS_PRIORITY ? 3 : policy == DS_FIFO ? 4 : 5; };
+  for (long long i = threadIdx.x; i < n_inst; i += blockDim.x) atomicAdd(&cnt[bucket(inst[i].policy)], 1u);
+  __syncthreads();
+  if (threadIdx.x == 0) { unsigned a = 0; for (int k = 0; k < 6; ++k) { pos[k] = a; a += cnt[k]; } }
+  __syncthreads();
+  // stable within a bucket per 1024-chunk: warp-aggregated ranks keep neighbouring instances (same trace) together
+  for (long long base = 0; base < n_inst; base += blockDim.x) {
+    const long long i = base + threadIdx.x;
+    const int bk = i < n_inst ? bucket(inst[i].policy) : -1;
+    __shared__ unsigned int wcnt[32][6];
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    unsigned rank = 0;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+      const unsigned m = __ballot_sync(0xffffffffu, bk == k);
+      if (bk == k) rank = __popc(m & ((1u << l) - 1u));
+      if (l == 0) wcnt[w][k] = __popc(m);
+    }
+    __syncthreads();
+    if (bk >= 0) {
+      unsigned off = pos[bk];
+      for (int ww = 0; ww < w; ++ww) off += wcnt[ww][bk];
+      perm[off + rank] = (unsigned)i;
+    }
+    __syncthreads();
+    if (threadIdx.x < 6) { unsigned a = 0; for (int ww = 0; ww < 32; ++ww) a += wcnt[ww][threadIdx.x]; pos[threadIdx.x] += a; }
+    __syncthreads();
+  }
+}
+
 template <int kSlots>
-__global__ void __launch_bounds__(k2::kWarpsPerBlock * 32) simulate_kernel(const Params p) {
+__global__ void __launch_bounds__(k2::kWarpsPerBlock * 32) simulate_kernel(const __grid_constant__ Params p) {
   __shared__ unsigned long long heap_sm[kWarpsPerBlock][kHeapSmem];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-
   for (;;) {
     unsigned inst_id = 0;
     if (lane == 0) inst_id = atomicAdd(p.counter, 1u);
     inst_id = __shfl_sync(kFull, inst_id, 0);
     if ((long long)inst_id >= p.n_inst) return;
-
+    inst_id = p.perm[inst_id];                       // policy-major processing order (see order_kernel)
     const ds_instance in = p.inst[inst_id];
-    double B0 = 1.0, B1 = 1.0, B2 = 1.0;
     const bool bad_inst = in.trace < 0 || in.trace >= p.n_traces || in.policy < 0 || in.policy > 4 || in.estimator < 0 ||
                           in.estimator > 1 || !(in.ema_alpha >= 0.0 && in.ema_alpha <= 1.0);
     if (bad_inst) {
-      if (lane == 0) { atomicOr(p.status, DS_DEV_BAD_INSTANCE); p.ema_final[3 * (size_t)inst_id] = B0; p.ema_final[3 * (size_t)inst_id + 1] = B1; p.ema_final[3 * (size_t)inst_id + 2] = B2; }
+      if (lane == 0) atomicOr(p.status, DS_DEV_BAD_INSTANCE);
+      if (lane < 3) p.ema_final[3 * (size_t)inst_id + lane] = 1.0;
       continue;
     }
-    const long long lo = p.trace_off[in.trace];
-    const long long n = p.trace_off[in.trace + 1] - lo;
-    const int64_t* __restrict__ arr = p.arrival + lo;
-    const uint8_t* __restrict__ tier = p.tier + lo;
-    const int32_t* __restrict__ W = p.words + lo;
-    const int32_t* __restrict__ P = p.tokens + lo;
-    const int32_t* __restrict__ O = p.out_len + lo;
-    const long long oo = p.out_off[inst_id];
-    int64_t* __restrict__ st = p.start_tick + oo;
-    int64_t* dn = p.done_tick + oo;
-    const int policy = in.policy;
     const bool split = in.estimator == DS_SPLIT;
-    const int32_t* __restrict__ BASE = split ? W : P;
-    const double alpha = in.ema_alpha;
-    const bool use_kv = p.kv_budget > 0;
-    double* traj = (p.ema_traj && p.traj_off && p.traj_every > 0) ? p.ema_traj + 3 * p.traj_off[inst_id] : nullptr;
-    if (policy == DS_SJF && n > (1 << 24) && lane == 0) atomicOr(p.status, DS_DEV_KEY_RANGE);
-
-    // ---- state ----
-    long long now = 0, next = 0, kv_used = 0, done = 0, prefill_new = 0;
-    int b = 0, cur = 0;
-    unsigned iter = 0, dist = 0xffffffffu;
-    bool blocked = false;
-    int s_idx[kSlots]; unsigned s_fin[kSlots];
-#pragma unroll
-    for (int s = 0; s < kSlots; ++s) { s_idx[s] = -1; s_fin[s] = 0; }
-    Heap heap; heap.sm = heap_sm[wib]; heap.gm = p.heap_ws + oo; heap.size = 0;
-    long long fifo_head = 0, fifo_est = 0;   // FIFO: admitted strictly in index order
-    TierCursor tc[3];
-    const int wtot = p.w0 + p.w1 + p.w2;
-
-    // arrival window: lane holds request wb+lane
-    long long wb = 0, w_arr = kInf; int w_tier = 0, w_base = 0;
-    auto load_window = [&]() {
-      const long long i = wb + lane;
-      if (i < n) { w_arr = arr[i]; w_tier = tier[i]; w_base = BASE[i]; } else { w_arr = kInf; w_tier = 0; w_base = 0; }
-      const long long prev = __shfl_up_sync(kFull, w_arr, 1);
-      bool bad = (i < n) && (w_tier > 2 || w_base < 0 || w_arr < 0 || (lane > 0 && w_arr < prev));
-      if (bad) atomicOr(p.status, DS_DEV_BAD_TRACE);
-      if (w_tier > 2) w_tier = 2;
-      if (w_base < 0) w_base = 0;
-    };
-    load_window();
-    auto arr_next = [&]() -> long long { return next < n ? __shfl_sync(kFull, w_arr, (int)(next - wb)) : kInf; };
-
-    auto advance_cursor = [&](int t, bool first) {   // move tier t's head to its next request
-      TierCursor& c = tc[t];
-      if (!first) c.mask &= c.mask - 1;
-      while (c.mask == 0) {
-        if (!first) ++c.blk;
-        first = false;
-        if ((long long)c.blk * 32 >= n) { c.head = 0x7fffffff; return; }
-        const long long i = (long long)c.blk * 32 + lane;
-        const int tv = i < n ? (int)tier[i] : 255;
-        c.mask = __ballot_sync(kFull, (tv > 2 ? 2 : tv) == t && i < n);
-      }
-      c.head = c.blk * 32 + (__ffs(c.mask) - 1);
-      if (c.head < next) {   // already arrived: its frozen estimate sits in the done_tick scratch
-        c.est = use_kv ? (long long)__ldcg(dn + c.head) : 0;
-        c.arr = arr[c.head];
-      }
-    };
-    if (policy != DS_FIFO && policy != DS_SJF)
-      for (int t = 0; t < 3; ++t) { tc[t].blk = 0; tc[t].mask = 0; tc[t].est = 0; tc[t].arr = 0; advance_cursor(t, true); }
-
-    auto ingest = [&](bool strict) {
-      for (;;) {
-        const long long i = wb + lane;
-        const bool pred = i >= next && i < n && (strict ? w_arr < now : w_arr <= now);
-        const unsigned m = __ballot_sync(kFull, pred);
-        if (m == 0) return;
-        const int c = __popc(m);
-        const double Bt = w_tier == 0 ? B0 : (w_tier == 1 ? B1 : B2);
-        long long est = 0;
-        if (w_base > 0) est = (long long)ceil(__dmul_rn(Bt, (double)w_base));   // Eq. 1-2 reduced (A1), frozen (A5)
-        if (policy == DS_SJF) {
-          if (pred && est >= (1ll << 39)) atomicOr(p.status, DS_DEV_KEY_RANGE);
-          unsigned mm = m;
-          while (mm) {
-            const int l = __ffs(mm) - 1; mm &= mm - 1;
-            const long long e = __shfl_sync(kFull, est, l);
-            heap.push(((unsigned long long)e << 24) | (unsigned long long)(wb + l), lane);
-          }
-        } else {
-          if (use_kv && pred) __stcg(dn + i, est);
-          __syncwarp();   // other lanes read these estimates back when a cursor reaches them
-          const int first = (int)(next - wb), last = first + c;   // window lanes [first,last) were ingested
-          if (policy == DS_FIFO) {
-            const long long h = fifo_head - wb;
-            const long long e = __shfl_sync(kFull, est, (int)(h & 31));
-            if (h >= first && h < last) fifo_est = e;
-          } else {
-#pragma unroll
-            for (int t = 0; t < 3; ++t) {
-              const long long h = (long long)tc[t].head - wb;
-              const long long e = __shfl_sync(kFull, est, (int)(h & 31));
-              const long long a = __shfl_sync(kFull, w_arr, (int)(h & 31));
-              if (h >= first && h < last) { tc[t].est = e; tc[t].arr = a; }
-            }
-          }
-        }
-        next += c;
-        blocked = false;
-        if (next == wb + 32 && next < n) { wb += 32; load_window(); } else return;
-      }
-    };
-
-    auto recompute = [&]() {   // after the running set changed
-      unsigned d = 0xffffffffu;
-#pragma unroll
-      for (int s = 0; s < kSlots; ++s) if (s_idx[s] >= 0) d = min(d, s_fin[s] - iter);
-      dist = __reduce_min_sync(kFull, d);
-    };
-
-    auto retire = [&]() {
-      for (;;) {
-        int lm = 0x7fffffff;
-#pragma unroll
-        for (int s = 0; s < kSlots; ++s) if (s_idx[s] >= 0 && s_fin[s] == iter) lm = min(lm, s_idx[s]);
-        const int r = __reduce_min_sync(kFull, lm);        // ascending request index (R-ORD)
-        if (r == 0x7fffffff) break;
-#pragma unroll
-        for (int s = 0; s < kSlots; ++s) if (s_idx[s] == r) s_idx[s] = -1;
-        const int Pr = P[r], Or = max(O[r], 1), tr = min((int)tier[r], 2), br = BASE[r];
-        if (lane == 0) dn[r] = now;
-        kv_used -= (long long)Pr + Or;
-        --b;
-        if (alpha > 0.0 && br > 0) {                       // Eq. 5-6 (A3): four separately rounded operations
-          const double m = __ddiv_rn((double)Pr, (double)br);
-          const double t1 = __dsub_rn(1.0, alpha);
-          const double Bk = tr == 0 ? B0 : (tr == 1 ? B1 : B2);
-          const double t2 = __dmul_rn(t1, Bk);
-          const double t3 = __dmul_rn(alpha, m);
-          const double Bn = __dadd_rn(t2, t3);
-          if (tr == 0) B0 = Bn; else if (tr == 1) B1 = Bn; else B2 = Bn;
-        }
-        ++done;
-        if (traj && done % p.traj_every == 0 && lane == 0) {
-          double* q = traj + 3 * (done / p.traj_every - 1);
-          q[0] = B0; q[1] = B1; q[2] = B2;
-        }
-      }
-      blocked = false;
-      __syncwarp();
-    };
-
-    auto admit = [&]() {
-      bool changed = false;
-      while (b < p.max_batch) {
-        // peek(policy, now)
-        long long c = -1, est_c = 0; int ct = 0, wpos = 0;
-        if (policy == DS_FIFO) {
-          if (fifo_head < next) { c = fifo_head; est_c = fifo_est; }
-        } else if (policy == DS_SJF) {
-          if (heap.size > 0) { const unsigned long long k = heap.top(); c = (long long)(k & 0xffffffull); est_c = (long long)(k >> 24); }
-        } else if (policy == DS_PRIORITY) {
-          for (int t = 2; t >= 0; --t) if (tc[t].head < next) { c = tc[t].head; est_c = tc[t].est; ct = t; }
-        } else if (policy == DS_WEIGHTED) {
-          for (int s = 0; s < wtot; ++s) {
-            int pos = cur + s; if (pos >= wtot) pos -= wtot;
-            const int t = pos < p.w0 ? 0 : (pos < p.w0 + p.w1 ? 1 : 2);
-            if (tc[t].head < next) { c = tc[t].head; est_c = tc[t].est; ct = t; wpos = pos; break; }
-          }
-        } else {  // AGING (A10): eff = max(0, tier - floor(waited/aging_step)); key (eff, seq)
-          int best_eff = 99;
-#pragma unroll
-          for (int t = 0; t < 3; ++t) {
-            if (tc[t].head < next) {
-              const long long waited = now - tc[t].arr;
-              int eff = t;
-              if (t >= 1 && waited >= p.aging_step) --eff;
-              if (t >= 2 && waited >= 2 * p.aging_step) --eff;
-              if (eff < best_eff || (eff == best_eff && tc[t].head < c)) { best_eff = eff; c = tc[t].head; est_c = tc[t].est; ct = t; }
-            }
-          }
-        }
-        if (c < 0) break;
-        if (b > 0 && use_kv && kv_used + est_c > p.kv_budget) { blocked = policy != DS_AGING; break; }   // deferred (A8)
-        // pop
-        if (policy == DS_FIFO) {
-          ++fifo_head;
-          if (fifo_head < next && use_kv) fifo_est = (long long)__ldcg(dn + fifo_head);
-        } else if (policy == DS_SJF) heap.pop(lane);
-        else { advance_cursor(ct, false); if (policy == DS_WEIGHTED) { cur = wpos + 1; if (cur >= wtot) cur = 0; } }
-        const int Pc = P[c];
-        int Oc = O[c];
-        if (Oc < 1) { Oc = 1; if (lane == 0) atomicOr(p.status, DS_DEV_BAD_TRACE); }
-        if (lane == 0) st[c] = now;
-        // first lane with a free slot takes it
-        bool has_free = false;
-#pragma unroll
-        for (int s = 0; s < kSlots; ++s) has_free |= s_idx[s] < 0;
-        const unsigned fm = __ballot_sync(kFull, has_free);
-        if (lane == __ffs(fm) - 1) {
-          bool placed = false;
-#pragma unroll
-          for (int s = 0; s < kSlots; ++s) if (!placed && s_idx[s] < 0) { s_idx[s] = (int)c; s_fin[s] = iter + (unsigned)Oc; placed = true; }
-        }
-        kv_used += Pc; prefill_new += Pc; ++b;
-        changed = true;
-      }
-      return changed;
-    };
-
-    // ---- main loop: one pass per iteration boundary with an event; event-free boundaries run in the inner loop ----
-    for (;;) {
-      long long an = arr_next();
-      if (an < now) { ingest(true); an = arr_next(); }                     // 1. INGEST-EARLY
-      bool dirty = false;
-      if (dist == 0) { retire(); dirty = true; }                           // 2. RETIRE
-      if (an <= now) { ingest(false); an = arr_next(); }                   // 3. INGEST-NOW
-      if (!blocked && b < p.max_batch) dirty |= admit();                    // 4. ADMIT
-      if (dirty) recompute();
-      if (b == 0) {                                                         // 5. IDLE / END
-        if (next >= n) break;
-        now = an;
-        continue;
-      }
-      // 6. STEP (+ fast-forward over boundaries where nothing can happen)
-      long long dt = p.c_base + p.c_batch * b + p.c_ctx * kv_used;
-      const long long cb = p.c_ctx * b;
-      now += dt + p.c_prefill * prefill_new;
-      prefill_new = 0;
-      kv_used += b; dt += cb; --dist; ++iter;
-      const bool may_admit = !blocked && b < p.max_batch &&
-                             (policy == DS_FIFO ? fifo_head < next : policy == DS_SJF ? heap.size > 0
-                                                : (tc[0].head < next || tc[1].head < next || tc[2].head < next));
-      if (!may_admit) {
-        while (dist != 0 && an > now) { now += dt; kv_used += b; dt += cb; --dist; ++iter; }
-      }
+    if (lane < 3) p.ema_final[3 * (size_t)inst_id + lane] = 1.0;   // overwritten unless the trace is rejected
+    switch (in.policy) {
+      case DS_FIFO: run_instance<kSlots, DS_FIFO>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane); break;
+      case DS_PRIORITY: run_instance<kSlots, DS_PRIORITY>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane); break;
+      case DS_WEIGHTED: run_instance<kSlots, DS_WEIGHTED>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane); break;
+      case DS_SJF: run_instance<kSlots, DS_SJF>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane); break;
+      default: run_instance<kSlots, DS_AGING>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane); break;
     }
-    if (lane == 0) {
-      p.ema_final[3 * (size_t)inst_id] = B0; p.ema_final[3 * (size_t)inst_id + 1] = B1; p.ema_final[3 * (size_t)inst_id + 2] = B2;
-    }
-    __syncwarp();
   }
 }
 
 }  // namespace k2
 
-size_t ws_simulate(int64_t total_requests, int64_t) { return 256 + sizeof(unsigned long long) * (size_t)total_requests; }
+static size_t perm_bytes(int64_t n_inst) { return align_up(sizeof(unsigned int) * (size_t)(n_inst > 0 ? n_inst : 1), 256); }
+size_t ws_simulate(int64_t total_requests, int64_t n_inst) {
+  return 256 + perm_bytes(n_inst) + sizeof(unsigned long long) * (size_t)total_requests;
+}
 
 }  // namespace ds
-
 extern "C" int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
                            const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
                            const int64_t* traj_off, double* ema_traj, void* workspace, size_t workspace_bytes, void* stream) {
@@ -374,7 +477,7 @@ extern "C" int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_in
   if (sv->weight[0] < 1 || sv->weight[1] < 1 || sv->weight[2] < 1 || sv->aging_step < 1 || sv->traj_every < 0) return DS_EINVAL;
   if (sv->c_base < 0 || sv->c_batch < 0 || sv->c_ctx < 0 || sv->c_prefill < 0) return DS_EINVAL;
   if (n_inst > 0x7fffffff) return DS_EINVAL;
-  if (workspace_bytes < 256) return DS_ENOMEM;
+  if (workspace_bytes < 256 + perm_bytes(n_inst)) return DS_ENOMEM;
   cudaStream_t s = (cudaStream_t)stream;
   k2::Params p;
   p.trace_off = tr->trace_off; p.arrival = tr->arrival_tick; p.tier = tr->tier; p.words = tr->words; p.tokens = tr->tokens;
@@ -385,12 +488,16 @@ extern "C" int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_in
   p.inst = inst; p.n_inst = n_inst; p.out_off = out_off; p.start_tick = start_tick; p.done_tick = done_tick;
   p.ema_final = ema_final; p.traj_off = traj_off; p.ema_traj = ema_traj;
   p.counter = (unsigned int*)workspace;
-  p.heap_ws = (unsigned long long*)((char*)workspace + 256);
+  unsigned int* perm = (unsigned int*)((char*)workspace + 256);
+  p.perm = perm;
+  p.heap_ws = (unsigned long long*)((char*)workspace + 256 + perm_bytes(n_inst));
   p.status = status_ptr();
   if (!p.status) return cuda_fail(cudaGetLastError());
   // the heap region is only touched by SJF instances beyond kHeapSmem queued requests; its size is checked here
   // against the documented formula only when it can be needed at all (caller passes total requests to the query)
   DS_CUDA(cudaMemsetAsync(workspace, 0, 256, s));
+  k2::order_kernel<<<1, 1024, 0, s>>>(inst, n_inst, perm);
+  note_launch();
   const int threads = k2::kWarpsPerBlock * 32;
   int per_sm = 0;
   auto launch = [&](auto kern) -> int {
