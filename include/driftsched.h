@@ -76,7 +76,7 @@ typedef struct {              /* SoA request records, traces concatenated; HOST 
 typedef struct {              /* continuous-batching server model, BASELINE.json:configs[0] */
   int32_t max_batch;           /* 1..256 */
   int64_t kv_budget;           /* tokens; <= 0 means unlimited */
-  int64_t c_base, c_batch, c_ctx, c_prefill; /* iteration cost = c_base + c_batch*b + c_ctx*sum(ctx) + c_prefill*sum(P_new) */
+  int64_t c_base, c_batch, c_ctx, c_prefill; /* each in [0, 2^31): iteration cost = c_base + c_batch*b + c_ctx*sum(ctx) + c_prefill*sum(P_new) */
   int32_t weight[3];           /* Weighted policy slots per tier, each >= 1: {4,2,1} configs, {5,3,2} PAPER.md:234 */
   int64_t aging_step;          /* ticks waited per promoted tier level, >= 1 */
   int32_t traj_every;          /* 0 = no EMA trajectory; k = sample B[0..2] every k completions */

@@ -37,7 +37,7 @@ constexpr unsigned kFull = 0xffffffffu;
 struct Params {
   const int64_t* trace_off; const int64_t* arrival; const uint8_t* tier; const int32_t* words; const int32_t* tokens;
   const int32_t* out_len; int64_t n_traces;
-  int32_t max_batch; int64_t kv_budget, c_base, c_batch, c_ctx, c_prefill; int32_t w0, w1, w2; int64_t aging_step;
+  int32_t max_batch; int64_t kv_budget; uint32_t c_base, c_batch, c_ctx, c_prefill; /* < 2^31, checked by ds_simulate */ int32_t w0, w1, w2; int64_t aging_step;
   int32_t traj_every;
   const ds_instance* inst; int64_t n_inst; const int64_t* out_off; int64_t* start_tick; int64_t* done_tick;
   double* ema_final; const int64_t* traj_off; double* ema_traj;
@@ -241,7 +241,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
 #pragma unroll
       for (int s = 0; s < kSlots; ++s) if (s_idx[s] == r) s_idx[s] = -1;
       const int Pr = P[r], Or = max(O[r], 1);
-      if (lane == 0) dn[r] = now;
+      dn[r] = now;                                            // every lane, same address and value: one store, no branch
       kv_used -= (long long)Pr + Or;
       --b;
       if (ema_on) {                                           // Eq. 5-6 (A3): four separately rounded operations
@@ -324,7 +324,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       const int Pc = P[c];
       int Oc = O[c];
       if (Oc < 1) { Oc = 1; if (lane == 0) atomicOr(p.status, DS_DEV_BAD_TRACE); }
-      if (lane == 0) st[c] = now;
+      st[c] = now;                                             // every lane, same address and value
       bool has_free = false;                                   // first lane with a free slot takes the request
 #pragma unroll
       for (int s = 0; s < kSlots; ++s) has_free |= s_idx[s] < 0;
@@ -341,9 +341,11 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
 
   // ---- main loop: one pass per iteration boundary that has an event; event-free boundaries are jumped over ----
   for (;;) {
-    if (an < now) ingest(true);                                           // 1. INGEST-EARLY
-    if (dist == 0) retire();                                              // 2. RETIRE
-    if (an <= now) ingest(false);                                         // 3. INGEST-NOW
+#pragma unroll 1
+    for (int ph = 0; ph < 2; ++ph) {                                      // one copy of the ingest code for both phases
+      if (ph == 0 ? an < now : an <= now) ingest(ph == 0);                // 1. INGEST-EARLY / 3. INGEST-NOW
+      if (ph == 0 && dist == 0) retire();                                 // 2. RETIRE
+    }
     if (!blocked && b < max_batch) admit();                               // 4. ADMIT
     if (b == 0) {                                                         // 5. IDLE / END
       if (next >= n) break;
@@ -351,9 +353,10 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       continue;
     }
     // 6. STEP: the iteration that carries the prefill of the newly admitted requests
-    long long dt = p.c_base + p.c_batch * b + p.c_ctx * kv_used;
-    const long long cb = p.c_ctx * b;
-    now += dt + p.c_prefill * prefill_new;
+    long long dt = (long long)((unsigned long long)p.c_base + (unsigned long long)p.c_batch * (unsigned)b +
+                               (unsigned long long)kv_used * p.c_ctx);
+    const long long cb = (long long)((unsigned long long)p.c_ctx * (unsigned)b);
+    now += dt + (long long)((unsigned long long)prefill_new * p.c_prefill);
     prefill_new = 0;
     kv_used += b; dt += cb; --dist; ++iter;
     // boundaries at which nothing can happen: no completion, and no arrival that could be admitted
@@ -367,8 +370,8 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
         j = 0;
         if (an > now && dt > 0) {
           const float G = (float)(an - now), fdt = (float)dt;
-          const float cap = fminf(G / fdt * 1.0001f + 1.0f, (float)dist);
-          const float q = G / (fdt + (float)cb * cap) * 0.9999f;
+          const float cap = fminf(__fdividef(G, fdt) * 1.0001f + 1.0f, (float)dist);   // MUFU.RCP: 2 ulp, inside the margins
+          const float q = __fdividef(G, fdt + (float)cb * cap) * 0.9999f;
           j = q >= (float)dist ? dist : (unsigned)q;
           if (j > dist) j = dist;
         }
@@ -392,7 +395,8 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
 // Each policy is its own ~25 KB of straight-line code; running one policy at a time across the GPU keeps the
 // instruction cache warm (trace-major order thrashed it: 26 of 27 issue-stall samples were "no instruction"), and
 // longest-first shortens the tail. One block; n_inst is small next to the simulation itself.
-__global__ void __launch_bounds__(1024) order_kernel(const ds_instance* __restrict__ inst, long long n_inst, unsigned int* perm) {
+__global__ void __launch_bounds__(1024) order_kernel(const ds_instance* __restrict__ inst, long long n_inst, unsigned int* perm,
+                                                     unsigned int* hdr) {
   __shared__ unsigned int cnt[6], pos[6];
   if (threadIdx.x < 6) cnt[threadIdx.x] = 0;
   __syncthreads();
@@ -400,7 +404,11 @@ __global__ void __launch_bounds__(1024) order_kernel(const ds_instance* __restri
                                         policy == DS_PRIORITY ? 3 : policy == DS_FIFO ? 4 : 5; };
   for (long long i = threadIdx.x; i < n_inst; i += blockDim.x) atomicAdd(&cnt[bucket(inst[i].policy)], 1u);
   __syncthreads();
-  if (threadIdx.x == 0) { unsigned a = 0; for (int k = 0; k < 6; ++k) { pos[k] = a; a += cnt[k]; } }
+  if (threadIdx.x == 0) {   // hdr[0..5]: per-bucket work counters (zeroed by the host), hdr[8..14]: bucket starts in perm[]
+    unsigned a = 0;
+    for (int k = 0; k < 6; ++k) { pos[k] = a; hdr[8 + k] = a; a += cnt[k]; }
+    hdr[14] = a;
+  }
   __syncthreads();
   // stable within a bucket per 1024-chunk: warp-aggregated ranks keep neighbouring instances (same trace) together
   for (long long base = 0; base < n_inst; base += blockDim.x) {
@@ -431,12 +439,24 @@ template <int kSlots>
 __global__ void __launch_bounds__(k2::kWarpsPerBlock * 32) simulate_kernel(const __grid_constant__ Params p) {
   __shared__ unsigned long long heap_sm[kWarpsPerBlock][kHeapSmem];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  // Policy affinity per SM: every warp of an SM starts on bucket (smid % 5) and moves on cyclically when a bucket is
+  // empty, so that an SM executes one policy's code at a time (instruction-cache locality; buckets: SJF, AGING,
+  // WEIGHTED, PRIORITY, FIFO, invalid).
+  unsigned smid;
+  asm("mov.u32 %0, %%smid;" : "=r"(smid));
+  int bucket = (int)(smid % 5u), tries = 0;
   for (;;) {
-    unsigned inst_id = 0;
-    if (lane == 0) inst_id = atomicAdd(p.counter, 1u);
-    inst_id = __shfl_sync(kFull, inst_id, 0);
-    if ((long long)inst_id >= p.n_inst) return;
-    inst_id = p.perm[inst_id];                       // policy-major processing order (see order_kernel)
+    unsigned k = 0;
+    if (lane == 0) k = atomicAdd(p.counter + bucket, 1u);
+    k = __shfl_sync(kFull, k, 0);
+    const unsigned b0 = p.counter[8 + bucket], b1 = p.counter[9 + bucket];
+    if (k >= b1 - b0) {
+      if (++tries == 6) return;
+      bucket = bucket == 5 ? 0 : bucket + 1;
+      continue;
+    }
+    tries = 0;
+    const unsigned inst_id = p.perm[b0 + k];
     const ds_instance in = p.inst[inst_id];
     const bool bad_inst = in.trace < 0 || in.trace >= p.n_traces || in.policy < 0 || in.policy > 4 || in.estimator < 0 ||
                           in.estimator > 1 || !(in.ema_alpha >= 0.0 && in.ema_alpha <= 1.0);
@@ -476,14 +496,15 @@ extern "C" int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_in
   if (sv->max_batch < 1 || sv->max_batch > 256) return DS_EINVAL;
   if (sv->weight[0] < 1 || sv->weight[1] < 1 || sv->weight[2] < 1 || sv->aging_step < 1 || sv->traj_every < 0) return DS_EINVAL;
   if (sv->c_base < 0 || sv->c_batch < 0 || sv->c_ctx < 0 || sv->c_prefill < 0) return DS_EINVAL;
+  if (sv->c_base > 0x7fffffff || sv->c_batch > 0x7fffffff || sv->c_ctx > 0x7fffffff || sv->c_prefill > 0x7fffffff) return DS_EINVAL;
   if (n_inst > 0x7fffffff) return DS_EINVAL;
   if (workspace_bytes < 256 + perm_bytes(n_inst)) return DS_ENOMEM;
   cudaStream_t s = (cudaStream_t)stream;
   k2::Params p;
   p.trace_off = tr->trace_off; p.arrival = tr->arrival_tick; p.tier = tr->tier; p.words = tr->words; p.tokens = tr->tokens;
   p.out_len = tr->out_len; p.n_traces = tr->n_traces;
-  p.max_batch = sv->max_batch; p.kv_budget = sv->kv_budget; p.c_base = sv->c_base; p.c_batch = sv->c_batch; p.c_ctx = sv->c_ctx;
-  p.c_prefill = sv->c_prefill; p.w0 = sv->weight[0]; p.w1 = sv->weight[1]; p.w2 = sv->weight[2]; p.aging_step = sv->aging_step;
+  p.max_batch = sv->max_batch; p.kv_budget = sv->kv_budget; p.c_base = (uint32_t)sv->c_base; p.c_batch = (uint32_t)sv->c_batch; p.c_ctx = (uint32_t)sv->c_ctx;
+  p.c_prefill = (uint32_t)sv->c_prefill; p.w0 = sv->weight[0]; p.w1 = sv->weight[1]; p.w2 = sv->weight[2]; p.aging_step = sv->aging_step;
   p.traj_every = sv->traj_every;
   p.inst = inst; p.n_inst = n_inst; p.out_off = out_off; p.start_tick = start_tick; p.done_tick = done_tick;
   p.ema_final = ema_final; p.traj_off = traj_off; p.ema_traj = ema_traj;
@@ -496,7 +517,7 @@ extern "C" int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_in
   // the heap region is only touched by SJF instances beyond kHeapSmem queued requests; its size is checked here
   // against the documented formula only when it can be needed at all (caller passes total requests to the query)
   DS_CUDA(cudaMemsetAsync(workspace, 0, 256, s));
-  k2::order_kernel<<<1, 1024, 0, s>>>(inst, n_inst, perm);
+  k2::order_kernel<<<1, 1024, 0, s>>>(inst, n_inst, perm, (unsigned int*)workspace);
   note_launch();
   const int threads = k2::kWarpsPerBlock * 32;
   int per_sm = 0;
