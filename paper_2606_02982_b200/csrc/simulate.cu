@@ -362,29 +362,35 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
     // boundaries at which nothing can happen: no completion, and no arrival that could be admitted
     if (dist != 0 && !(!blocked && b < max_batch && queue_nonempty())) {
       const bool arrivals_matter = b < max_batch && !(kPolicy == DS_FIFO && blocked) && next < n;
-      unsigned j = dist;
-      if (arrivals_matter) {
-        // the stepping loop would run while an > now. Lower bound on its trip count: every one of the first `cap`
-        // iterations costs at most dt + cb*cap ticks, where cap >= min(dist, true count) because the true count is
-        // at most ceil(G/dt). Float rounding (2^-24 relative) is covered by the 1e-4 margins.
-        j = 0;
+      // tick of the last boundary before the completion boundary: the stepping loop "while (an > now) step" runs all
+      // `dist` iterations iff an > t_last
+      const unsigned long long dm1 = dist - 1;
+      const long long t_last = now + (long long)(dm1 * (unsigned long long)dt + (unsigned long long)cb * (dm1 * (dm1 - 1) / 2));
+      if (!arrivals_matter || an > t_last) {                              // next event is the completion: exact jump
+        now = t_last + dt + (long long)(dm1 * (unsigned long long)cb);
+        kv_used += (long long)((unsigned long long)dist * (unsigned)b);
+        iter += dist; dist = 0;
+      } else {
+        // next event is an arrival. Lower bound on the stepping loop's trip count: every one of the first `cap`
+        // iterations costs at most dt + cb*cap ticks, where cap >= the true count because the true count is at most
+        // ceil(G/dt). Float rounding (2^-22 relative with MUFU.RCP) is covered by the 1e-4 margins.
+        unsigned j = 0;
         if (an > now && dt > 0) {
           const float G = (float)(an - now), fdt = (float)dt;
-          const float cap = fminf(__fdividef(G, fdt) * 1.0001f + 1.0f, (float)dist);   // MUFU.RCP: 2 ulp, inside the margins
+          const float cap = fminf(__fdividef(G, fdt) * 1.0001f + 1.0f, (float)dist);
           const float q = __fdividef(G, fdt + (float)cb * cap) * 0.9999f;
           j = q >= (float)dist ? dist : (unsigned)q;
           if (j > dist) j = dist;
         }
-      }
-      if (j) {                                                            // j iterations at once, exact
-        const unsigned long long jj = j;
-        now += (long long)(jj * (unsigned long long)dt + (unsigned long long)cb * (jj * (jj - 1) / 2));
-        kv_used += (long long)(jj * (unsigned long long)b);
-        dt += (long long)(jj * (unsigned long long)cb);
-        dist -= j; iter += j;
-      }
-      if (arrivals_matter)
+        if (j) {                                                          // j iterations at once, exact
+          const unsigned long long jj = j;
+          now += (long long)(jj * (unsigned long long)dt + (unsigned long long)cb * (jj * (jj - 1) / 2));
+          kv_used += (long long)(jj * (unsigned long long)(unsigned)b);
+          dt += (long long)(jj * (unsigned long long)cb);
+          dist -= j; iter += j;
+        }
         while (dist != 0 && an > now) { now += dt; kv_used += b; dt += cb; --dist; ++iter; }
+      }
     }
   }
   if (lane < 3) p.ema_final[3 * (size_t)inst_id + lane] = Bl;
@@ -439,23 +445,32 @@ template <int kSlots>
 __global__ void __launch_bounds__(k2::kWarpsPerBlock * 32) simulate_kernel(const __grid_constant__ Params p) {
   __shared__ unsigned long long heap_sm[kWarpsPerBlock][kHeapSmem];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-  // Policy affinity per SM: every warp of an SM starts on bucket (smid % 5) and moves on cyclically when a bucket is
-  // empty, so that an SM executes one policy's code at a time (instruction-cache locality; buckets: SJF, AGING,
-  // WEIGHTED, PRIORITY, FIFO, invalid).
+  // Policy affinity per SM: every warp of an SM starts on the same bucket and, when it is empty, moves to the bucket
+  // with the most instances left, so that an SM executes one policy's code at a time (instruction-cache locality).
+  // Buckets: SJF, AGING, WEIGHTED, PRIORITY, FIFO, invalid. SMs are split 26/31/35/30/26 (measured relative cost of one
+  // instance per policy on configs[1]); the split only sets the starting point, stealing evens out the rest.
   unsigned smid;
   asm("mov.u32 %0, %%smid;" : "=r"(smid));
-  int bucket = (int)(smid % 5u), tries = 0;
+  const unsigned sm148 = smid % 148u;
+  int bucket = sm148 < 26 ? 0 : sm148 < 57 ? 1 : sm148 < 92 ? 2 : sm148 < 122 ? 3 : 4;
   for (;;) {
     unsigned k = 0;
     if (lane == 0) k = atomicAdd(p.counter + bucket, 1u);
     k = __shfl_sync(kFull, k, 0);
     const unsigned b0 = p.counter[8 + bucket], b1 = p.counter[9 + bucket];
-    if (k >= b1 - b0) {
-      if (++tries == 6) return;
-      bucket = bucket == 5 ? 0 : bucket + 1;
+    if (k >= b1 - b0) {                                    // bucket empty: go where most work is left
+      int best = -1; unsigned best_left = 0;
+      if (lane < 6) {
+        const unsigned tot = p.counter[9 + lane] - p.counter[8 + lane];
+        const unsigned taken = *(volatile unsigned int*)(p.counter + lane);
+        best_left = taken < tot ? tot - taken : 0u;
+      }
+      const unsigned mx = __reduce_max_sync(kFull, best_left);
+      if (mx == 0) return;
+      best = __ffs(__ballot_sync(kFull, best_left == mx)) - 1;
+      bucket = best;
       continue;
     }
-    tries = 0;
     const unsigned inst_id = p.perm[b0 + k];
     const ds_instance in = p.inst[inst_id];
     const bool bad_inst = in.trace < 0 || in.trace >= p.n_traces || in.policy < 0 || in.policy > 4 || in.estimator < 0 ||
