@@ -24,9 +24,9 @@ sys.path.insert(0, ROOT)
 
 METRIC = "simulated requests/sec (policy x trace)"
 UNIT = "req/s"
-# executed warp-level instructions per simulated request of ds_simulate on configs[1], measured with ncu
-# (smsp__inst_executed.sum / 20.48e6; profiles/r01_ncu_simulate.md). Used for the issue-slot roofline only.
-K2_WARP_INST_PER_SIMREQ = None  # filled from profiles/k2_inst_per_simreq.txt when present
+# The issue-slot roofline of ds_simulate uses the executed warp instructions per simulated request measured with ncu
+# (paper_2606_02982_b200/k2_inst_per_simreq.txt, from profiles/r01_ncu_k2_v2.txt); DRAM traffic per launch comes from
+# the same captures (profiles/r01_traffic.json.txt).
 
 
 def _peaks():
@@ -251,13 +251,16 @@ def run_ours(args):
         "roofline_scan": {"kernel": "characterize_kernel", "bound": "hbm", "achieved": k1_gbs, "peak": hbm_peak, "unit": "GB/s",
                           "frac": k1_gbs / hbm_peak, "peak_source": which, "frac_of_8TBps": k1_gbs / 8000.0, "traffic": None},
     }
+    line["roofline_scan"]["traffic"] = _traffic().get("characterize_kernel")
+    if world == 1 and args.scan_gib > 0:
+        line["scan_configs2"] = scan_leg(dev, args.scan_gib, hbm_peak)
     # K2 roofline (dominant kernel): plain-ALU issue slots. peak = 148 SMs x 4 schedulers x 1 warp-inst/clk x max SM clock.
     ipr = _k2_inst_per_simreq()
     issue_peak = 148 * 4 * sm_max * 1e6 / 1e9
     if ipr is not None:
         ach = ipr * n_sim / (sim_ms * 1e-3) / 1e9
         line["roofline"] = {"kernel": "simulate_kernel<1>", "bound": "alu", "achieved": ach, "peak": issue_peak,
-                            "unit": "Gwarp-inst/s", "frac": ach / issue_peak, "traffic": None,
+                            "unit": "Gwarp-inst/s", "frac": ach / issue_peak, "traffic": _traffic().get("simulate_kernel"),
                             "note": "achieved = ncu-counted executed warp instructions per sim-request x sim-requests / live duration"}
     else:
         line["roofline"] = {"kernel": "simulate_kernel<1>", "bound": "alu", "achieved": None, "peak": issue_peak,
@@ -272,6 +275,42 @@ def run_ours(args):
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+
+
+def _traffic():
+    try:
+        return json.load(open(os.path.join(ROOT, "profiles", "r01_traffic.json.txt")))
+    except Exception:
+        return {}
+
+
+def scan_leg(dev, gib, hbm_peak):
+    """configs[2]: characterization-only scan of `gib` GiB of packed text (8 GiB = the full configuration)."""
+    import torch
+    import paper_2606_02982_b200 as ds
+    from paper_2606_02982_b200 import workload as wl
+    buf, off = wl.config2(int(gib * (1 << 30)))
+    t = torch.from_numpy(buf).to(dev)
+    o = torch.from_numpy(off).to(dev)
+    n = len(off) - 1
+    w = torch.empty(n, dtype=torch.int32, device=dev)
+    k = torch.empty_like(w)
+    for _ in range(3):
+        ds.characterize(t, o, w, k)
+    torch.cuda.synchronize()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    reps = 5
+    e0.record()
+    for _ in range(reps):
+        ds.characterize(t, o, w, k)                      # 8 GiB of input per call >> 126 MB L2
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    nbytes = buf.size + 16 * n
+    gbs = nbytes / (ms * 1e-3) / 1e9
+    return {"workload": "configs[2] scan, %.2f GiB packed text" % gib, "bytes": int(buf.size), "prompts": int(n), "ms": ms,
+            "achieved": gbs, "unit": "GB/s", "frac": gbs / hbm_peak, "frac_of_8TBps": gbs / 8000.0,
+            "algorithmic_bytes": int(nbytes)}
 
 
 def _k2_inst_per_simreq():
@@ -289,8 +328,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--traces", type=int, default=1024, help="traces per GPU (configs[1] = 1024)")
-    ap.add_argument("--cpu-traces", type=int, default=384, help="traces in the bounded oracle sample")
+    ap.add_argument("--cpu-traces", type=int, default=1024, help="traces in the bounded oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--scan-gib", type=float, default=8.0, help="size of the configs[2] scan leg in GiB (0 = skip)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
