@@ -142,6 +142,21 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+def max_over_ranks(ms, world, device):
+    """Timing rule of the bench contract: the job's time is the slowest rank's (all_reduce MAX); identity at N=1."""
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def rank_seed(rank):
+    """Weak scaling: rank r simulates its own 1024 traces, generated with seed 1+r (no data-path exchange)."""
+    return 1 + rank
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -158,7 +173,7 @@ def run_ours(args):
     from paper_2606_02982_b200.pipeline import HotPath
 
     # ---- setup (untimed): seeded inputs; W,P of the generated text come from ds_characterize itself ----
-    c = build_workload(args.traces, 1 + rank, gpu_characterize_fn(dev))   # weak scaling: every rank its own traces
+    c = build_workload(args.traces, rank_seed(rank), gpu_characterize_fn(dev))   # weak scaling: every rank its own traces
     hp = HotPath(c, dev)
     n_sim = c.sim_requests
     text_bytes = int(c.text.size)
@@ -190,10 +205,7 @@ def run_ours(args):
     sync_all()
     launches = ds.launch_count() - l0
     clocks = sampler.stop()
-    ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-    ms_total = float(ms.item())
+    ms_total = max_over_ranks(e0.elapsed_time(e1), world, dev)
     st_ms = np.array([[ev[i].elapsed_time(ev[i + 1]) for i in range(3)] for ev in stage_ev])   # characterize, simulate, stats
     char_ms, sim_ms, stat_ms = st_ms.mean(axis=0)
 
@@ -221,10 +233,7 @@ def run_ours(args):
         e2e_step()
     e1.record()
     sync_all()
-    ms2 = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(ms2, op=dist.ReduceOp.MAX)
-    e2e_val = world * n_sim * k2 / (float(ms2.item()) * 1e-3)
+    e2e_val = world * n_sim * k2 / (max_over_ranks(e0.elapsed_time(e1), world, dev) * 1e-3)
 
     if rank != 0:
         if world > 1:
