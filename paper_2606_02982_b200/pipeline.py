@@ -81,3 +81,63 @@ class HotPath:
         e = torch.cuda.Event(enable_timing=True)
         e.record()
         return e
+
+
+class HostPipeline:
+    """End-to-end path for HOST inputs and outputs: `depth` HotPath slots and three CUDA streams, so the host-to-device
+    copy of step i+1, the kernels of step i and the device-to-host copy of step i-1 overlap (PCIe is the slowest of the
+    three on configs[1]). Orchestration only: every computation still happens inside libdriftsched.so."""
+
+    IN_FIELDS = ("text", "offsets", "arrival", "tier", "out_len")
+
+    def __init__(self, wl_obj, device="cuda:0", depth=2):
+        self.dev = torch.device(device)
+        self.slots = [HotPath(wl_obj, device) for _ in range(depth)]
+        self.s_in, self.s_run, self.s_out = (torch.cuda.Stream(self.dev) for _ in range(3))
+        mk = lambda: [torch.cuda.Event() for _ in range(depth)]
+        self.ev_in, self.ev_run, self.ev_out = mk(), mk(), mk()
+        self.out_dev = [[hp.start, hp.done, hp.ema_final] + list(hp.stats.values()) for hp in self.slots]
+        self.out_host = [[torch.empty(t.shape, dtype=t.dtype).pin_memory() for t in outs] for outs in self.out_dev]
+        self.h2d_bytes = 0
+        self.d2h_bytes = sum(t.numel() * t.element_size() for t in self.out_host[0])
+
+    def pin_inputs(self, wl_obj):
+        """Pinned host copies of the per-step inputs (what a caller would hand over)."""
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        h = {f: pin(getattr(wl_obj, f)) for f in self.IN_FIELDS if getattr(wl_obj, f) is not None}
+        self.h2d_bytes = sum(t.numel() * t.element_size() for t in h.values())
+        return h
+
+    def run(self, host_inputs, n_steps):
+        """n_steps passes of the hot path, each with its inputs copied from `host_inputs` and its outputs copied to
+        pinned host memory. Returns the host output tensors of the last step. Synchronises at the end."""
+        cur = torch.cuda.current_stream(self.dev)
+        start = torch.cuda.Event()
+        start.record(cur)
+        for s in (self.s_in, self.s_run, self.s_out):
+            s.wait_event(start)
+        depth = len(self.slots)
+        for i in range(n_steps):
+            k = i % depth
+            hp = self.slots[k]
+            if i >= depth:
+                self.s_in.wait_event(self.ev_run[k])      # the kernels that last read this slot's inputs are done
+                self.s_run.wait_event(self.ev_out[k])     # and its outputs have left the device
+            with torch.cuda.stream(self.s_in):
+                for f, h in host_inputs.items():
+                    getattr(hp, f).copy_(h, non_blocking=True)
+                self.ev_in[k].record(self.s_in)
+            self.s_run.wait_event(self.ev_in[k])
+            with torch.cuda.stream(self.s_run):
+                hp.step()
+                self.ev_run[k].record(self.s_run)
+            self.s_out.wait_event(self.ev_run[k])
+            with torch.cuda.stream(self.s_out):
+                for h, d in zip(self.out_host[k], self.out_dev[k]):
+                    h.copy_(d, non_blocking=True)
+                self.ev_out[k].record(self.s_out)
+        for s in (self.s_in, self.s_run, self.s_out):
+            done = torch.cuda.Event()
+            done.record(s)
+            cur.wait_event(done)
+        return self.out_host[(n_steps - 1) % depth]
