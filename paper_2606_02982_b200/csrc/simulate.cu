@@ -24,6 +24,8 @@
 //    estimates of queued requests live in done_tick[] until the request completes;
 //  - SJF: warp-cooperative 32-ary min-heap of (est<<24 | index) keys, first 256 entries in shared memory, rest in the
 //    global workspace; sift-down compares 32 children per level with one shuffle min.
+#include <type_traits>
+
 #include "common.cuh"
 
 namespace ds {
@@ -107,7 +109,9 @@ struct TierCursor {
   long long arr;    // arrival tick of the head (AGING only)
 };
 
-template <int kSlots, int kPolicy>
+// kSmall: every per-iteration quantity of this trace (kv_used, dt, prefill) is proven < 2^31 and out_len <= 65535 by
+// trace_is_small(), so they are kept in 32-bit registers and the closed-form jump is two IMAD.WIDE; `now` stays 64-bit.
+template <int kSlots, int kPolicy, bool kSmall>
 __device__ __forceinline__ void run_instance(const Params& p, const unsigned inst_id, const int trace, const bool split, const double alpha,
                                           unsigned long long* heap_sm, const int lane) {
   constexpr bool kCursor = kPolicy == DS_PRIORITY || kPolicy == DS_WEIGHTED || kPolicy == DS_AGING;
@@ -136,7 +140,9 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   const int max_batch = p.max_batch;
 
   // ---- state (warp-uniform unless noted) ----
-  long long now = 0, kv_used = 0, prefill_new = 0, an = kInf;
+  using acc_t = typename std::conditional<kSmall, unsigned, unsigned long long>::type;
+  long long now = 0, an = kInf;
+  acc_t kv_used = 0, prefill_new = 0;
   int next = 0, b = 0, cur = 0, fifo_head = 0, done = 0;
   long long fifo_est = 0;
   unsigned iter = 0, dist = 0xffffffffu;
@@ -242,7 +248,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       for (int s = 0; s < kSlots; ++s) if (s_idx[s] == r) s_idx[s] = -1;
       const int Pr = P[r], Or = max(O[r], 1);
       dn[r] = now;                                            // every lane, same address and value: one store, no branch
-      kv_used -= (long long)Pr + Or;
+      kv_used -= (acc_t)Pr + (acc_t)Or;
       --b;
       if (ema_on) {                                           // Eq. 5-6 (A3): four separately rounded operations
         const int br = W[r], tr = min((int)tier[r], 2);
@@ -310,7 +316,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
         }
       }
       if (c < 0) break;
-      if (b > 0 && use_kv && kv_used + est_c > p.kv_budget) { blocked = kPolicy != DS_AGING; break; }   // deferred (A8)
+      if (b > 0 && use_kv && (long long)kv_used + est_c > p.kv_budget) { blocked = kPolicy != DS_AGING; break; }   // deferred (A8)
       // pop
       if (kPolicy == DS_FIFO) {
         ++fifo_head;
@@ -334,7 +340,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
 #pragma unroll
         for (int s = 0; s < kSlots; ++s) if (!placed && s_idx[s] < 0) { s_idx[s] = c; s_fin[s] = iter + (unsigned)Oc; placed = true; }
       }
-      kv_used += Pc; prefill_new += Pc; ++b;
+      kv_used += (acc_t)Pc; prefill_new += (acc_t)Pc; ++b;
       dist = min(dist, (unsigned)Oc);
     }
   };
@@ -353,22 +359,22 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       continue;
     }
     // 6. STEP: the iteration that carries the prefill of the newly admitted requests
-    long long dt = (long long)((unsigned long long)p.c_base + (unsigned long long)p.c_batch * (unsigned)b +
-                               (unsigned long long)kv_used * p.c_ctx);
-    const long long cb = (long long)((unsigned long long)p.c_ctx * (unsigned)b);
-    now += dt + (long long)((unsigned long long)prefill_new * p.c_prefill);
+    acc_t dt = (acc_t)p.c_base + (acc_t)p.c_batch * (unsigned)b + kv_used * p.c_ctx;
+    const acc_t cb = (acc_t)p.c_ctx * (unsigned)b;
+    now += (long long)(dt + prefill_new * p.c_prefill);
     prefill_new = 0;
-    kv_used += b; dt += cb; --dist; ++iter;
+    kv_used += (unsigned)b; dt += cb; --dist; ++iter;
     // boundaries at which nothing can happen: no completion, and no arrival that could be admitted
     if (dist != 0 && !(!blocked && b < max_batch && queue_nonempty())) {
       const bool arrivals_matter = b < max_batch && !(kPolicy == DS_FIFO && blocked) && next < n;
       // tick of the last boundary before the completion boundary: the stepping loop "while (an > now) step" runs all
       // `dist` iterations iff an > t_last
-      const unsigned long long dm1 = dist - 1;
-      const long long t_last = now + (long long)(dm1 * (unsigned long long)dt + (unsigned long long)cb * (dm1 * (dm1 - 1) / 2));
+      const unsigned dm1 = dist - 1;
+      const acc_t tri = (acc_t)dm1 * (acc_t)(dm1 - 1) / 2;               // kSmall: dist <= 65535, fits 32 bits
+      const long long t_last = now + (long long)((unsigned long long)dm1 * dt + (unsigned long long)cb * tri);
       if (!arrivals_matter || an > t_last) {                              // next event is the completion: exact jump
-        now = t_last + dt + (long long)(dm1 * (unsigned long long)cb);
-        kv_used += (long long)((unsigned long long)dist * (unsigned)b);
+        now = t_last + (long long)dt + (long long)((unsigned long long)dm1 * cb);
+        kv_used += (acc_t)dist * (unsigned)b;
         iter += dist; dist = 0;
       } else {
         // next event is an arrival. Lower bound on the stepping loop's trip count: every one of the first `cap`
@@ -383,18 +389,34 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
           if (j > dist) j = dist;
         }
         if (j) {                                                          // j iterations at once, exact
-          const unsigned long long jj = j;
-          now += (long long)(jj * (unsigned long long)dt + (unsigned long long)cb * (jj * (jj - 1) / 2));
-          kv_used += (long long)(jj * (unsigned long long)(unsigned)b);
-          dt += (long long)(jj * (unsigned long long)cb);
+          const acc_t trj = (acc_t)j * (acc_t)(j - 1) / 2;
+          now += (long long)((unsigned long long)j * dt + (unsigned long long)cb * trj);
+          kv_used += (acc_t)j * (unsigned)b;
+          dt += (acc_t)j * cb;
           dist -= j; iter += j;
         }
-        while (dist != 0 && an > now) { now += dt; kv_used += b; dt += cb; --dist; ++iter; }
+        while (dist != 0 && an > now) { now += (long long)dt; kv_used += (unsigned)b; dt += cb; --dist; ++iter; }
       }
     }
   }
   if (lane < 3) p.ema_final[3 * (size_t)inst_id + lane] = Bl;
   __syncwarp();
+}
+
+// true iff kv_used, the iteration cost (with prefill) and c_ctx*b of every reachable state of this trace stay below
+// 2^31 and every out_len is <= 65535: kv_used <= max_batch*(maxP+maxO) since a running request holds P+g <= P+O tokens.
+__device__ __forceinline__ bool trace_is_small(const Params& p, const int trace, const int lane) {
+  const long long lo = p.trace_off[trace], n = p.trace_off[trace + 1] - lo;
+  int mp = 0, mo = 0, mn = 0;
+  for (long long i = lane; i < n; i += 32) {
+    const int P = p.tokens[lo + i], O = p.out_len[lo + i];
+    mp = max(mp, P); mo = max(mo, O); mn = min(mn, P);
+  }
+  mp = __reduce_max_sync(kFull, mp); mo = __reduce_max_sync(kFull, mo); mn = __reduce_min_sync(kFull, mn);
+  const unsigned long long mb = (unsigned long long)p.max_batch;
+  const unsigned long long kvmax = mb * ((unsigned long long)mp + (unsigned long long)mo);
+  const unsigned long long dtmax = p.c_base + p.c_batch * mb + p.c_ctx * kvmax + p.c_prefill * mb * (unsigned long long)mp;
+  return mn >= 0 && mo <= 65535 && kvmax < (1ull << 31) && dtmax < (1ull << 31) && (unsigned long long)p.c_ctx * mb < (1ull << 31);
 }
 
 // Processing order: instances grouped by policy, most expensive policy first (SJF, AGING, WEIGHTED, PRIORITY, FIFO).
@@ -482,13 +504,18 @@ __global__ void __launch_bounds__(k2::kWarpsPerBlock * 32) simulate_kernel(const
     }
     const bool split = in.estimator == DS_SPLIT;
     if (lane < 3) p.ema_final[3 * (size_t)inst_id + lane] = 1.0;   // overwritten unless the trace is rejected
+    const bool small = trace_is_small(p, in.trace, lane);
+#define DS_RUN(POL)                                                                                             \
+  if (small) run_instance<kSlots, POL, true>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane);    \
+  else run_instance<kSlots, POL, false>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane)
     switch (in.policy) {
-      case DS_FIFO: run_instance<kSlots, DS_FIFO>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane); break;
-      case DS_PRIORITY: run_instance<kSlots, DS_PRIORITY>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane); break;
-      case DS_WEIGHTED: run_instance<kSlots, DS_WEIGHTED>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane); break;
-      case DS_SJF: run_instance<kSlots, DS_SJF>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane); break;
-      default: run_instance<kSlots, DS_AGING>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane); break;
+      case DS_FIFO: DS_RUN(DS_FIFO); break;
+      case DS_PRIORITY: DS_RUN(DS_PRIORITY); break;
+      case DS_WEIGHTED: DS_RUN(DS_WEIGHTED); break;
+      case DS_SJF: DS_RUN(DS_SJF); break;
+      default: DS_RUN(DS_AGING); break;
     }
+#undef DS_RUN
   }
 }
 

@@ -101,3 +101,17 @@ def test_bad_arguments(G):
     ds.simulate(d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"], c.server, d["inst"],
                 d["out_off"], int(c.out_off[-1]))
     assert ds.device_status() & 8
+
+
+def test_large_costs_take_the_64bit_path(G):
+    # cost constants near 2^31 and one huge out_len: the per-trace bound fails, so the kernel must use its 64-bit state
+    sv = wl.Server(max_batch=6, kv_budget=9000, aging_step=3_000_000_000, c_base=2_000_000_000, c_batch=150_000_000,
+                   c_ctx=1_000_003, c_prefill=5_000_000)
+    combos = [(p, e, 0.2) for p in wl.ALL_POLICIES for e in (wl.SPLIT, wl.EXACT)]
+    c = wl._trace_workload("t", 77, 2, 400, sv, combos, oracle.characterize, mean_ticks=3.0e10)
+    c.out_len[5] = 70_000                                                  # > 65535
+    _assert_same(G.gpu_simulate(c), _oracle(c), c)
+    import paper_2606_02982_b200 as ds
+    sv.c_base = 1 << 31                                                    # not representable: rejected on the host
+    with pytest.raises(ds.DsError):
+        G.gpu_simulate(c)
