@@ -6,7 +6,7 @@
  *   (a) ds_characterize : admission-time workload characterization of packed prompt text,
  *   (b) ds_simulate     : tick-exact simulation of tier queues x scheduling policy x continuous-batching
  *                         server model x per-tier EMA calibration, one instance per warp,
- *   (c) ds_latencies + ds_tail_stats : queue wait / end-to-end latency and their percentiles.
+ *   (c) ds_latencies + ds_tail_stats (or the fused ds_latency_stats) : queue wait / end-to-end latency and their percentiles.
  *
  * Conventions (all entry points)
  *  - extern "C"; plain pointers and sizes; no C++/torch types.
@@ -135,6 +135,20 @@ int ds_latencies(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, c
  * workspace: ds_workspace_bytes(DS_WS_TAIL_STATS, n_segments, n_pct). Launches: 1 memset + up to 9 x 2 kernels. */
 int ds_tail_stats(const int64_t* values, const int32_t* seg_id, int64_t n, int32_t n_segments, const int32_t* pct,
                   int32_t n_pct, int64_t* out, int64_t* count_out, void* workspace, size_t workspace_bytes, void* stream);
+
+/* Fused form of ds_latencies + 4 x ds_tail_stats for the report the paper's tables need (Tables VI-VIII: percentiles of
+ * end-to-end latency and queue wait per tenant tier and overall): nothing is materialised, every radix pass recomputes
+ * value = tick - arrival from start_tick / done_tick. With G = n_groups * (t_mid ? 2 : 1) and g as in ds_latencies:
+ *   e2e_out, qdelay_out [4*G*n_pct] int64 device (either may be NULL = not wanted): entries [(3*g+tier)*n_pct + q] are the
+ *     per-(group, tier) percentiles, entries [(3*G + g)*n_pct + q] the per-group ("overall") percentiles; -1 = empty.
+ *   count_out [4*G] nullable: segment sizes in the same order.
+ * Same nearest-rank definition and results as the unfused calls (bit-exact). pct: HOST array, n_pct <= 8.
+ * Requires 4*G*n_pct <= 200 histograms (shared memory); DS_EINVAL otherwise: use the unfused calls then.
+ * workspace: ds_workspace_bytes(DS_WS_TAIL_STATS, 4*G, n_pct). Launches per wanted metric: 2 memsets + 2 + up to 8 x 2 kernels. */
+int ds_latency_stats(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, const int64_t* out_off,
+                     const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, int32_t n_groups,
+                     const int64_t* t_mid, const int32_t* pct, int32_t n_pct, int64_t* e2e_out, int64_t* qdelay_out,
+                     int64_t* count_out, void* workspace, size_t workspace_bytes, void* stream);
 
 #define DS_WS_CHARACTERIZE 0
 #define DS_WS_SIMULATE 1

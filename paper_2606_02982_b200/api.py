@@ -139,3 +139,28 @@ def tail_stats(values, seg_id, n_segments, pct=(50, 99), out=None, count_out=Non
     check("ds_tail_stats", lib().ds_tail_stats(_ptr(values), _ptr(seg_id), values.numel(), n_segments, arr, n_pct, _ptr(out),
                                                _ptr(count_out), _ptr(workspace), workspace.numel(), _stream()))
     return out, count_out
+
+
+def latency_stats(trace_off, arrival, tier, words, tokens, out_len, inst, out_off, start, done, group, n_groups, t_mid=None,
+                  pct=(50, 99), e2e_out=None, qdelay_out=None, count_out=None, workspace=None):
+    """ds_latency_stats -> (e2e_out, qdelay_out, count_out), each laid out [4*G, n_pct] / [4*G] with G = n_groups * phases:
+    rows [0, 3G) are the (group, tier) segments 3*g+tier, rows [3G, 4G) the per-group overall segments."""
+    tr = _traces(trace_off, arrival, tier, words, tokens, out_len)
+    _need_cuda(inst, out_off, start, done, group, t_mid, e2e_out, qdelay_out, count_out)
+    n_inst = inst.numel() // INSTANCE_BYTES
+    dev = start.device
+    G = n_groups * (2 if t_mid is not None else 1)
+    n_pct = len(pct)
+    if e2e_out is None:
+        e2e_out = torch.empty((4 * G, n_pct), dtype=torch.int64, device=dev)
+    if qdelay_out is None:
+        qdelay_out = torch.empty((4 * G, n_pct), dtype=torch.int64, device=dev)
+    if count_out is None:
+        count_out = torch.empty(4 * G, dtype=torch.int64, device=dev)
+    if workspace is None:
+        workspace = _workspace(_lib.WS_TAIL_STATS, 4 * G, n_pct, dev)
+    arr = (C.c_int32 * n_pct)(*[int(x) for x in pct])
+    check("ds_latency_stats", lib().ds_latency_stats(C.byref(tr), _ptr(inst), n_inst, _ptr(out_off), _ptr(start), _ptr(done),
+                                                     _ptr(group), n_groups, _ptr(t_mid), arr, n_pct, _ptr(e2e_out), _ptr(qdelay_out),
+                                                     _ptr(count_out), _ptr(workspace), workspace.numel(), _stream()))
+    return e2e_out, qdelay_out, count_out

@@ -59,6 +59,7 @@ __global__ void latencies_kernel(const int64_t* __restrict__ trace_off, const in
 // Warp-aggregated shared-memory add: lanes of the warp that target the same bin are merged with MATCH.ANY so a hot
 // bin (latencies share their high digits) costs one atomic per warp instead of 32 serialised ones.
 __device__ __forceinline__ void agg_add(unsigned int* bins, bool pred, unsigned bin) {
+  if (!__any_sync(0xffffffffu, pred)) return;     // later digits: almost no key matches the prefix, skip the MATCH
   const unsigned m = __match_any_sync(0xffffffffu, pred ? bin : 0xffffffffu);
   if (pred && (threadIdx.x & 31) == (unsigned)(__ffs(m) - 1)) atomicAdd(&bins[bin], (unsigned)__popc(m));
 }
@@ -190,6 +191,79 @@ __global__ void select_kernel(int n_seg, int n_pct, int d, const Ws* hdr, const 
   }
 }
 
+// ---- fused latency statistics (ds_latency_stats): the percentiles of e2e / queue delay per (group, tier) and per
+// group straight from start/done ticks. Nothing is materialised: every radix pass recomputes value = tick - arrival
+// (8 B per request from HBM; arrival and tier are shared by the instances of a trace and stay in L2), and each value is
+// counted in two segments: 3*g+tier ("tier" block, 3*G segments) and 3*G+g ("all" block, G segments).
+struct LatArgs {
+  const int64_t* trace_off; const int64_t* arrival; const uint8_t* tier; const ds_instance* inst; const int64_t* out_off;
+  const int64_t* ticks; const int32_t* group; const int64_t* t_mid; long long n_inst; int n_groups;   // groups after phases
+};
+
+// kCount: segment counts + AND/OR of all keys. Otherwise: digit-d histogram of the keys matching each (segment, pct) prefix.
+template <bool kCount>
+__global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pct, int d, Ws* hdr, unsigned long long* counts,
+                                                       const unsigned long long* __restrict__ prefix, unsigned int* hist) {
+  extern __shared__ unsigned int sh[];
+  const int n_seg = 4 * a.n_groups;
+  const int nb = kCount ? n_seg : n_seg * n_pct * 256;
+  if (!kCount) {
+    const unsigned long long diff = hdr->and_bits ^ hdr->or_bits;
+    if (!hdr->any || ((diff >> (8 * d)) & 0xffull) == 0) return;   // every key has the same digit here: skipped
+  }
+  for (int i = threadIdx.x; i < nb; i += blockDim.x) sh[i] = 0;
+  __syncthreads();
+  unsigned long long kand = ~0ull, kor = 0ull; bool any = false;
+  const int shift = 8 * d;
+  // one WARP per instance: the dependent header loads (instance -> trace -> offsets) of 16 warps per block overlap
+  const int lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
+  for (long long ii = (long long)blockIdx.x * nwarp + (threadIdx.x >> 5); ii < a.n_inst; ii += (long long)gridDim.x * nwarp) {
+    const int t = a.inst[ii].trace;
+    const long long lo = a.trace_off[t], n = a.trace_off[t + 1] - lo, oo = a.out_off[ii];
+    const int g0 = a.group ? a.group[ii] : 0;
+    const bool ph = a.t_mid != nullptr;
+    const long long tm = ph ? a.t_mid[t] : 0;
+    const bool gok = g0 >= 0 && (ph ? 2 * g0 + 1 : g0) < a.n_groups;
+    for (long long base = 0; base < n; base += 32 * kUnroll) {   // warp-uniform trip count
+      long long av[kUnroll], tv[kUnroll]; int tr[kUnroll];
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u) {
+        const long long r = base + u * 32 + lane;
+        const bool in = r < n;
+        av[u] = in ? a.arrival[lo + r] : 0; tv[u] = in ? a.ticks[oo + r] : 0; tr[u] = in ? (int)a.tier[lo + r] : -1;
+      }
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u) {
+        const bool ok = gok && tr[u] >= 0 && tr[u] <= 2;
+        const unsigned long long k = (unsigned long long)(tv[u] - av[u]) ^ kSign;
+        const int g = !ok ? 0 : (ph ? g0 * 2 + (av[u] >= tm ? 1 : 0) : g0);
+        const unsigned s_t = (unsigned)(3 * g + (ok ? tr[u] : 0)), s_a = (unsigned)(3 * a.n_groups + g);
+        if (kCount) {
+          if (ok) { kand &= k; kor |= k; any = true; }
+          agg_add(sh, ok, s_t);
+          agg_add(sh, ok, s_a);
+        } else {
+          const unsigned long long hi = d == 7 ? 0ull : (k >> (shift + 8));
+          const unsigned dig = (unsigned)(k >> shift) & 0xffu;
+          for (int q = 0; q < n_pct; ++q) {
+            agg_add(sh, ok && hi == prefix[s_t * n_pct + q], (s_t * n_pct + q) * 256 + dig);
+            agg_add(sh, ok && hi == prefix[s_a * n_pct + q], (s_a * n_pct + q) * 256 + dig);
+          }
+        }
+      }
+    }
+  }
+  __syncthreads();
+  if (kCount) {
+    for (int dd = 16; dd > 0; dd >>= 1) { kand &= __shfl_xor_sync(0xffffffffu, kand, dd); kor |= __shfl_xor_sync(0xffffffffu, kor, dd); }
+    const unsigned anym = __ballot_sync(0xffffffffu, any);
+    if ((threadIdx.x & 31) == 0 && anym) { atomicAnd(&hdr->and_bits, kand); atomicOr(&hdr->or_bits, kor); atomicOr(&hdr->any, 1u); }
+    for (int i = threadIdx.x; i < nb; i += blockDim.x) if (sh[i]) atomicAdd(&counts[i], (unsigned long long)sh[i]);
+  } else {
+    for (int i = threadIdx.x; i < nb; i += blockDim.x) if (sh[i]) atomicAdd(&hist[i], sh[i]);
+  }
+}
+
 }  // namespace k3
 
 size_t ws_tail_stats(int64_t n_seg, int64_t n_pct) { return k3::make_layout(nullptr, n_seg, n_pct).total; }
@@ -249,6 +323,60 @@ extern "C" int ds_tail_stats(const int64_t* values, const int32_t* seg_id, int64
     else k3::hist_kernel<false><<<(unsigned)blocks, threads, 0, s>>>(values, seg_id, n, n_segments, n_pct, d, L.hdr, L.prefix, L.hist);
     k3::select_kernel<<<(nsq + 3) / 4, 128, 0, s>>>(n_segments, n_pct, d, L.hdr, L.counts, L.prefix, L.rank, L.hist, out);
     note_launch(2);
+  }
+  DS_CUDA(cudaGetLastError());
+  return DS_OK;
+}
+
+extern "C" int ds_latency_stats(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, const int64_t* out_off,
+                                const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, int32_t n_groups,
+                                const int64_t* t_mid, const int32_t* pct, int32_t n_pct, int64_t* e2e_out, int64_t* qdelay_out,
+                                int64_t* count_out, void* workspace, size_t workspace_bytes, void* stream) {
+  using namespace ds;
+  if (!tr || n_inst < 0 || n_groups < 1 || n_pct < 1 || n_pct > k3::kMaxPct || !pct || !workspace) return DS_EINVAL;
+  if (!e2e_out && !qdelay_out) return DS_EINVAL;
+  if (n_inst > 0 && (!inst || !out_off || !tr->trace_off || !tr->arrival_tick || !tr->tier)) return DS_EINVAL;
+  if ((e2e_out && !done_tick) || (qdelay_out && !start_tick)) { if (n_inst > 0) return DS_EINVAL; }
+  const int G = n_groups * (t_mid ? 2 : 1), n_seg = 4 * G, nsq = n_seg * n_pct;
+  const size_t hsm = sizeof(unsigned) * 256 * (size_t)nsq;
+  if (hsm > 200 * 1024) return DS_EINVAL;   // (groups x phases x 4 x percentiles) histograms must fit shared memory
+  k3::Pcts pc;
+  for (int q = 0; q < n_pct; ++q) { if (pct[q] < 0 || pct[q] > 100) return DS_EINVAL; pc.p[q] = pct[q]; }
+  k3::Layout L = k3::make_layout(workspace, n_seg, n_pct);
+  if (workspace_bytes < L.total) return DS_ENOMEM;
+  cudaStream_t s = (cudaStream_t)stream;
+  static bool attr_set = false;
+  if (!attr_set) {
+    DS_CUDA(cudaFuncSetAttribute(k3::lat_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+    attr_set = true;
+  }
+  long long per_sm = (long long)(200 * 1024) / (long long)(hsm + 1024);
+  if (per_sm > 3) per_sm = 3;
+  if (per_sm < 1) per_sm = 1;
+  long long blocks = (long long)kNumSMs * per_sm;
+  if (blocks > (n_inst + 15) / 16) blocks = (n_inst + 15) / 16;
+  if (blocks < 1) blocks = 1;
+  for (int metric = 0; metric < 2; ++metric) {
+    int64_t* out = metric == 0 ? e2e_out : qdelay_out;
+    if (!out) continue;
+    DS_CUDA(cudaMemsetAsync(workspace, 0, L.total, s));
+    DS_CUDA(cudaMemsetAsync(&L.hdr->and_bits, 0xff, 8, s));
+    if (n_inst == 0) {   // all segments empty
+      k3::init_kernel<<<(nsq + 255) / 256, 256, 0, s>>>(L.counts, n_seg, n_pct, pc, L.prefix, L.rank, count_out);
+      k3::select_kernel<<<(nsq + 3) / 4, 128, 0, s>>>(n_seg, n_pct, 0, L.hdr, L.counts, L.prefix, L.rank, L.hist, out);
+      note_launch(2);
+      continue;
+    }
+    k3::LatArgs a{tr->trace_off, tr->arrival_tick, tr->tier, inst, out_off, metric == 0 ? done_tick : start_tick, group, t_mid,
+                  (long long)n_inst, G};
+    k3::lat_pass_kernel<true><<<(unsigned)blocks, 512, sizeof(unsigned) * (size_t)n_seg, s>>>(a, n_pct, 0, L.hdr, L.counts, L.prefix, L.hist);
+    k3::init_kernel<<<(nsq + 255) / 256, 256, 0, s>>>(L.counts, n_seg, n_pct, pc, L.prefix, L.rank, count_out);
+    note_launch(2);
+    for (int d = 7; d >= 0; --d) {
+      k3::lat_pass_kernel<false><<<(unsigned)blocks, 512, hsm, s>>>(a, n_pct, d, L.hdr, L.counts, L.prefix, L.hist);
+      k3::select_kernel<<<(nsq + 3) / 4, 128, 0, s>>>(n_seg, n_pct, d, L.hdr, L.counts, L.prefix, L.rank, L.hist, out);
+      note_launch(2);
+    }
   }
   DS_CUDA(cudaGetLastError());
   return DS_OK;

@@ -1,5 +1,5 @@
 """One pass of the whole hot path over a resident workload:
-ds_characterize -> ds_simulate -> ds_latencies -> 4 x ds_tail_stats. Orchestration and buffer ownership only;
+ds_characterize -> ds_simulate -> ds_latency_stats (fused; or ds_latencies -> 4 x ds_tail_stats with fused=False). Orchestration and buffer ownership only;
 every computation happens inside libdriftsched.so."""
 from __future__ import annotations
 
@@ -12,11 +12,12 @@ from . import _lib, api
 class HotPath:
     """Device-resident buffers for one workload (see workload.Workload) and the step that runs the path."""
 
-    def __init__(self, wl_obj, device="cuda:0", pct=(50, 99)):
+    def __init__(self, wl_obj, device="cuda:0", pct=(50, 99), fused=True):
         c = wl_obj
         self.c = c
         self.dev = torch.device(device)
         self.pct = tuple(pct)
+        self.fused = fused
         up = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(self.dev)
         self.text = up(c.text) if c.text is not None else None
         self.offsets = up(c.offsets) if c.offsets is not None else None
@@ -46,15 +47,24 @@ class HotPath:
         ws = lambda which, a, b: torch.empty(api.workspace_bytes(which, a, b), dtype=torch.uint8, device=dev)
         self.ws_char = ws(_lib.WS_CHARACTERIZE, 0 if self.text is None else self.text.numel(), c.n_traces * c.n_req)
         self.ws_sim = ws(_lib.WS_SIMULATE, n, self.n_inst)
-        self.ws_tail = ws(_lib.WS_TAIL_STATS, 3 * self.n_groups, len(self.pct))
-        self.stats = {k: torch.empty((ns, len(self.pct)), dtype=torch.int64, device=dev)
-                      for k, ns in (("e2e_tier", 3 * self.n_groups), ("e2e_all", self.n_groups),
-                                    ("qdelay_tier", 3 * self.n_groups), ("qdelay_all", self.n_groups))}
-        self.counts = {k: torch.empty(v.shape[0], dtype=torch.int64, device=dev) for k, v in self.stats.items()}
-        self.e2e = torch.empty(n, dtype=torch.int64, device=dev)
-        self.qdelay = torch.empty(n, dtype=torch.int64, device=dev)
-        self.seg_tier = torch.empty(n, dtype=torch.int32, device=dev)
-        self.seg_all = torch.empty(n, dtype=torch.int32, device=dev)
+        G = self.n_groups
+        self.ws_tail = ws(_lib.WS_TAIL_STATS, 4 * G, len(self.pct))
+        # percentiles: rows [0,3G) = (group, tier) segments, rows [3G,4G) = per-group overall (ds_latency_stats layout)
+        self.e2e_stats = torch.empty((4 * G, len(self.pct)), dtype=torch.int64, device=dev)
+        self.qd_stats = torch.empty((4 * G, len(self.pct)), dtype=torch.int64, device=dev)
+        self.counts4 = torch.empty(4 * G, dtype=torch.int64, device=dev)
+        self.stats = {"e2e_tier": self.e2e_stats[:3 * G], "e2e_all": self.e2e_stats[3 * G:],
+                      "qdelay_tier": self.qd_stats[:3 * G], "qdelay_all": self.qd_stats[3 * G:]}
+        if fused:
+            self.counts = {"e2e_tier": self.counts4[:3 * G], "e2e_all": self.counts4[3 * G:],
+                           "qdelay_tier": self.counts4[:3 * G], "qdelay_all": self.counts4[3 * G:]}
+            self.e2e = self.qdelay = self.seg_tier = self.seg_all = None
+        else:
+            self.counts = {k: torch.empty(v.shape[0], dtype=torch.int64, device=dev) for k, v in self.stats.items()}
+            self.e2e = torch.empty(n, dtype=torch.int64, device=dev)
+            self.qdelay = torch.empty(n, dtype=torch.int64, device=dev)
+            self.seg_tier = torch.empty(n, dtype=torch.int32, device=dev)
+            self.seg_all = torch.empty(n, dtype=torch.int32, device=dev)
 
     def step(self, timed_events=False):
         """Run the path once on the current stream. With timed_events, returns CUDA events bracketing each stage."""
@@ -67,12 +77,17 @@ class HotPath:
         api.simulate(self.trace_off, self.arrival, self.tier, self.words, self.tokens, self.out_len, self.c.server, self.inst,
                      self.out_off, self.n_total, self.start, self.done, self.ema_final, self.traj_off, self.ema_traj, self.ws_sim)
         mark()
-        e2e, qd, seg_t, seg_a = api.latencies(self.trace_off, self.arrival, self.tier, self.words, self.tokens, self.out_len,
-                                              self.inst, self.out_off, self.n_total, self.start, self.done, self.group, self.t_mid,
-                                              out=(self.e2e, self.qdelay, self.seg_tier, self.seg_all))
-        for name, vals, seg in (("e2e_tier", e2e, seg_t), ("e2e_all", e2e, seg_a), ("qdelay_tier", qd, seg_t),
-                                ("qdelay_all", qd, seg_a)):
-            api.tail_stats(vals, seg, self.stats[name].shape[0], self.pct, self.stats[name], self.counts[name], self.ws_tail)
+        if self.fused:
+            api.latency_stats(self.trace_off, self.arrival, self.tier, self.words, self.tokens, self.out_len, self.inst,
+                              self.out_off, self.start, self.done, self.group, self.c.n_groups, self.t_mid, self.pct,
+                              self.e2e_stats, self.qd_stats, self.counts4, self.ws_tail)
+        else:
+            e2e, qd, seg_t, seg_a = api.latencies(self.trace_off, self.arrival, self.tier, self.words, self.tokens, self.out_len,
+                                                  self.inst, self.out_off, self.n_total, self.start, self.done, self.group,
+                                                  self.t_mid, out=(self.e2e, self.qdelay, self.seg_tier, self.seg_all))
+            for name, vals, seg in (("e2e_tier", e2e, seg_t), ("e2e_all", e2e, seg_a), ("qdelay_tier", qd, seg_t),
+                                    ("qdelay_all", qd, seg_a)):
+                api.tail_stats(vals, seg, self.stats[name].shape[0], self.pct, self.stats[name], self.counts[name], self.ws_tail)
         mark()
         return ev
 

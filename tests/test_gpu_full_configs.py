@@ -120,12 +120,16 @@ def test_cfg1_full_pipeline(G):
     st, dn = hp.start.cpu().numpy(), hp.done.cpu().numpy()
     e2e, qd, seg_t, seg_a = oracle.latencies(c.trace_off, c.arrival, c.tier, c.words, c.tokens, c.out_len, c.instances,
                                              c.out_off, st, dn, c.group)
-    assert np.array_equal(hp.e2e.cpu().numpy(), e2e) and np.array_equal(hp.seg_tier.cpu().numpy(), seg_t)
+    hp2 = HotPath(c, G.DEV, fused=False)                      # unfused ds_latencies + ds_tail_stats give the same numbers
+    hp2.step()
+    assert np.array_equal(hp2.e2e.cpu().numpy(), e2e) and np.array_equal(hp2.seg_tier.cpu().numpy(), seg_t)
+    assert np.array_equal(hp2.qdelay.cpu().numpy(), qd) and np.array_equal(hp2.seg_all.cpu().numpy(), seg_a)
     for name, vals, seg, ns in (("e2e_tier", e2e, seg_t, 30), ("e2e_all", e2e, seg_a, 10), ("qdelay_tier", qd, seg_t, 30),
                                 ("qdelay_all", qd, seg_a, 10)):
         o, cnt = oracle.tail_stats(vals, seg, ns)
-        assert np.array_equal(hp.stats[name].cpu().numpy(), o), name
-        assert np.array_equal(hp.counts[name].cpu().numpy(), cnt), name
+        for h in (hp, hp2):
+            assert np.array_equal(h.stats[name].cpu().numpy(), o), name
+            assert np.array_equal(h.counts[name].cpu().numpy(), cnt), name
 
 
 def test_cfg2_full_scan(G):

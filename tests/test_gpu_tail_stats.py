@@ -63,3 +63,39 @@ def test_pipeline_cfg1_small(G):
             g, gc = ds.tail_stats(vals, seg, ns)
             o, oc = oracle.tail_stats(ovals, oseg, ns)
             assert np.array_equal(g.cpu().numpy(), o) and np.array_equal(gc.cpu().numpy(), oc)
+
+
+def _fused_vs_oracle(G, c, pct=(50, 99)):
+    import paper_2606_02982_b200 as ds
+    from paper_2606_02982_b200 import workload as wl
+    st, dn, _ = oracle.simulate(c.trace_off, c.arrival, c.tier, c.words, c.tokens, c.out_len, c.server, c.instances)
+    e2e, qd, seg_t, seg_a = oracle.latencies(c.trace_off, c.arrival, c.tier, c.words, c.tokens, c.out_len, c.instances, c.out_off,
+                                             st, dn, c.group, c.t_mid)
+    Gn = c.n_groups * (2 if c.t_mid is not None else 1)
+    d = G.upload(c)
+    import torch
+    ge, gq, gc = ds.latency_stats(d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"], d["inst"],
+                                  d["out_off"], torch.from_numpy(st).to(G.DEV), torch.from_numpy(dn).to(G.DEV), d["group"],
+                                  c.n_groups, d["t_mid"], pct)
+    ge, gq, gc = ge.cpu().numpy(), gq.cpu().numpy(), gc.cpu().numpy()
+    for vals, got in ((e2e, ge), (qd, gq)):
+        ot, ct = oracle.tail_stats(vals, seg_t, 3 * Gn, pct)
+        oa, ca = oracle.tail_stats(vals, seg_a, Gn, pct)
+        assert np.array_equal(got[:3 * Gn], ot) and np.array_equal(got[3 * Gn:], oa)
+        assert np.array_equal(gc[:3 * Gn], ct) and np.array_equal(gc[3 * Gn:], ca)
+
+
+def test_fused_latency_stats(G):
+    from paper_2606_02982_b200 import workload as wl
+    sv = wl.Server(max_batch=8, kv_budget=3000)
+    combos = [(p, e, 0.1) for p in wl.ALL_POLICIES for e in (wl.SPLIT, wl.EXACT)]
+    c = wl._trace_workload("t", 5, 7, 1500, sv, combos, oracle.characterize, rho=1.1)          # ragged block tails
+    _fused_vs_oracle(G, c)
+    c2 = wl._trace_workload("t", 8, 3, 700, sv, combos[:3], oracle.characterize, rho=0.9)
+    _fused_vs_oracle(G, c2, pct=(0, 1, 50, 95, 99, 100))
+    c4 = wl.config4(oracle.characterize, n_traces=3, n_req=2500, materialise=True, traj_every=0)   # pre/post-drift phases
+    c4.server.max_batch = 32
+    _fused_vs_oracle(G, c4)
+    c1 = wl._trace_workload("t", 6, 1, 40, sv, [(wl.FIFO, wl.EXACT, 0.0)], oracle.characterize, rho=0.5)
+    c1.tier[:] = 1                                                                               # tiers 0 and 2 empty -> -1
+    _fused_vs_oracle(G, c1)
