@@ -189,11 +189,11 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
 #pragma unroll
     for (int t = 0; t < 3; ++t) { tc[t].blk = 0; tc[t].mask = 0; tc[t].est = 0; tc[t].arr = 0; advance_cursor(tc[t], t, true); }
 
-  // enqueue every request of the window that has arrived (strictly) by `now`; 32 at a time
-  auto ingest = [&](const bool strict) {
+  // enqueue every request of the window with arrival <= limit (now-1 for INGEST-EARLY, now for INGEST-NOW); 32 at a time
+  auto ingest = [&](const long long limit) {
     for (;;) {
       const int i = wb + lane;
-      const bool pred = i >= next && i < n && (strict ? w_arr < now : w_arr <= now);
+      const bool pred = i >= next && w_arr <= limit;            // lanes past the trace hold kInf
       const unsigned m = __ballot_sync(kFull, pred);
       if (m == 0) break;
       const int c = __popc(m);
@@ -349,7 +349,8 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   for (;;) {
 #pragma unroll 1
     for (int ph = 0; ph < 2; ++ph) {                                      // one copy of the ingest code for both phases
-      if (ph == 0 ? an < now : an <= now) ingest(ph == 0);                // 1. INGEST-EARLY / 3. INGEST-NOW
+      const long long limit = now - 1 + ph;                               // ticks are integers: "< now" is "<= now-1"
+      if (an <= limit) ingest(limit);                                     // 1. INGEST-EARLY / 3. INGEST-NOW
       if (ph == 0 && dist == 0) retire();                                 // 2. RETIRE
     }
     if (!blocked && b < max_batch) admit();                               // 4. ADMIT
