@@ -353,7 +353,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       if (an <= limit) ingest(limit);                                     // 1. INGEST-EARLY / 3. INGEST-NOW
       if (ph == 0 && dist == 0) retire();                                 // 2. RETIRE
     }
-    if (!blocked && b < max_batch) admit();                               // 4. ADMIT
+    if (!blocked && b < max_batch && queue_nonempty()) admit();           // 4. ADMIT
     if (b == 0) {                                                         // 5. IDLE / END
       if (next >= n) break;
       now = an;
