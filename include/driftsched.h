@@ -42,7 +42,7 @@ extern "C" {
 #define DS_DEV_BAD_OFFSETS 1u  /* ds_characterize: offsets not in [0,n_bytes] or decreasing */
 #define DS_DEV_BAD_TRACE 2u    /* ds_simulate: tier > 2, out_len < 1, words/tokens < 0 or arrivals decreasing */
 #define DS_DEV_KEY_RANGE 4u    /* ds_simulate: SJF key overflow (est >= 2^39 or trace longer than 2^24) */
-#define DS_DEV_BAD_INSTANCE 8u /* ds_simulate: instance field out of range */
+#define DS_DEV_BAD_INSTANCE 8u /* ds_simulate: instance field out of range; ds_estimation_error: group out of range */
 
 /* ---------------------------------------------------------------------------------------------- (a)
  * Workload characterization ("whitespace-delimited word counts" vs
@@ -115,6 +115,26 @@ typedef struct {
 int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
                 const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
                 const int64_t* traj_off, double* ema_traj, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ds_simulate that also returns the frozen admission-time estimate of every simulated request (reading A5):
+ * est_out [out_off[n_inst]] int64 device, same indexing as start_tick. Everything else as ds_simulate. */
+int ds_simulate_est(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
+                    const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
+                    const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace, size_t workspace_bytes,
+                    void* stream);
+
+/* Estimation fidelity: job classes of Eq. 3-4 (short est<=128, medium
+ * est<=512, long otherwise), token-estimation error (Tables IV, X) and queue wait by job class
+ * (Table IX), per reporting group g = group[instance] (nullable -> 0) in [0, n_groups).
+ * out [n_groups*11] int64 device, exact integer sums over the group's simulated requests:
+ *   { n, sum|est-P|, sum(est-P)^2, sum est, sum P, n_short, n_medium, n_long, sum qdelay_short, _medium, _long }
+ *   with P = tokens (the observed length, reading A3) and qdelay = start_tick - arrival (0 if start_tick is NULL).
+ *   MAE = out[1]/out[0], RMSE = sqrt(out[2]/out[0]), mean bias = out[4]/out[3] are left to the caller (fp64).
+ * class_seg (nullable) [out_off[n_inst]] int32 device: 3*g + class, usable as seg_id for ds_tail_stats.
+ * A group outside [0, n_groups) sets DS_DEV_BAD_INSTANCE. Launches: 1 memset + 1 kernel. */
+int ds_estimation_error(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, const int64_t* out_off,
+                        const int64_t* est, const int64_t* start_tick, const int32_t* group, int32_t n_groups,
+                        int64_t* out, int32_t* class_seg, void* stream);
 
 /* ---------------------------------------------------------------------------------------------- (c)
  * Latency derivation (worker timestamps separate queueing from inference):

@@ -47,7 +47,9 @@ def _o():
         lib = C.CDLL(build())
         p = C.c_void_p
         lib.oracle_characterize.argtypes = [p, C.c_int64, p, C.c_int64, p, p]
-        lib.oracle_simulate.argtypes = [p, p, p, C.c_int64, p, p, p, p, p, p]
+        lib.oracle_simulate.argtypes = [p, p, p, C.c_int64, p, p, p, p, p, p, p]
+        lib.oracle_estimation_error.argtypes = [p, p, C.c_int64, p, p, p, p, C.c_int32, p, p]
+        lib.oracle_estimation_error.restype = C.c_int
         lib.oracle_latencies.argtypes = [p, p, C.c_int64, p, p, p, p, p, p, p, p, p]
         lib.oracle_tail_stats.argtypes = [p, p, C.c_int64, C.c_int32, p, C.c_int32, p, p]
         for f in (lib.oracle_characterize, lib.oracle_simulate, lib.oracle_latencies, lib.oracle_tail_stats):
@@ -95,8 +97,9 @@ def traj_offsets(trace_off, instances, traj_every):
     return np.concatenate([[0], np.cumsum(k)]).astype(np.int64)
 
 
-def simulate(trace_off, arrival, tier, words, tokens, out_len, server, instances, out_off=None, want_traj=False):
-    """Returns start_tick, done_tick, ema_final[n_inst,3] (and ema_traj[samples,3] if want_traj)."""
+def simulate(trace_off, arrival, tier, words, tokens, out_len, server, instances, out_off=None, want_traj=False,
+             want_est=False):
+    """Returns start_tick, done_tick, ema_final[n_inst,3] (then ema_traj[samples,3] if want_traj, then est if want_est)."""
     tr, keep = _traces(trace_off, arrival, tier, words, tokens, out_len)
     sv = _server(server)
     inst = _c(instances, INSTANCE_DTYPE)
@@ -113,11 +116,13 @@ def simulate(trace_off, arrival, tier, words, tokens, out_len, server, instances
     if want_traj and server.traj_every > 0:
         toff = traj_offsets(keep[0], inst, server.traj_every)
         traj = np.zeros((int(toff[-1]), 3), np.float64)
+    est = np.full(total, -1, np.int64) if want_est else None
     rc = _o().oracle_simulate(C.byref(tr), C.byref(sv), _p(inst), n_inst, _p(out_off), _p(start), _p(done), _p(ema),
-                              _p(toff), _p(traj))
+                              _p(toff), _p(traj), _p(est))
     if rc:
         raise ValueError("oracle_simulate: contract violation")
-    return (start, done, ema, traj) if want_traj else (start, done, ema)
+    out = (start, done, ema) + ((traj,) if want_traj else ()) + ((est,) if want_est else ())
+    return out
 
 
 def latencies(trace_off, arrival, tier, words, tokens, out_len, instances, out_off, start, done, group=None, t_mid=None):
@@ -148,3 +153,25 @@ def tail_stats(values, seg_id, n_segments, pct=(50, 99)):
     rc = _o().oracle_tail_stats(_p(values), _p(seg_id), values.size, n_segments, _p(pct), len(pct), _p(out), _p(cnt))
     assert rc == 0
     return out, cnt
+
+
+ERR_FIELDS = ("n", "sum_abs_err", "sum_sq_err", "sum_est", "sum_tokens", "n_short", "n_medium", "n_long",
+              "sum_qdelay_short", "sum_qdelay_medium", "sum_qdelay_long")
+
+
+def estimation_error(trace_off, arrival, tier, words, tokens, out_len, instances, out_off, est, start, group, n_groups,
+                     want_class_seg=False):
+    """-> sums int64[n_groups, 11] (ERR_FIELDS) and, if asked, class_seg int32 per simulated request."""
+    tr, keep = _traces(trace_off, arrival, tier, words, tokens, out_len)
+    inst = _c(instances, INSTANCE_DTYPE)
+    out_off = _c(out_off, np.int64)
+    est = _c(est, np.int64)
+    start = None if start is None else _c(start, np.int64)
+    g = None if group is None else _c(group, np.int32)
+    out = np.zeros((n_groups, 11), np.int64)
+    seg = np.zeros(est.size, np.int32) if want_class_seg else None
+    rc = _o().oracle_estimation_error(C.byref(tr), _p(inst), len(inst), _p(out_off), _p(est), _p(start), _p(g), n_groups,
+                                      _p(out), _p(seg))
+    if rc:
+        raise ValueError("oracle_estimation_error: contract violation")
+    return (out, seg) if want_class_seg else out

@@ -126,7 +126,7 @@ struct Sim {
 
 extern "C" int oracle_simulate(const oracle_traces* tr, const oracle_server* sv, const oracle_instance* inst,
                                int64_t n_inst, const int64_t* out_off, int64_t* start_tick, int64_t* done_tick,
-                               double* ema_final, const int64_t* traj_off, double* ema_traj) {
+                               double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out) {
   if (sv->max_batch < 1) return -1;
   if (sv->weight[0] < 1 || sv->weight[1] < 1 || sv->weight[2] < 1) return -1;
   if (sv->aging_step < 1) return -1;
@@ -198,6 +198,7 @@ extern "C" int oracle_simulate(const oracle_traces* tr, const oracle_server* sv,
       s.now += dt;
     }
     ema_final[ii * 3 + 0] = s.B[0]; ema_final[ii * 3 + 1] = s.B[1]; ema_final[ii * 3 + 2] = s.B[2];
+    if (est_out) for (int64_t r = 0; r < n; ++r) est_out[out_off[ii] + r] = s.est[r];   // frozen at arrival (A5)
   }
   return 0;
 }
@@ -237,6 +238,28 @@ extern "C" int oracle_tail_stats(const int64_t* values, const int32_t* seg_id, i
       if (rank < 1) rank = 1;
       if (rank > (int64_t)v.size()) rank = (int64_t)v.size();
       out[s * n_pct + q] = v[rank - 1];
+    }
+  }
+  return 0;
+}
+
+extern "C" int oracle_estimation_error(const oracle_traces* tr, const oracle_instance* inst, int64_t n_inst,
+                                       const int64_t* out_off, const int64_t* est, const int64_t* start_tick,
+                                       const int32_t* group, int32_t n_groups, int64_t* out, int32_t* class_seg) {
+  for (int64_t k = 0; k < (int64_t)n_groups * 11; ++k) out[k] = 0;
+  for (int64_t ii = 0; ii < n_inst; ++ii) {
+    int64_t t = inst[ii].trace, lo = tr->trace_off[t], n = tr->trace_off[t + 1] - lo;
+    int32_t g = group ? group[ii] : 0;
+    if (g < 0 || g >= n_groups) return -1;
+    int64_t* o = out + (int64_t)g * 11;
+    for (int64_t r = 0; r < n; ++r) {
+      int64_t e = est[out_off[ii] + r], P = tr->tokens[lo + r];
+      int64_t err = e - P;                                  // estimate minus observed length (A3: T_actual = tokens)
+      int cls = e <= 128 ? 0 : (e <= 512 ? 1 : 2);          // Eq. 4
+      o[0] += 1; o[1] += err < 0 ? -err : err; o[2] += err * err; o[3] += e; o[4] += P;
+      o[5 + cls] += 1;
+      if (start_tick) o[8 + cls] += start_tick[out_off[ii] + r] - tr->arrival_tick[lo + r];   // queue wait
+      if (class_seg) class_seg[out_off[ii] + r] = 3 * g + cls;
     }
   }
   return 0;

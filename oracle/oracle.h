@@ -46,7 +46,16 @@ int oracle_characterize(const uint8_t* bytes, int64_t n_bytes, const int64_t* of
 int oracle_simulate(const oracle_traces* tr, const oracle_server* sv, const oracle_instance* inst, int64_t n_inst,
                     const int64_t* out_off, int64_t* start_tick, int64_t* done_tick,
                     double* ema_final /*[n_inst*3]*/,
-                    const int64_t* traj_off /*nullable; [n_inst+1] sample ranges*/, double* ema_traj /*nullable; [samples][3]*/);
+                    const int64_t* traj_off /*nullable; [n_inst+1] sample ranges*/, double* ema_traj /*nullable; [samples][3]*/,
+                    int64_t* est_out /*nullable; frozen admission-time estimate per simulated request*/);
+
+/* Estimation fidelity (Eq. 3-4 job classes; Tables IV, IX, X): per reporting group, exact integer sums
+ * over its simulated requests: out[g*11 + ..] = { n, sum|est-P|, sum(est-P)^2, sum est, sum P, n_short, n_medium, n_long,
+ * sum qdelay_short, sum qdelay_medium, sum qdelay_long } with class short: est<=128, medium: est<=512, long: else.
+ * start_tick nullable (qdelay sums 0). class_seg nullable: 3*group+class per simulated request. */
+int oracle_estimation_error(const oracle_traces* tr, const oracle_instance* inst, int64_t n_inst, const int64_t* out_off,
+                            const int64_t* est, const int64_t* start_tick, const int32_t* group, int32_t n_groups,
+                            int64_t* out, int32_t* class_seg);
 
 /* PAPER.md:270 (queue wait vs end-to-end latency). seg outputs nullable. */
 int oracle_latencies(const oracle_traces* tr, const oracle_instance* inst, int64_t n_inst, const int64_t* out_off,

@@ -81,7 +81,7 @@ def instances_to_device(instances: np.ndarray, device):
 
 
 def simulate(trace_off, arrival, tier, words, tokens, out_len, server, inst, out_off, n_total, start=None, done=None,
-             ema_final=None, traj_off=None, ema_traj=None, workspace=None):
+             ema_final=None, traj_off=None, ema_traj=None, workspace=None, est_out=None):
     """ds_simulate. inst: uint8 CUDA tensor holding ds_instance[n_inst]; out_off int64[n_inst+1] (CUDA);
     n_total = out_off[-1] (host int). Returns (start_tick, done_tick, ema_final[n_inst,3])."""
     tr = _traces(trace_off, arrival, tier, words, tokens, out_len)
@@ -97,10 +97,44 @@ def simulate(trace_off, arrival, tier, words, tokens, out_len, server, inst, out
         ema_final = torch.empty((n_inst, 3), dtype=torch.float64, device=dev)
     if workspace is None:
         workspace = _workspace(_lib.WS_SIMULATE, n_total, n_inst, dev)
+    if est_out is not None:                     # ds_simulate_est: same call, also writes the frozen estimates
+        _need_cuda(est_out)
+        assert est_out.dtype == torch.int64 and est_out.numel() >= n_total
+        check("ds_simulate_est", lib().ds_simulate_est(C.byref(tr), C.byref(sv), _ptr(inst), n_inst, _ptr(out_off), _ptr(start),
+                                                       _ptr(done), _ptr(ema_final), _ptr(traj_off), _ptr(ema_traj), _ptr(est_out),
+                                                       _ptr(workspace), workspace.numel(), _stream()))
+        return start, done, ema_final
     check("ds_simulate", lib().ds_simulate(C.byref(tr), C.byref(sv), _ptr(inst), n_inst, _ptr(out_off), _ptr(start), _ptr(done),
                                            _ptr(ema_final), _ptr(traj_off), _ptr(ema_traj), _ptr(workspace), workspace.numel(),
                                            _stream()))
     return start, done, ema_final
+
+
+def simulate_est(trace_off, arrival, tier, words, tokens, out_len, server, inst, out_off, n_total, **kw):
+    """ds_simulate_est -> (start_tick, done_tick, ema_final, est int64[n_total])."""
+    est = kw.pop("est_out", None)
+    if est is None:
+        est = torch.empty(n_total, dtype=torch.int64, device=arrival.device)
+    s, d, e = simulate(trace_off, arrival, tier, words, tokens, out_len, server, inst, out_off, n_total, est_out=est, **kw)
+    return s, d, e, est
+
+
+ERR_FIELDS = 11
+
+
+def estimation_error(trace_off, arrival, tier, words, tokens, out_len, inst, out_off, n_total, est, start=None, group=None,
+                     n_groups=1, want_class_seg=False, out=None):
+    """ds_estimation_error -> sums int64[n_groups, 11] (and class_seg int32[n_total] if asked)."""
+    tr = _traces(trace_off, arrival, tier, words, tokens, out_len)
+    _need_cuda(inst, out_off, est, start, group, out)
+    n_inst = inst.numel() // INSTANCE_BYTES
+    dev = est.device
+    if out is None:
+        out = torch.empty((n_groups, ERR_FIELDS), dtype=torch.int64, device=dev)
+    seg = torch.empty(n_total, dtype=torch.int32, device=dev) if want_class_seg else None
+    check("ds_estimation_error", lib().ds_estimation_error(C.byref(tr), _ptr(inst), n_inst, _ptr(out_off), _ptr(est), _ptr(start),
+                                                           _ptr(group), n_groups, _ptr(out), _ptr(seg), _stream()))
+    return (out, seg) if want_class_seg else out
 
 
 def latencies(trace_off, arrival, tier, words, tokens, out_len, inst, out_off, n_total, start, done, group=None, t_mid=None,

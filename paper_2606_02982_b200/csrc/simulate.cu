@@ -42,7 +42,7 @@ struct Params {
   int32_t max_batch; int64_t kv_budget; uint32_t c_base, c_batch, c_ctx, c_prefill; /* < 2^31, checked by ds_simulate */ int32_t w0, w1, w2; int64_t aging_step;
   int32_t traj_every;
   const ds_instance* inst; int64_t n_inst; const int64_t* out_off; int64_t* start_tick; int64_t* done_tick;
-  double* ema_final; const int64_t* traj_off; double* ema_traj;
+  double* ema_final; const int64_t* traj_off; double* ema_traj; int64_t* est_out;
   unsigned long long* heap_ws; unsigned int* counter; unsigned int* status; const unsigned int* perm;
 };
 
@@ -132,7 +132,8 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   int64_t* dn = p.done_tick + oo;
   const int32_t* __restrict__ BASE = split ? W : P;
   const bool use_kv = p.kv_budget > 0;
-  const bool need_est = use_kv || kPolicy == DS_SJF;
+  int64_t* est_o = p.est_out ? p.est_out + oo : nullptr;
+  const bool need_est = use_kv || kPolicy == DS_SJF || est_o != nullptr;
   // EXACT estimator: m = P/P = 1.0, and (1-a)*1 + a*1 rounds to exactly 1.0 for every a in [0,1] (DESIGN.md §4 A4),
   // so B stays 1.0 and est = base: no fp64 work at all on that path.
   const bool ema_on = split && alpha > 0.0;
@@ -204,6 +205,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
           if (w_base > 0) est = (long long)ceil(__dmul_rn(Bt, (double)w_base));
         } else est = w_base;                                  // B == 1.0 exactly
       }
+      if (est_o && pred) est_o[i] = est;                      // frozen admission-time estimate (ds_simulate_est)
       if (kPolicy == DS_SJF) {
         if (pred && est >= (1ll << 39)) atomicOr(p.status, DS_DEV_KEY_RANGE);
         unsigned mm = m;
@@ -528,9 +530,10 @@ size_t ws_simulate(int64_t total_requests, int64_t n_inst) {
 }
 
 }  // namespace ds
-extern "C" int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
-                           const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
-                           const int64_t* traj_off, double* ema_traj, void* workspace, size_t workspace_bytes, void* stream) {
+static int simulate_impl(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
+                         const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
+                         const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace, size_t workspace_bytes,
+                         void* stream) {
   using namespace ds;
   if (!tr || !sv || n_inst < 0) return DS_EINVAL;
   if (n_inst == 0) return DS_OK;
@@ -550,7 +553,7 @@ extern "C" int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_in
   p.c_prefill = (uint32_t)sv->c_prefill; p.w0 = sv->weight[0]; p.w1 = sv->weight[1]; p.w2 = sv->weight[2]; p.aging_step = sv->aging_step;
   p.traj_every = sv->traj_every;
   p.inst = inst; p.n_inst = n_inst; p.out_off = out_off; p.start_tick = start_tick; p.done_tick = done_tick;
-  p.ema_final = ema_final; p.traj_off = traj_off; p.ema_traj = ema_traj;
+  p.ema_final = ema_final; p.traj_off = traj_off; p.ema_traj = ema_traj; p.est_out = est_out;
   p.counter = (unsigned int*)workspace;
   unsigned int* perm = (unsigned int*)((char*)workspace + 256);
   p.perm = perm;
@@ -579,4 +582,20 @@ extern "C" int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_in
   if (sv->max_batch <= 64) return launch(k2::simulate_kernel<2>);
   if (sv->max_batch <= 128) return launch(k2::simulate_kernel<4>);
   return launch(k2::simulate_kernel<8>);
+}
+
+extern "C" int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
+                           const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
+                           const int64_t* traj_off, double* ema_traj, void* workspace, size_t workspace_bytes, void* stream) {
+  return simulate_impl(tr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, nullptr, workspace,
+                       workspace_bytes, stream);
+}
+
+extern "C" int ds_simulate_est(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
+                               const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
+                               const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace,
+                               size_t workspace_bytes, void* stream) {
+  if (n_inst > 0 && !est_out) return DS_EINVAL;
+  return simulate_impl(tr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out, workspace,
+                       workspace_bytes, stream);
 }

@@ -1,0 +1,94 @@
+"""Pins for oracle.estimation_error and the frozen estimates oracle.simulate returns.
+
+What fixes the expected values, independently of the oracle:
+  * Eq. 4: short <= 128 < medium <= 512 < long, checked on the boundary values themselves;
+  * with alpha = 0 the factor stays 1.0 (I7), so est = words (SPLIT) or tokens (EXACT): the sums are numpy one-liners;
+  * hand trace H2/H3: r1 and r2 arrive before r0 completes, their estimates are frozen at 8 and 2 (A5);
+  * the paper's qualitative result (Tables IV, X): EMA feedback lowers MAE and RMSE of the
+    split() estimate, brings the mean bias to ~1, and changes nothing for the tokenizer-aware estimate.
+"""
+import numpy as np
+
+import oracle
+from paper_2606_02982_b200 import workload as wl
+from _simutil import server
+
+
+def _run(req, sv, combos, group=None, n_groups=1):
+    req = np.asarray(req, np.int64).reshape(-1, 5)
+    inst = np.zeros(len(combos), wl.INSTANCE_DTYPE)
+    for i, (p, e, a) in enumerate(combos):
+        inst[i] = (0, p, e, 0, a)
+    n = len(req)
+    out_off = np.arange(len(combos) + 1, dtype=np.int64) * n
+    tr = ([0, n], req[:, 0], req[:, 1], req[:, 2], req[:, 3], req[:, 4])
+    st, dn, ema, est = oracle.simulate(*tr, sv, inst, out_off=out_off, want_est=True)
+    sums, seg = oracle.estimation_error(*tr, inst, out_off, est, st, group, n_groups, want_class_seg=True)
+    return req, st, est, sums, seg
+
+
+def test_class_thresholds_eq4():
+    # EXACT, alpha=0: est = tokens. tokens chosen on both sides of each threshold of Eq. 4.
+    P = [1, 128, 129, 512, 513, 4000, 0]
+    req = [[i * 10, 1, 5, p, 1] for i, p in enumerate(P)]
+    req, st, est, sums, seg = _run(req, server(), [(wl.FIFO, wl.EXACT, 0.0)])
+    assert est.tolist() == P
+    assert seg.tolist() == [0, 0, 1, 1, 2, 2, 0]
+    s = dict(zip(oracle.ERR_FIELDS, sums[0].tolist()))
+    assert s["n"] == 7 and s["sum_abs_err"] == 0 and s["sum_sq_err"] == 0
+    assert s["sum_est"] == sum(P) and s["sum_tokens"] == sum(P)
+    assert (s["n_short"], s["n_medium"], s["n_long"]) == (3, 2, 2)
+    qd = st - req[:, 0]
+    cls = np.array([0, 0, 1, 1, 2, 2, 0])
+    assert [s["sum_qdelay_short"], s["sum_qdelay_medium"], s["sum_qdelay_long"]] == [int(qd[cls == k].sum()) for k in range(3)]
+
+
+def test_alpha0_split_sums_are_numpy_one_liners():
+    rng = np.random.default_rng(5)
+    n = 400
+    W = rng.integers(0, 700, n)
+    P = rng.integers(0, 900, n)
+    req = np.stack([np.cumsum(rng.integers(0, 3000, n)), rng.integers(0, 3, n), W, P, rng.integers(1, 6, n)], 1)
+    req, st, est, sums, seg = _run(req, server(max_batch=4), [(wl.SJF, wl.SPLIT, 0.0), (wl.PRIORITY, wl.EXACT, 0.3)],
+                                   group=np.array([1, 0], np.int32), n_groups=2)
+    assert np.array_equal(est[:n], W) and np.array_equal(est[n:], P)      # I7 / A4
+    e = W - P
+    assert sums[1].tolist()[:5] == [n, int(np.abs(e).sum()), int((e * e).sum()), int(W.sum()), int(P.sum())]
+    assert sums[0].tolist()[:5] == [n, 0, 0, int(P.sum()), int(P.sum())]
+    cls_w = np.where(W <= 128, 0, np.where(W <= 512, 1, 2))
+    assert np.array_equal(seg[:n], 3 * 1 + cls_w)
+    cls_p = np.where(P <= 128, 0, np.where(P <= 512, 1, 2))
+    assert np.array_equal(seg[n:], cls_p)
+    qd = st[:n] - req[:, 0]
+    assert sums[1].tolist()[8:] == [int(qd[cls_w == k].sum()) for k in range(3)]
+    assert sums[1].tolist()[5:8] == [int((cls_w == k).sum()) for k in range(3)]
+
+
+def test_h3_estimates_frozen_at_arrival():
+    # H2/H3: r1, r2 arrive (ticks 1000, 1500) before r0 completes (4329): est uses B = 1.0 -> 8 and 2; a 4th request
+    # arriving after the completion of r0 (Standard) sees B[Std] = 1.0333.. -> ceil(1.0333*3) = 4, Premium still 1.0.
+    req = [[0, 1, 3, 4, 2], [1000, 0, 8, 10, 1], [1500, 2, 2, 3, 2], [5000, 1, 3, 4, 1], [5001, 0, 3, 4, 1]]
+    req, st, est, sums, seg = _run(req, server(), [(wl.SJF, wl.SPLIT, 0.1)])
+    assert est.tolist() == [3, 8, 2, 4, 3]
+
+
+def test_group_out_of_range_is_rejected():
+    import pytest
+    with pytest.raises(ValueError):
+        _run([[0, 0, 1, 1, 1]], server(), [(wl.FIFO, wl.EXACT, 0.0)], group=np.array([2], np.int32), n_groups=2)
+
+
+def test_feedback_lowers_estimation_error_like_tables_iv_x():
+    combos = [(wl.FIFO, wl.SPLIT, 0.0), (wl.FIFO, wl.SPLIT, 0.1), (wl.FIFO, wl.EXACT, 0.0), (wl.FIFO, wl.EXACT, 0.1)]
+    sv = wl.Server(max_batch=32, kv_budget=16384)
+    c = wl._trace_workload("t", 3, 4, 3000, sv, combos, oracle.characterize, rho=0.85)
+    tr = (c.trace_off, c.arrival, c.tier, c.words, c.tokens, c.out_len)
+    st, dn, ema, est = oracle.simulate(*tr, sv, c.instances, out_off=c.out_off, want_est=True)
+    sums = oracle.estimation_error(*tr, c.instances, c.out_off, est, st, c.group, c.n_groups).astype(np.float64)
+    n, mae, rmse = sums[:, 0], sums[:, 1] / sums[:, 0], np.sqrt(sums[:, 2] / sums[:, 0])
+    bias = sums[:, 4] / sums[:, 3]                 # observed / estimated, ~tokens per word when the factor is 1
+    assert n.tolist() == [4 * 3000] * 4
+    assert mae[1] < 0.5 * mae[0] and rmse[1] < 0.5 * rmse[0]      # paper: -38.8 % / -40.5 % on its corpus
+    assert 1.30 < bias[0] < 1.50                                   # closed form 1.3977 (SURVEY.md §8(c) C.1 pin 3)
+    assert abs(bias[1] - 1.0) < 0.03                               # Table IV: mean bias 0.999 with feedback on
+    assert mae[2] == 0 and mae[3] == 0 and bias[2] == 1.0 and bias[3] == 1.0   # tokenizer-aware: nothing to correct
