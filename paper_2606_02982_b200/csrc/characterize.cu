@@ -8,15 +8,25 @@
 //   tokflag[j]   = PUNCT[j] || (LETTER[j] && (# letters before j in its run, runs reset at prompt starts) % 4 == 0)
 //   words[i] = popcount(wordstart over [a,b)),  tokens[i] = popcount(tokflag over [a,b)).
 //
-// Design (v2, B200): every WARP is its own pipeline. It owns one contiguous span of 2 KiB chunks and a private ring
-// of kStages shared-memory stages filled by 1-D TMA bulk copies (cp.async.bulk + one mbarrier per stage, issued by
-// lane 0), so there is no block-wide barrier anywhere and the LSU pipe carries no global loads of text. Each lane
-// owns 64 contiguous bytes of the chunk: SWAR byte classification 4 bytes per 32-bit word (threshold adds on
-// x|0x80808080, XOR-combined intervals, result masked to bit 7), bit-7 compaction by IDP4A with power-of-two
-// weights, then pure 64-bit mask logic (Kogge-Stone stride-4 propagation for the mod-4 run position). Carries
-// between lanes are 2 bits + 1 bit and compose associatively; carries between chunks live in warp-uniform registers.
-// Prompt boundaries come from a 32-entry register window over offsets[]; a prompt that closes inside the warp's
-// span is a plain store, the (at most two) prompts cut by the span's edges are integer atomicAdds.
+// Design (v3, B200). The v2 kernel was bound by the ALU pipe (LOP3/SHF at half rate), not by HBM: 731 warp
+// instructions per 2 KiB. v3 cuts that to about a third:
+//  * every WARP is its own pipeline: it owns one contiguous span of 4 KiB chunks and a private ring of stages filled
+//    by 2-D TMA tile copies (32 rows x 128 B, SWIZZLE_128B, one mbarrier per stage, issued by lane 0): no block-wide
+//    barrier anywhere, and a lane reads its own 128-byte row with eight conflict-free LDS.128;
+//  * byte classification is BIT-SLICED: each 32-byte group (8 registers) is transposed into its 8 bit planes
+//    (2 PRMT stages + 3 masked-shift stages, shifts issued as IMAD/IMAD.HI on the FMA pipe), after which WS and LETTER
+//    are a ~20-LOP3 boolean network evaluated for 32 bytes at a time, and the results already are position masks;
+//  * the mod-4 position inside a letter run comes from two carry-propagating ADDs (a start bit added to the run
+//    ripples through it, so `L & ~(L + starts_of_class)` labels every byte of a run with the class of its start)
+//    instead of a Kogge-Stone shift network;
+//  * carries between lanes are one bit + one bit + a count mod 4 and compose associatively; carries between
+//    chunks live in warp-uniform registers;
+//  * prompt boundaries come from a 32-entry register window over offsets[], held as 32-bit positions relative to the
+//    warp's span; the counts at a boundary are read back from a per-32-byte table {wordstart mask, token mask,
+//    running count} that the owning lanes leave in the already consumed stage buffer. A prompt that closes inside
+//    the warp's span is a plain store, the (at most two) prompts cut by the span's edges are integer atomicAdds.
+#include <cuda.h>
+
 #include "common.cuh"
 
 namespace ds {
@@ -24,20 +34,23 @@ namespace k1 {
 
 constexpr int kWarps = 8;                     // warps per CTA (each fully independent)
 constexpr int kThreads = kWarps * 32;
-constexpr int kSeg = 64;                      // bytes per lane per chunk
-constexpr int kChunk = 32 * kSeg;             // 2 KiB per warp per step
-constexpr int kStages = 4;
-constexpr int kCtasPerSM = 3;
+constexpr int NW = 4;                         // 32-byte groups (= 32-bit mask words) per lane per chunk
+constexpr int kSeg = 32 * NW;                 // 128 bytes per lane per chunk = one TMA box row
+constexpr int kChunk = 32 * kSeg;             // 4 KiB per warp per step
+constexpr int kStages = 3;
+constexpr int kCtasPerSM = 2;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr long long kInfOff = 0x7fffffffffffffffLL;
+constexpr unsigned kNoRel = 0xffffffffu;      // "no boundary" in span-relative 32-bit positions
+static_assert(kChunk % 4 == 0 && kSeg == 128, "a TMA box row is one 128-byte swizzle row");
 
 struct Smem {
-  alignas(128) uint8_t data[kWarps][kStages][kChunk];
+  alignas(1024) uint8_t data[kWarps][kStages][kChunk];   // SWIZZLE_128B needs 1024-byte aligned stages
+  unsigned int sbits[kWarps][kChunk / 32];               // prompt-start bit per byte of the warp's current chunk
   unsigned long long mbar[kWarps][kStages];
-  unsigned int sbits[kWarps][kChunk / 32];    // prompt-start bit per byte of the warp's current chunk
 };
 
-// ---- PTX wrappers: mbarrier + 1-D TMA bulk copy (SASS: UBLKCP, SYNCS) ----
+// ---- PTX wrappers: mbarrier + 2-D TMA tile copy (SASS: UTMALDG, SYNCS) ----
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
@@ -58,51 +71,62 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
       "}\n" ::"r"(smem_u32(bar)), "r"(parity)
       : "memory");
 }
-__device__ __forceinline__ void tma_load_1d(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+// rows [row, row+32) x 128 bytes of the text viewed as u8[rows][128] -> 4 KiB at dst, 16-byte pieces XOR-swizzled by row&7
+__device__ __forceinline__ void tma_load_rows(void* dst, const CUtensorMap* map, int row, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+                   smem_u32(dst)),
+               "l"(map), "r"(0), "r"(row), "r"(smem_u32(bar))
                : "memory");
 }
 
-// ---- byte classification, 4 bytes per 32-bit word ----
-// z = x|0x80808080 keeps every byte >= 0x80 so the per-byte subtractions never borrow across bytes; bit 7 of
-// (z - n*0x01010101) is (low7(x) >= n). Intervals are XORs of nested thresholds. m = ~x & 0x80808080 both drops
-// bytes >= 0x80 (LETTER) and clears the 7 low garbage bits, so the results are exactly 0x80 / 0x00 per byte.
-// The threshold adds are issued as IMAD (z * one + (-n)) with a run-time `one` == 1 so that they execute on the FMA
-// pipe: the ALU pipe (LOP3/SHF/ISETP, half rate) is the limiter of this kernel, not HBM.
-__device__ __forceinline__ uint32_t thr(uint32_t z, uint32_t one, uint32_t n) {
-  uint32_t t;
-  asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(t) : "r"(z), "r"(one), "r"(0u - n * 0x01010101u));
-  return t;
-}
-__device__ __forceinline__ uint32_t lop3_xor3(uint32_t a, uint32_t b, uint32_t c) {
+// ---- bit-sliced byte classification: 32 bytes (8 words) -> WS mask, LETTER mask ----
+// Masked-shift exchange of one register-index bit with one position bit (distance S, M = positions keeping their
+// register). The shifts are multiplies by run-time powers of two so that they issue on the FMA pipe (IMAD / IMAD.HI):
+// the ALU pipe (LOP3, PRMT) is this kernel's limiter.
+struct Mul { unsigned l1, l2, l4, r1, r2, r4; };   // 2, 4, 16, 2^31, 2^30, 2^28
+__device__ __forceinline__ uint32_t shl_fma(uint32_t x, unsigned pow2) {
   uint32_t r;
-  asm("lop3.b32 %0, %1, %2, %3, 0x96;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+  asm("mul.lo.u32 %0, %1, %2;" : "=r"(r) : "r"(x), "r"(pow2));
   return r;
 }
-__device__ __forceinline__ uint32_t lop3_xor_and(uint32_t a, uint32_t b, uint32_t c) {   // (a ^ b) & c
+__device__ __forceinline__ uint32_t shr_fma(uint32_t x, unsigned pow2_of_32_minus_s) {
   uint32_t r;
-  asm("lop3.b32 %0, %1, %2, %3, 0x28;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+  asm("mul.hi.u32 %0, %1, %2;" : "=r"(r) : "r"(x), "r"(pow2_of_32_minus_s));
   return r;
 }
-__device__ __forceinline__ void classify4(uint32_t x, uint32_t one, uint32_t& ws7, uint32_t& d7) {
-  const uint32_t z = x | 0x80808080u;
-  const uint32_t m = ~x & 0x80808080u;
-  const uint32_t t9 = thr(z, one, 9), t14 = thr(z, one, 14), t32 = thr(z, one, 32), t33 = thr(z, one, 33);
-  const uint32_t t48 = thr(z, one, 48), t58 = thr(z, one, 58), t65 = thr(z, one, 65), t91 = thr(z, one, 91);
-  const uint32_t t97 = thr(z, one, 97), t123 = thr(z, one, 123), t127 = thr(z, one, 127);
-  const uint32_t s1 = lop3_xor3(t9, t14, t32);              // [9,13] u [32,..)
-  ws7 = lop3_xor_and(s1, t33, m);                           // WS = [9,13] u {32}
-  const uint32_t a = lop3_xor3(t48, t58, t65), b = lop3_xor3(t91, t97, t123);
-  d7 = lop3_xor_and(lop3_xor3(s1, a, b), t127, m);          // non-LETTER = WS u PUNCT
+template <uint32_t M>
+__device__ __forceinline__ void exchange(uint32_t& a, uint32_t& b, unsigned ml, unsigned mr) {
+  const uint32_t bs = shl_fma(b, ml), as = shr_fma(a, mr);
+  a = (a & M) | (bs & ~M);
+  b = (as & M) | (b & ~M);
 }
-
-// 8 bytes holding 0x80/0x00 -> 128 * (8-bit mask): two IDP4A with weights 1,2,4,8 | 16,32,64,128
-__device__ __forceinline__ uint32_t mask8x128(uint32_t w0, uint32_t w1) {
-  uint32_t acc;
-  asm("dp4a.u32.u32 %0, %1, %2, %3;" : "=r"(acc) : "r"(w0), "r"(0x08040201u), "r"(0u));
-  asm("dp4a.u32.u32 %0, %1, %2, %3;" : "=r"(acc) : "r"(w1), "r"(0x80402010u), "r"(acc));
-  return acc;
+__device__ __forceinline__ void prmt_pair(uint32_t& a, uint32_t& b, uint32_t s0, uint32_t s1) {
+  const uint32_t x = __byte_perm(a, b, s0), y = __byte_perm(a, b, s1);
+  a = x; b = y;
+}
+// w[i] = bytes 4i..4i+3 of the group. Register index bits (a4,a3,a2), position bits (a1,a0 | k2,k1,k0); five exchanges
+// bring the address bits into the position (natural byte order) and the bit index into the register index.
+__device__ __forceinline__ void classify32(uint32_t (&w)[8], const Mul& mu, uint32_t& ws, uint32_t& letter) {
+#pragma unroll
+  for (int i = 0; i < 4; ++i) prmt_pair(w[i], w[i + 4], 0x5410u, 0x7632u);            // a4 <-> byte-index bit 1
+#pragma unroll
+  for (int i = 0; i < 8; ++i) if (!(i & 2)) prmt_pair(w[i], w[i + 2], 0x6240u, 0x7351u);   // a3 <-> byte-index bit 0
+#pragma unroll
+  for (int i = 0; i < 4; ++i) exchange<0x33333333u>(w[i], w[i + 4], mu.l2, mu.r2);    // -> position bit 1
+#pragma unroll
+  for (int i = 0; i < 8; ++i) if (!(i & 2)) exchange<0x55555555u>(w[i], w[i + 2], mu.l1, mu.r1);   // -> position bit 0
+#pragma unroll
+  for (int i = 0; i < 8; i += 2) exchange<0x0f0f0f0fu>(w[i], w[i + 1], mu.l4, mu.r4); // a2 <-> position bit 2
+  // register r now holds bit plane k with k2 = r&1, k1 = (r>>2)&1, k0 = (r>>1)&1
+  const uint32_t b0 = w[0], b4 = w[1], b1 = w[2], b5 = w[3], b2 = w[4], b6 = w[5], b3 = w[6], b7 = w[7];
+  const uint32_t u9_13 = b3 & ((~b2 & (b1 | b0)) | (b2 & ~b1));                        // low nibble in 9..13
+  const uint32_t z0 = ~(b3 | b2 | b1 | b0);                                           // low nibble == 0
+  const uint32_t ge10 = b3 & (b2 | b1), ge11 = b3 & (b2 | (b1 & b0));
+  const uint32_t u11_14 = b3 & ((~b2 & b1 & b0) | (b2 & ~(b1 & b0)));                  // low nibble in 11..14
+  const uint32_t nonletter = ~b7 & ((~b6 & ~b5 & ~b4 & u9_13) | (~b6 & b5 & ~b4) | (~b6 & b5 & b4 & ge10) | (b6 & ~b4 & z0) |
+                                    (b6 & ~b5 & b4 & ge11) | (b6 & b5 & b4 & u11_14));
+  ws = ~b7 & ~b6 & ~b4 & ((~b5 & u9_13) | (b5 & z0));
+  letter = ~nonletter;
 }
 
 __device__ __forceinline__ bool is_ws_scalar(uint32_t c) { return (c - 9u) <= 4u || c == 32u; }
@@ -111,17 +135,59 @@ __device__ __forceinline__ bool is_letter_scalar(uint32_t c) {
   return !punct && !is_ws_scalar(c);
 }
 
-__device__ __forceinline__ int clz64(unsigned long long v) { return __clzll((long long)v); }
-__device__ __forceinline__ unsigned long long shfl64(unsigned long long v, int src) {
-  const unsigned lo = __shfl_sync(kFull, (unsigned)v, src), hi = __shfl_sync(kFull, (unsigned)(v >> 32), src);
-  return ((unsigned long long)hi << 32) | lo;
+// s = a + b over NW 32-bit words (carry chain; the carry out of the top word is dropped)
+__device__ __forceinline__ void add_wide(const uint32_t (&a)[NW], const uint32_t (&b)[NW], uint32_t (&s)[NW]) {
+  static_assert(NW == 4, "carry chain written for four words");
+  asm("add.cc.u32 %0, %4, %8;\n\t"
+      "addc.cc.u32 %1, %5, %9;\n\t"
+      "addc.cc.u32 %2, %6, %10;\n\t"
+      "addc.u32 %3, %7, %11;"
+      : "=r"(s[0]), "=r"(s[1]), "=r"(s[2]), "=r"(s[3])
+      : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]), "r"(b[2]), "r"(b[3]));
 }
-// rotate left by 16*r bits, r in 0..3
-__device__ __forceinline__ unsigned long long rotl16(uint32_t lo, uint32_t hi, int r) {
-  const uint32_t a = (r & 2) ? hi : lo, b = (r & 2) ? lo : hi;          // after the 32-bit part of the rotation: (b:a)
-  const int s = (r & 1) * 16;
-  const uint32_t nlo = __funnelshift_l(b, a, s), nhi = __funnelshift_l(a, b, s);
-  return ((unsigned long long)nhi << 32) | nlo;
+
+// Letter bytes whose 0-based position in their run is a multiple of 4.
+//   L   letter mask of the lane's 128 bytes (bit p of word g = byte 32g+p), pl = "previous byte is a letter" (L shifted
+//   up by one with the neighbour's carry), S = prompt-start bits, r_in = class of the virtual start of the run that
+//   continues into bit 0 (= -count mod 4), used only if bit 0 continues a run.
+// A start bit added to L ripples through its run and clears it, so L & ~(L + starts_of_class_c) marks every byte of
+// the runs whose start has class c; two adds (classes {0,2} and {0,1}) give both bits of the start's position mod 4,
+// and a byte is flagged iff its own position mod 4 equals that.
+__device__ __forceinline__ void token_letter_flags(const uint32_t (&L)[NW], const uint32_t (&pl)[NW], const uint32_t (&S)[NW],
+                                                   unsigned r_in, uint32_t (&tl)[NW]) {
+  uint32_t sb_any = 0;
+#pragma unroll
+  for (int g = 0; g < NW; ++g) sb_any |= L[g] & pl[g] & S[g];       // a prompt starts in the middle of a letter run
+  uint32_t aE[NW], a01[NW], s1[NW], s2[NW];
+  if (sb_any == 0) {
+#pragma unroll
+    for (int g = 0; g < NW; ++g) { aE[g] = L[g] & ~pl[g] & 0x55555555u; a01[g] = L[g] & ~pl[g] & 0x33333333u; }
+    const uint32_t c0 = L[0] & pl[0] & 1u;                            // bit 0 continues the previous lane's run
+    aE[0] |= c0 & ~r_in; a01[0] |= c0 & ~(r_in >> 1);
+    add_wide(L, aE, s1); add_wide(L, a01, s2);
+#pragma unroll
+    for (int g = 0; g < NW; ++g) tl[g] = L[g] & ~(s1[g] ^ 0xAAAAAAAAu) & ~(s2[g] ^ 0xCCCCCCCCu);
+    return;
+  }
+  // rare path: cut the runs at the in-run prompt starts by removing that letter (it is a run start: flag set), and
+  // give the run that follows it the class of the removed position
+  uint32_t Lp[NW], SB[NW], SB1[NW];
+#pragma unroll
+  for (int g = 0; g < NW; ++g) { SB[g] = L[g] & pl[g] & S[g]; Lp[g] = L[g] & ~SB[g]; }
+#pragma unroll
+  for (int g = 0; g < NW; ++g) SB1[g] = (SB[g] << 1) | (g ? SB[g - 1] >> 31 : 0u);
+#pragma unroll
+  for (int g = 0; g < NW; ++g) {
+    const uint32_t prevl = (Lp[g] << 1) | (g ? Lp[g - 1] >> 31 : (pl[0] & 1u));
+    const uint32_t st = Lp[g] & ~prevl, n = st & ~SB1[g], x = st & SB1[g];
+    aE[g] = (n & 0x55555555u) | (x & 0xAAAAAAAAu);
+    a01[g] = (n & 0x33333333u) | (x & 0x66666666u);
+  }
+  const uint32_t c0 = Lp[0] & pl[0] & 1u;
+  aE[0] |= c0 & ~r_in; a01[0] |= c0 & ~(r_in >> 1);
+  add_wide(Lp, aE, s1); add_wide(Lp, a01, s2);
+#pragma unroll
+  for (int g = 0; g < NW; ++g) tl[g] = (Lp[g] & ~(s1[g] ^ 0xAAAAAAAAu) & ~(s2[g] ^ 0xCCCCCCCCu)) | SB[g];
 }
 
 // number of k in [0,n) with off[k] < pos; executed by one full warp, 32-ary search (offsets non-decreasing)
@@ -143,9 +209,10 @@ __device__ __forceinline__ long long warp_count_lt(const int64_t* __restrict__ o
 }
 
 __global__ void __launch_bounds__(kThreads, kCtasPerSM)
-characterize_kernel(const uint8_t* __restrict__ bytes, long long n_bytes, const int64_t* __restrict__ off, long long n_prompts,
-                    int32_t* __restrict__ words, int32_t* __restrict__ tokens, long long n_chunks, unsigned int* status, unsigned int one) {
-  extern __shared__ __align__(128) unsigned char smem_raw[];
+characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __restrict__ bytes, long long n_bytes,
+                    const int64_t* __restrict__ off, long long n_prompts, int32_t* __restrict__ words, int32_t* __restrict__ tokens,
+                    long long n_chunks, long long n_tma_chunks, unsigned int* status, Mul mu) {
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
   Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -154,7 +221,7 @@ characterize_kernel(const uint8_t* __restrict__ bytes, long long n_bytes, const 
   if (c_begin >= c_end) return;                                                     // (no block-wide barrier below)
 
   const long long mis = (long long)((unsigned long long)bytes & 15ull);
-  const uint8_t* abase = bytes - mis;                         // 16-byte aligned
+  const uint8_t* abase = bytes - mis;                         // 16-byte aligned; chunk c = abase[c*kChunk, (c+1)*kChunk)
   const long long load_end = (mis + n_bytes + 15) & ~15ll;    // bytes from abase that may be read
   unsigned long long* mbar = sm.mbar[warp];
   uint8_t (*stage)[kChunk] = sm.data[warp];
@@ -165,28 +232,32 @@ characterize_kernel(const uint8_t* __restrict__ bytes, long long n_bytes, const 
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
-  sb[lane] = 0u; sb[lane + 32] = 0u;
+#pragma unroll
+  for (int k = 0; k < kChunk / 32 / 32; ++k) sb[lane + 32 * k] = 0u;
   __syncwarp();
 
-  auto issue = [&](unsigned it) {  // lane 0 only: chunk c_begin + it -> stage it % kStages
-    const int s = (int)(it & (kStages - 1));
-    const long long a0 = (c_begin + it) * (long long)kChunk;
-    long long len = load_end - a0;
-    if (len > kChunk) len = kChunk;
-    mbar_expect_tx(&mbar[s], (unsigned)len);
-    tma_load_1d(stage[s], abase + a0, (unsigned)len, &mbar[s]);
+  // chunks [0, n_tma_chunks) lie wholly inside the readable range and come by TMA; the last, partial one is read directly
+  auto issue = [&](unsigned it, int s) {  // lane 0 only
+    const long long c = c_begin + it;
+    if (c < n_tma_chunks) {
+      mbar_expect_tx(&mbar[s], (unsigned)kChunk);
+      tma_load_rows(stage[s], &tmap, (int)(c * 32), &mbar[s]);
+    }
   };
   const unsigned n_it = (unsigned)(c_end - c_begin);
   if (lane == 0)
-    for (unsigned it = 0; it < n_it && it < (unsigned)kStages; ++it) issue(it);
+    for (unsigned it = 0; it < n_it && it < (unsigned)kStages; ++it) issue(it, (int)it);
 
   // ---- span prologue: boundary cursor and the carries at the span's first byte ----
   const long long nb_total = n_prompts + 1;                   // boundaries off[0..n_prompts]
   const long long pos0 = c_begin * (long long)kChunk - mis;   // position (relative to bytes) of the span's first byte
   long long kb = warp_count_lt(off, nb_total, pos0, lane);    // first boundary not before the span
-  unsigned c_cnt = 0, c_prevnw = 0;                           // letters (mod 4) of the run ending at pos0-1; nonWS[pos0-1]
+  unsigned c_cnt = 0;                                         // letters (mod 4) of the run ending at pos0-1
+  unsigned c_ws = 0x80000000u, c_L = 0u;                      // bit 31: byte pos0-1 is WS / is a LETTER (lane 0's carry-in)
   if (pos0 > 0) {
-    c_prevnw = !is_ws_scalar(bytes[pos0 - 1]);
+    const uint32_t pb = bytes[pos0 - 1];
+    c_ws = is_ws_scalar(pb) ? 0x80000000u : 0u;
+    c_L = is_letter_scalar(pb) ? 0x80000000u : 0u;
     const long long lb = kb >= 1 ? max((long long)off[kb - 1], 0ll) : 0ll;   // runs reset at the last boundary before pos0
     long long k = pos0 - 1;
     bool found = false;
@@ -200,31 +271,78 @@ characterize_kernel(const uint8_t* __restrict__ bytes, long long n_bytes, const 
   }
   unsigned accW = 0, accT = 0;        // flags seen so far in the prompt that is open at the current position
   bool open_before_span = true;       // that prompt started before this warp's span (other warps add to it too)
-  long long last_o = -1;              // largest boundary seen (validation of monotonicity across windows)
+  unsigned last_rel = 0;              // largest boundary seen, span-relative (validation of monotonicity across windows)
 
-  // boundary window: lane holds off[kb + lane]
-  long long o = kInfOff;
+  // boundary window: lane holds off[kb + lane] as a 32-bit position relative to pos0 (kNoRel: none / beyond 4 GiB)
+  unsigned orel = kNoRel;
   auto load_window = [&]() {
     const long long idx = kb + lane;
-    o = idx < nb_total ? off[idx] : kInfOff;
-    long long prev = __shfl_up_sync(kFull, o, 1);
-    if (lane == 0) prev = last_o;
-    if (idx < nb_total && (o < 0 || o > n_bytes || o < prev)) atomicOr(status, DS_DEV_BAD_OFFSETS);
+    const bool have = idx < nb_total;
+    const long long o = have ? off[idx] : kInfOff;
+    const long long d = o - pos0;
+    orel = (d < 0 || d >= (long long)kNoRel) ? kNoRel : (unsigned)d;
+    unsigned prev = __shfl_up_sync(kFull, orel, 1);
+    if (lane == 0) prev = last_rel;
+    if (have && (o < 0 || o > n_bytes || d < 0 || orel < prev)) atomicOr(status, DS_DEV_BAD_OFFSETS);
   };
   load_window();
 
-  const int rot = (lane >> 1) & 3;    // 16-byte pieces are read in rotated order: conflict-free LDS.128 at a 64-byte lane stride
-  static_assert((kStages & (kStages - 1)) == 0, "kStages must be a power of two");
-  long long cs = pos0;
-  for (unsigned it = 0; it < n_it; ++it, cs += kChunk) {
-    const int s = (int)(it & (kStages - 1));
-    const unsigned parity = (it / kStages) & 1u;
-    const long long ce = cs + kChunk;   // chunk = positions [cs,ce) relative to bytes
+  // lane's eight 16-byte pieces inside a stage (SWIZZLE_128B: piece p of row r sits at piece p ^ (r & 7))
+  const uint8_t* lrow = &stage[0][0] + lane * kSeg;
+  const unsigned lx = (unsigned)(lane & 7) << 4;
+  const int lane_prev = (lane + 31) & 31;
 
-    // (a) prompt boundaries inside this chunk -> start bits (lanes 0..nb-1 of the window hold them)
-    bool inb = o >= cs && o < ce;
+  int s = 0;
+  unsigned parity = 0, crel = 0;      // stage index, its mbarrier phase, chunk start relative to pos0
+  long long cs = pos0;
+  for (unsigned it = 0; it < n_it; ++it, cs += kChunk, crel += kChunk) {
+    const long long ce = cs + kChunk;   // chunk = positions [cs,ce) relative to bytes
+    const bool by_tma = c_begin + it < n_tma_chunks;
+
+    // (a) the lane's 128 bytes -> WS / LETTER masks, 32 bytes at a time
+    uint32_t ws[NW], L[NW];
+    if (by_tma) {
+      mbar_wait(&mbar[s], parity);
+      const uint8_t* row = lrow + s * kChunk;
+#pragma unroll
+      for (int g = 0; g < NW; ++g) {
+        const uint4 v0 = *reinterpret_cast<const uint4*>(row + (((2 * g) << 4) ^ lx));
+        const uint4 v1 = *reinterpret_cast<const uint4*>(row + (((2 * g + 1) << 4) ^ lx));
+        uint32_t w[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
+        classify32(w, mu, ws[g], L[g]);
+      }
+    } else {                            // partial last chunk: guarded 16-byte loads, zero beyond the readable range
+      const long long a0 = (c_begin + it) * (long long)kChunk + lane * kSeg;
+#pragma unroll
+      for (int g = 0; g < NW; ++g) {
+        uint4 v[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const long long a = a0 + (2 * g + h) * 16;
+          v[h] = a < load_end ? *reinterpret_cast<const uint4*>(abase + a) : make_uint4(0u, 0u, 0u, 0u);
+        }
+        uint32_t w[8] = {v[0].x, v[0].y, v[0].z, v[0].w, v[1].x, v[1].y, v[1].z, v[1].w};
+        classify32(w, mu, ws[g], L[g]);
+      }
+    }
+    if (cs < 0 || ce > n_bytes) {       // bytes outside [0,n_bytes) count as whitespace
+#pragma unroll
+      for (int g = 0; g < NW; ++g) {
+        const long long sp = cs + (long long)lane * kSeg + 32 * g;
+        long long lo = -sp, hi = n_bytes - sp;
+        lo = lo < 0 ? 0 : (lo > 32 ? 32 : lo);
+        hi = hi < 0 ? 0 : (hi > 32 ? 32 : hi);
+        uint32_t valid = 0u;
+        if (hi > lo) valid = (hi == 32 ? ~0u : ((1u << hi) - 1u)) & ~((1u << lo) - 1u);
+        ws[g] |= ~valid; L[g] &= valid;
+      }
+    }
+
+    // (b) prompt boundaries inside this chunk -> start bits (the window's lanes hold them in order)
+    unsigned rel = orel - crel;
+    bool inb = rel < (unsigned)kChunk;
     unsigned bm = __ballot_sync(kFull, inb);
-    if (inb) atomicOr(&sb[(int)(o - cs) >> 5], 1u << ((int)(o - cs) & 31));
+    if (inb) atomicOr(&sb[rel >> 5], 1u << (rel & 31));
     if (bm == kFull) {                                   // rare: more than 32 boundaries may fall into one chunk
       for (long long kk = kb + 32; kk < nb_total; kk += 32) {
         const long long idx = kk + lane;
@@ -234,94 +352,80 @@ characterize_kernel(const uint8_t* __restrict__ bytes, long long n_bytes, const 
         if (__ballot_sync(kFull, in2) != kFull) break;
       }
     }
-
-    // (b) wait for the chunk, classify own 64 bytes
-    mbar_wait(&mbar[s], parity);
-    const uint8_t* seg = stage[s] + lane * kSeg;
-    uint32_t wf[4], df[4];                               // 128 x (16-bit mask) of piece (j+rot)&3
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const int r = (j + rot) & 3;
-      const uint4 v = *reinterpret_cast<const uint4*>(seg + r * 16);
-      uint32_t w0, w1, w2, w3, e0, e1, e2, e3;
-      classify4(v.x, one, w0, e0); classify4(v.y, one, w1, e1); classify4(v.z, one, w2, e2); classify4(v.w, one, w3, e3);
-      wf[j] = mask8x128(w2, w3) * 256u + mask8x128(w0, w1);
-      df[j] = mask8x128(e2, e3) * 256u + mask8x128(e0, e1);
-    }
     __syncwarp();
-    if (lane == 0 && it + kStages < n_it) issue(it + kStages);   // the stage's bytes are all in registers now
-    unsigned long long ws = rotl16(wf[1] * 512u + (wf[0] >> 7), wf[3] * 512u + (wf[2] >> 7), rot);
-    unsigned long long d = rotl16(df[1] * 512u + (df[0] >> 7), df[3] * 512u + (df[2] >> 7), rot);
-    if (cs < 0 || ce > n_bytes) {                        // bytes outside [0,n_bytes) count as whitespace
-      const long long sp = cs + (long long)lane * kSeg;
-      long long lo = -sp, hi = n_bytes - sp;
-      lo = lo < 0 ? 0 : (lo > 64 ? 64 : lo);
-      hi = hi < 0 ? 0 : (hi > 64 ? 64 : hi);
-      unsigned long long valid = 0ull;
-      if (hi > lo) valid = (hi == 64 ? ~0ull : ((1ull << hi) - 1ull)) & ~((1ull << lo) - 1ull);
-      ws |= ~valid; d |= ~valid;
-    }
-    const unsigned long long S = *reinterpret_cast<const unsigned long long*>(sb + 2 * lane);
-    *reinterpret_cast<unsigned long long*>(sb + 2 * lane) = 0ull;
+    const uint4 S4 = reinterpret_cast<const uint4*>(sb)[lane];
+    reinterpret_cast<uint4*>(sb)[lane] = make_uint4(0u, 0u, 0u, 0u);
+    const uint32_t S[NW] = {S4.x, S4.y, S4.z, S4.w};
 
-    // (c) letter-run summary of this segment and the carries between lanes
-    const unsigned long long L = ~d, nonws = ~ws;
-    const unsigned long long cont = L & ~S & ((L << 1) | 1ull);   // letter that continues the previous byte's run
-    const bool has_break = cont != ~0ull;
+    // (c) carries between lanes: one WS bit, one LETTER bit, the letter count (mod 4) of the run that is still open
+    const unsigned rw = __shfl_sync(kFull, ws[NW - 1], lane_prev), rl = __shfl_sync(kFull, L[NW - 1], lane_prev);
+    const unsigned wprev = lane ? rw : c_ws, lprev = lane ? rl : c_L;
+    c_ws = rw; c_L = rl;                                              // lane 0 keeps lane 31's words for the next chunk
+    uint32_t pw[NW], pl[NW];                                          // previous byte is WS / is a LETTER
+#pragma unroll
+    for (int g = 0; g < NW; ++g) {
+      pw[g] = __funnelshift_l(g ? ws[g - 1] : wprev, ws[g], 1);
+      pl[g] = __funnelshift_l(g ? L[g - 1] : lprev, L[g], 1);
+    }
+    uint32_t call = ~0u;                                              // AND of the continuation masks
+#pragma unroll
+    for (int g = 0; g < NW; ++g) call &= L[g] & pl[g] & ~S[g];
+    const bool has_break = call != ~0u;
     unsigned cnt_out = 0;
     if (has_break) {
-      const int k = clz64(~cont);                                 // trailing continuation bytes
-      cnt_out = (unsigned)(k + (int)((L >> (63 - k)) & 1ull)) & 3u;
+      // highest byte that does not continue its predecessor's run: the trailing run starts there (if a letter) or after it
+      int g = NW - 1;
+      uint32_t ct = L[g] & pl[g] & ~S[g];
+      while (ct == ~0u) { --g; ct = g == 2 ? (L[2] & pl[2] & ~S[2]) : g == 1 ? (L[1] & pl[1] & ~S[1]) : (L[0] & pl[0] & ~S[0]); }
+      const uint32_t lt = g == 3 ? L[3] : g == 2 ? L[2] : g == 1 ? L[1] : L[0];
+      const int k = __clz((int)~ct);                                 // trailing continuation bytes (mod 32)
+      cnt_out = (unsigned)(k + (int)((lt >> (31 - k)) & 1u)) & 3u;    // lower words add multiples of 32 = 0 (mod 4)
     }
     const unsigned brk_mask = __ballot_sync(kFull, has_break);
     const unsigned below = brk_mask & ((1u << lane) - 1u);
     const unsigned from_lane = __shfl_sync(kFull, cnt_out, below ? 31 - __clz(below) : 0);
     const unsigned cnt_in = below ? from_lane : c_cnt;
-    unsigned prevnw = __shfl_up_sync(kFull, (unsigned)(nonws >> 63), 1);
-    if (lane == 0) prevnw = c_prevnw;
-    c_prevnw = __shfl_sync(kFull, (unsigned)(nonws >> 63), 31);
-    if (brk_mask) c_cnt = __shfl_sync(kFull, cnt_out, 31 - __clz(brk_mask));   // else unchanged: 2048 = 0 (mod 4)
+    if (brk_mask) c_cnt = __shfl_sync(kFull, cnt_out, 31 - __clz(brk_mask));   // else unchanged: 4096 = 0 (mod 4)
 
-    // (d) flags
-    const unsigned long long fwm = nonws & (S | ~((nonws << 1) | (unsigned long long)prevnw));
-    unsigned long long F = L & ~cont;                             // run starts
-    if (cont & 1ull) {                                            // the carried-in run's next multiple-of-4 position
-      const unsigned q = (4u - cnt_in) & 3u;
-      const unsigned long long mq = (2ull << q) - 1ull;
-      if ((cont & mq) == mq) F |= 1ull << q;
+    // (d) flags and their counts per 32-byte word, packed words | tokens << 16
+    uint32_t tl[NW], fw[NW], ft[NW], cpk[NW];
+    token_letter_flags(L, pl, S, (4u - cnt_in) & 3u, tl);
+    unsigned own = 0;
+#pragma unroll
+    for (int g = 0; g < NW; ++g) {
+      fw[g] = ~ws[g] & (S[g] | pw[g]);
+      ft[g] = tl[g] | (~ws[g] & ~L[g]);
+      cpk[g] = (unsigned)__popc(fw[g]) + ((unsigned)__popc(ft[g]) << 16);
+      own += cpk[g];
     }
-    unsigned long long P = cont & (cont << 1) & (cont << 2) & (cont << 3);
-    F |= (F << 4) & P;  P &= P << 4;
-    F |= (F << 8) & P;  P &= P << 8;
-    F |= (F << 16) & P; P &= P << 16;
-    F |= (F << 32) & P;
-    const unsigned long long ftm = F | (d & ~ws);
-    const unsigned own = (unsigned)__popcll(fwm) | ((unsigned)__popcll(ftm) << 16);
-    const unsigned total = __reduce_add_sync(kFull, own);         // <= 2048 per field: no carry between the halves
+    const unsigned total = __reduce_add_sync(kFull, own);             // <= 4096 per field: no carry between the halves
 
     // (e) attribute to prompts: boundary k (= off[k]) closes prompt k-1
-    unsigned base_c = 0;                                          // packed prefix count at the last boundary handled
+    unsigned base_c = 0;                                              // packed prefix count at the last boundary handled
     if (bm) {
-      unsigned incl = own;                                        // inclusive prefix over lanes
+      unsigned incl = own;                                            // inclusive prefix over lanes
 #pragma unroll
       for (int sft = 1; sft < 32; sft <<= 1) {
         const unsigned y = __shfl_up_sync(kFull, incl, sft);
         if (lane >= sft) incl += y;
       }
-      const unsigned cum = incl - own;
+      // table in the consumed stage: per 32-byte word {wordstart mask, token mask, packed count before the word}
+      uint4* att = reinterpret_cast<uint4*>(stage[s]);
+      unsigned run = incl - own;
+#pragma unroll
+      for (int g = 0; g < NW; ++g) { att[lane * NW + g] = make_uint4(fw[g], ft[g], run, 0u); run += cpk[g]; }
+      __syncwarp();
       for (;;) {
         const int nb = __popc(bm);
-        const int rel = inb ? (int)(o - cs) : 0;
-        const int t = rel >> 6, bit = rel & 63;
-        const unsigned cum_t = __shfl_sync(kFull, cum, t);
-        const unsigned long long fw_t = shfl64(fwm, t), ft_t = shfl64(ftm, t);
-        const unsigned long long mk = (1ull << bit) - 1ull;
-        const unsigned cj = cum_t + (unsigned)__popcll(fw_t & mk) + ((unsigned)__popcll(ft_t & mk) << 16);
+        const unsigned r = inb ? rel : 0u;
+        const uint4 a = att[r >> 5];
+        const unsigned mk = (1u << (r & 31)) - 1u;
+        const unsigned cj = a.z + (unsigned)__popc(a.x & mk) + ((unsigned)__popc(a.y & mk) << 16);
         unsigned prev = __shfl_up_sync(kFull, cj, 1);
         if (lane == 0) prev = base_c;
-        const unsigned dlt = cj - prev;                           // both fields are non-decreasing: no borrow
+        const unsigned dlt = cj - prev;                               // both fields are non-decreasing: no borrow
         unsigned nwd = dlt & 0xffffu, ntk = dlt >> 16;
-        const long long p = kb + lane - 1;                        // prompt closed by this lane's boundary
+        const long long p = kb + lane - 1;                            // prompt closed by this lane's boundary
         if (lane == 0) { nwd += accW; ntk += accT; }
         if (inb && p >= 0) {
           if (lane == 0 && open_before_span) {
@@ -333,11 +437,12 @@ characterize_kernel(const uint8_t* __restrict__ bytes, long long n_bytes, const 
         }
         accW = 0; accT = 0; open_before_span = false;
         base_c = __shfl_sync(kFull, cj, nb - 1);
-        last_o = __shfl_sync(kFull, o, nb - 1);
+        last_rel = __shfl_sync(kFull, orel, nb - 1);
         kb += nb;
         load_window();
         if (nb < 32) break;
-        inb = o >= cs && o < ce;
+        rel = orel - crel;
+        inb = rel < (unsigned)kChunk;
         bm = __ballot_sync(kFull, inb);
         if (!bm) break;
       }
@@ -345,6 +450,13 @@ characterize_kernel(const uint8_t* __restrict__ bytes, long long n_bytes, const 
     const unsigned tail = total - base_c;
     accW += tail & 0xffffu; accT += tail >> 16;
     __syncwarp();
+
+    // (f) the stage (text and table) is dead: refill it with the chunk kStages ahead
+    if (lane == 0 && it + kStages < n_it) {
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      issue(it + kStages, s);
+    }
+    if (++s == kStages) { s = 0; parity ^= 1u; }
   }
 
   // the prompt still open at the span's end continues in the next warp's span
@@ -360,11 +472,27 @@ size_t ws_characterize(int64_t, int64_t) { return 256; }
 
 }  // namespace ds
 
+namespace {
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled() {   // driver entry point through the runtime: no link-time dependency on libcuda
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+  }
+  return fn;
+}
+}  // namespace
+
 extern "C" int ds_characterize(const uint8_t* bytes, int64_t n_bytes, const int64_t* offsets, int64_t n_prompts,
                                int32_t* words_out, int32_t* tokens_out, void* workspace, size_t workspace_bytes, void* stream) {
   using namespace ds;
   (void)workspace; (void)workspace_bytes;
-  if (n_bytes < 0 || n_prompts < 0) return DS_EINVAL;
+  if (n_bytes < 0 || n_prompts < 0 || n_bytes > (1ll << 44)) return DS_EINVAL;
   if (n_prompts > 0 && (!offsets || !words_out || !tokens_out)) return DS_EINVAL;
   if (n_bytes > 0 && !bytes) return DS_EINVAL;
   if (n_prompts == 0) return DS_OK;
@@ -375,7 +503,22 @@ extern "C" int ds_characterize(const uint8_t* bytes, int64_t n_bytes, const int6
   DS_CUDA(cudaMemsetAsync(tokens_out, 0, sizeof(int32_t) * (size_t)n_prompts, st));
   if (n_bytes == 0) return DS_OK;
   const long long mis = (long long)((unsigned long long)bytes & 15ull);
+  const long long load_end = (mis + n_bytes + 15) & ~15ll;
   const long long n_chunks = (mis + n_bytes + k1::kChunk - 1) / k1::kChunk;
+  const long long n_tma_chunks = load_end / k1::kChunk;          // chunks wholly inside the readable range
+  CUtensorMap tmap;
+  memset(&tmap, 0, sizeof(tmap));
+  if (n_tma_chunks > 0) {
+    EncodeTiledFn enc = encode_tiled();
+    if (!enc) return cuda_fail(cudaErrorNotSupported);
+    const cuuint64_t dims[2] = {(cuuint64_t)k1::kSeg, (cuuint64_t)n_tma_chunks * 32ull};
+    const cuuint64_t strides[1] = {(cuuint64_t)k1::kSeg};
+    const cuuint32_t box[2] = {(cuuint32_t)k1::kSeg, 32u};
+    const cuuint32_t estr[2] = {1u, 1u};
+    if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, (void*)(bytes - mis), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return cuda_fail(cudaErrorInvalidValue);
+  }
   static bool attr_set = false;
   if (!attr_set) {
     DS_CUDA(cudaFuncSetAttribute(k1::characterize_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(k1::Smem)));
@@ -384,8 +527,9 @@ extern "C" int ds_characterize(const uint8_t* bytes, int64_t n_bytes, const int6
   long long grid = (long long)kNumSMs * k1::kCtasPerSM;
   const long long need = (n_chunks + k1::kWarps - 1) / k1::kWarps;
   if (grid > need) grid = need;
-  k1::characterize_kernel<<<(unsigned)grid, k1::kThreads, sizeof(k1::Smem), st>>>(bytes, n_bytes, offsets, n_prompts, words_out,
-                                                                               tokens_out, n_chunks, status, 1u);
+  const k1::Mul mu = {2u, 4u, 16u, 1u << 31, 1u << 30, 1u << 28};
+  k1::characterize_kernel<<<(unsigned)grid, k1::kThreads, sizeof(k1::Smem), st>>>(tmap, bytes, n_bytes, offsets, n_prompts, words_out,
+                                                                               tokens_out, n_chunks, n_tma_chunks, status, mu);
   note_launch();
   DS_CUDA(cudaGetLastError());
   return DS_OK;
