@@ -37,8 +37,8 @@ constexpr int kThreads = kWarps * 32;
 constexpr int NW = 4;                         // 32-byte groups (= 32-bit mask words) per lane per chunk
 constexpr int kSeg = 32 * NW;                 // 128 bytes per lane per chunk = one TMA box row
 constexpr int kChunk = 32 * kSeg;             // 4 KiB per warp per step
-constexpr int kStages = 3;
-constexpr int kCtasPerSM = 2;
+constexpr int kStages = 2;
+constexpr int kCtasPerSM = 3;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr long long kInfOff = 0x7fffffffffffffffLL;
 constexpr unsigned kNoRel = 0xffffffffu;      // "no boundary" in span-relative 32-bit positions
@@ -95,10 +95,16 @@ __device__ __forceinline__ uint32_t shr_fma(uint32_t x, unsigned pow2_of_32_minu
   return r;
 }
 template <uint32_t M>
+__device__ __forceinline__ uint32_t bitsel(uint32_t x, uint32_t y) {   // (x & M) | (y & ~M) as ONE LOP3 with one immediate
+  uint32_t r;
+  asm("lop3.b32 %0, %1, %2, %3, 0xE4;" : "=r"(r) : "r"(x), "r"(y), "n"(M));
+  return r;
+}
+template <uint32_t M>
 __device__ __forceinline__ void exchange(uint32_t& a, uint32_t& b, unsigned ml, unsigned mr) {
   const uint32_t bs = shl_fma(b, ml), as = shr_fma(a, mr);
-  a = (a & M) | (bs & ~M);
-  b = (as & M) | (b & ~M);
+  a = bitsel<M>(a, bs);
+  b = bitsel<M>(as, b);
 }
 __device__ __forceinline__ void prmt_pair(uint32_t& a, uint32_t& b, uint32_t s0, uint32_t s1) {
   const uint32_t x = __byte_perm(a, b, s0), y = __byte_perm(a, b, s1);
@@ -146,48 +152,34 @@ __device__ __forceinline__ void add_wide(const uint32_t (&a)[NW], const uint32_t
       : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]), "r"(b[2]), "r"(b[3]));
 }
 
-// Letter bytes whose 0-based position in their run is a multiple of 4.
-//   L   letter mask of the lane's 128 bytes (bit p of word g = byte 32g+p), pl = "previous byte is a letter" (L shifted
-//   up by one with the neighbour's carry), S = prompt-start bits, r_in = class of the virtual start of the run that
-//   continues into bit 0 (= -count mod 4), used only if bit 0 continues a run.
-// A start bit added to L ripples through its run and clears it, so L & ~(L + starts_of_class_c) marks every byte of
-// the runs whose start has class c; two adds (classes {0,2} and {0,1}) give both bits of the start's position mod 4,
-// and a byte is flagged iff its own position mod 4 equals that.
-__device__ __forceinline__ void token_letter_flags(const uint32_t (&L)[NW], const uint32_t (&pl)[NW], const uint32_t (&S)[NW],
-                                                   unsigned r_in, uint32_t (&tl)[NW]) {
-  uint32_t sb_any = 0;
-#pragma unroll
-  for (int g = 0; g < NW; ++g) sb_any |= L[g] & pl[g] & S[g];       // a prompt starts in the middle of a letter run
+// Token flags of the lane's 128 bytes: PUNCT bytes, run starts, and continuation letters whose 0-based position in their
+// run is a multiple of 4.
+//   L = letter mask (bit p of word g = byte 32g+p), C = L & "previous byte is a letter" & ~prompt_start = letters that
+//   CONTINUE a run (so prompt starts cut runs for free), r_in = position class of the virtual start of the run that
+//   continues into bit 0 (= -count mod 4; used only if C bit 0 is set).
+// A carry injected at the first continuation byte of a run ripples through the run's continuation bytes and clears
+// them, so C & ~(C + inject_c) marks the runs whose START has a position class in set c; two adds (c = even, c in
+// {0,1}) give both bits of the start's position mod 4, and a continuation byte is flagged iff its own position mod 4
+// equals that.
+__device__ __forceinline__ void token_flags(const uint32_t (&L)[NW], const uint32_t (&C)[NW], const uint32_t (&ws)[NW],
+                                            unsigned r_in, uint32_t (&ft)[NW]) {
   uint32_t aE[NW], a01[NW], s1[NW], s2[NW];
-  if (sb_any == 0) {
-#pragma unroll
-    for (int g = 0; g < NW; ++g) { aE[g] = L[g] & ~pl[g] & 0x55555555u; a01[g] = L[g] & ~pl[g] & 0x33333333u; }
-    const uint32_t c0 = L[0] & pl[0] & 1u;                            // bit 0 continues the previous lane's run
-    aE[0] |= c0 & ~r_in; a01[0] |= c0 & ~(r_in >> 1);
-    add_wide(L, aE, s1); add_wide(L, a01, s2);
-#pragma unroll
-    for (int g = 0; g < NW; ++g) tl[g] = L[g] & ~(s1[g] ^ 0xAAAAAAAAu) & ~(s2[g] ^ 0xCCCCCCCCu);
-    return;
-  }
-  // rare path: cut the runs at the in-run prompt starts by removing that letter (it is a run start: flag set), and
-  // give the run that follows it the class of the removed position
-  uint32_t Lp[NW], SB[NW], SB1[NW];
-#pragma unroll
-  for (int g = 0; g < NW; ++g) { SB[g] = L[g] & pl[g] & S[g]; Lp[g] = L[g] & ~SB[g]; }
-#pragma unroll
-  for (int g = 0; g < NW; ++g) SB1[g] = (SB[g] << 1) | (g ? SB[g - 1] >> 31 : 0u);
 #pragma unroll
   for (int g = 0; g < NW; ++g) {
-    const uint32_t prevl = (Lp[g] << 1) | (g ? Lp[g - 1] >> 31 : (pl[0] & 1u));
-    const uint32_t st = Lp[g] & ~prevl, n = st & ~SB1[g], x = st & SB1[g];
-    aE[g] = (n & 0x55555555u) | (x & 0xAAAAAAAAu);
-    a01[g] = (n & 0x33333333u) | (x & 0x66666666u);
+    const uint32_t csh = __funnelshift_l(g ? C[g - 1] : 0u, C[g], 1);   // bit 0 of the lane: always a first continuation
+    aE[g] = C[g] & ~csh & 0xAAAAAAAAu;                                  // start (= previous byte) at an even position
+    a01[g] = C[g] & ~csh & 0x66666666u;                                 // start at a position = 0, 1 (mod 4)
   }
-  const uint32_t c0 = Lp[0] & pl[0] & 1u;
+  const uint32_t c0 = C[0] & 1u;
   aE[0] |= c0 & ~r_in; a01[0] |= c0 & ~(r_in >> 1);
-  add_wide(Lp, aE, s1); add_wide(Lp, a01, s2);
+  add_wide(C, aE, s1); add_wide(C, a01, s2);
 #pragma unroll
-  for (int g = 0; g < NW; ++g) tl[g] = (Lp[g] & ~(s1[g] ^ 0xAAAAAAAAu) & ~(s2[g] ^ 0xCCCCCCCCu)) | SB[g];
+  for (int g = 0; g < NW; ++g) {
+    const uint32_t t = C[g] & ~(s1[g] ^ 0xAAAAAAAAu);
+    const uint32_t u = t & ~(s2[g] ^ 0xCCCCCCCCu);
+    const uint32_t v = (L[g] & ~C[g]) | (~ws[g] & ~L[g]);              // run starts and PUNCT bytes
+    ft[g] = u | v;
+  }
 }
 
 // number of k in [0,n) with off[k] < pos; executed by one full warp, 32-ary search (offsets non-decreasing)
@@ -291,6 +283,9 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
   const uint8_t* lrow = &stage[0][0] + lane * kSeg;
   const unsigned lx = (unsigned)(lane & 7) << 4;
   const int lane_prev = (lane + 31) & 31;
+  unsigned scan_on[5];                  // 1 if lane >= 2^k: this lane takes the scan's k-th partial sum
+#pragma unroll
+  for (int k = 0; k < 5; ++k) scan_on[k] = lane >= (1 << k) ? 1u : 0u;
 
   int s = 0;
   unsigned parity = 0, crel = 0;      // stage index, its mbarrier phase, chunk start relative to pos0
@@ -367,16 +362,16 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
       pw[g] = __funnelshift_l(g ? ws[g - 1] : wprev, ws[g], 1);
       pl[g] = __funnelshift_l(g ? L[g - 1] : lprev, L[g], 1);
     }
-    uint32_t call = ~0u;                                              // AND of the continuation masks
+    uint32_t C[NW], call = ~0u;                                       // letters that continue a run; AND over the words
 #pragma unroll
-    for (int g = 0; g < NW; ++g) call &= L[g] & pl[g] & ~S[g];
+    for (int g = 0; g < NW; ++g) { C[g] = L[g] & pl[g] & ~S[g]; call &= C[g]; }
     const bool has_break = call != ~0u;
     unsigned cnt_out = 0;
     if (has_break) {
       // highest byte that does not continue its predecessor's run: the trailing run starts there (if a letter) or after it
       int g = NW - 1;
-      uint32_t ct = L[g] & pl[g] & ~S[g];
-      while (ct == ~0u) { --g; ct = g == 2 ? (L[2] & pl[2] & ~S[2]) : g == 1 ? (L[1] & pl[1] & ~S[1]) : (L[0] & pl[0] & ~S[0]); }
+      uint32_t ct = C[g];
+      while (ct == ~0u) { --g; ct = g == 2 ? C[2] : g == 1 ? C[1] : C[0]; }
       const uint32_t lt = g == 3 ? L[3] : g == 2 ? L[2] : g == 1 ? L[1] : L[0];
       const int k = __clz((int)~ct);                                 // trailing continuation bytes (mod 32)
       cnt_out = (unsigned)(k + (int)((lt >> (31 - k)) & 1u)) & 3u;    // lower words add multiples of 32 = 0 (mod 4)
@@ -388,13 +383,12 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
     if (brk_mask) c_cnt = __shfl_sync(kFull, cnt_out, 31 - __clz(brk_mask));   // else unchanged: 4096 = 0 (mod 4)
 
     // (d) flags and their counts per 32-byte word, packed words | tokens << 16
-    uint32_t tl[NW], fw[NW], ft[NW], cpk[NW];
-    token_letter_flags(L, pl, S, (4u - cnt_in) & 3u, tl);
+    uint32_t fw[NW], ft[NW], cpk[NW];
+    token_flags(L, C, ws, (4u - cnt_in) & 3u, ft);
     unsigned own = 0;
 #pragma unroll
     for (int g = 0; g < NW; ++g) {
       fw[g] = ~ws[g] & (S[g] | pw[g]);
-      ft[g] = tl[g] | (~ws[g] & ~L[g]);
       cpk[g] = (unsigned)__popc(fw[g]) + ((unsigned)__popc(ft[g]) << 16);
       own += cpk[g];
     }
@@ -403,11 +397,11 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
     // (e) attribute to prompts: boundary k (= off[k]) closes prompt k-1
     unsigned base_c = 0;                                              // packed prefix count at the last boundary handled
     if (bm) {
-      unsigned incl = own;                                            // inclusive prefix over lanes
+      unsigned incl = own;                                            // inclusive prefix over lanes (0/1 multipliers: IMAD)
 #pragma unroll
-      for (int sft = 1; sft < 32; sft <<= 1) {
-        const unsigned y = __shfl_up_sync(kFull, incl, sft);
-        if (lane >= sft) incl += y;
+      for (int k = 0; k < 5; ++k) {
+        const unsigned y = __shfl_up_sync(kFull, incl, 1 << k);
+        asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(incl) : "r"(y), "r"(scan_on[k]));
       }
       // table in the consumed stage: per 32-byte word {wordstart mask, token mask, packed count before the word}
       uint4* att = reinterpret_cast<uint4*>(stage[s]);
