@@ -83,7 +83,7 @@ __device__ __forceinline__ void tma_load_rows(void* dst, const CUtensorMap* map,
 // Masked-shift exchange of one register-index bit with one position bit (distance S, M = positions keeping their
 // register). The shifts are multiplies by run-time powers of two so that they issue on the FMA pipe (IMAD / IMAD.HI):
 // the ALU pipe (LOP3, PRMT) is this kernel's limiter.
-struct Mul { unsigned l1, l2, l4, r1, r2, r4; };   // 2, 4, 16, 2^31, 2^30, 2^28
+struct Mul { unsigned l1, l2, l4, r1, r2, r4, p16, n16; };   // 2, 4, 16, 2^31, 2^30, 2^28, 2^16, -2^16
 __device__ __forceinline__ uint32_t shl_fma(uint32_t x, unsigned pow2) {
   uint32_t r;
   asm("mul.lo.u32 %0, %1, %2;" : "=r"(r) : "r"(x), "r"(pow2));
@@ -110,11 +110,27 @@ __device__ __forceinline__ void prmt_pair(uint32_t& a, uint32_t& b, uint32_t s0,
   const uint32_t x = __byte_perm(a, b, s0), y = __byte_perm(a, b, s1);
   a = x; b = y;
 }
+// 16-bit halves exchange [a.lo, b.lo] / [a.hi, b.hi] (PRMT 0x5410 / 0x7632) done with five multiply-adds instead of two
+// PRMTs: five FMA-pipe slots are cheaper than two ALU-pipe slots here.
+__device__ __forceinline__ uint32_t mad_fma(uint32_t x, unsigned m, uint32_t c) {
+  uint32_t r;
+  asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(r) : "r"(x), "r"(m), "r"(c));
+  return r;
+}
+__device__ __forceinline__ void halves_pair(uint32_t& a, uint32_t& b, const Mul& mu) {
+  const uint32_t ah = shr_fma(a, mu.p16), bh = shr_fma(b, mu.p16);
+  const uint32_t alo = mad_fma(ah, mu.n16, a);          // a - (a.hi << 16)
+  a = mad_fma(b, mu.p16, alo);                          // (b << 16) + a.lo
+  b = mad_fma(bh, mu.p16, ah);                          // (b.hi << 16) + a.hi
+}
+constexpr bool kHalvesOnFma = false;   // measured: no gain (an ALU-pipe op costs about two issue slots, an IMAD one)
 // w[i] = bytes 4i..4i+3 of the group. Register index bits (a4,a3,a2), position bits (a1,a0 | k2,k1,k0); five exchanges
 // bring the address bits into the position (natural byte order) and the bit index into the register index.
 __device__ __forceinline__ void classify32(uint32_t (&w)[8], const Mul& mu, uint32_t& ws, uint32_t& letter) {
 #pragma unroll
-  for (int i = 0; i < 4; ++i) prmt_pair(w[i], w[i + 4], 0x5410u, 0x7632u);            // a4 <-> byte-index bit 1
+  for (int i = 0; i < 4; ++i) {                                                       // a4 <-> byte-index bit 1
+    if (kHalvesOnFma) halves_pair(w[i], w[i + 4], mu); else prmt_pair(w[i], w[i + 4], 0x5410u, 0x7632u);
+  }
 #pragma unroll
   for (int i = 0; i < 8; ++i) if (!(i & 2)) prmt_pair(w[i], w[i + 2], 0x6240u, 0x7351u);   // a3 <-> byte-index bit 0
 #pragma unroll
@@ -229,14 +245,15 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
   __syncwarp();
 
   // chunks [0, n_tma_chunks) lie wholly inside the readable range and come by TMA; the last, partial one is read directly
+  const unsigned n_it = (unsigned)(c_end - c_begin);
+  const unsigned it_tma = n_tma_chunks <= c_begin ? 0u : (n_tma_chunks - c_begin >= (long long)n_it ? n_it : (unsigned)(n_tma_chunks - c_begin));
+  const int row0 = (int)(c_begin * 32);   // first TMA row of the span (rows < 2^31: n_bytes <= 2^37 checked by the host)
   auto issue = [&](unsigned it, int s) {  // lane 0 only
-    const long long c = c_begin + it;
-    if (c < n_tma_chunks) {
+    if (it < it_tma) {
       mbar_expect_tx(&mbar[s], (unsigned)kChunk);
-      tma_load_rows(stage[s], &tmap, (int)(c * 32), &mbar[s]);
+      tma_load_rows(stage[s], &tmap, row0 + (int)it * 32, &mbar[s]);
     }
   };
-  const unsigned n_it = (unsigned)(c_end - c_begin);
   if (lane == 0)
     for (unsigned it = 0; it < n_it && it < (unsigned)kStages; ++it) issue(it, (int)it);
 
@@ -285,14 +302,21 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
   const int lane_prev = (lane + 31) & 31;
   unsigned scan_on[5];                  // 1 if lane >= 2^k: this lane takes the scan's k-th partial sum
 #pragma unroll
-  for (int k = 0; k < 5; ++k) scan_on[k] = lane >= (1 << k) ? 1u : 0u;
+  for (int k = 0; k < 5; ++k) {         // (asm volatile: keep them in registers instead of recomputing ISETP+SEL per chunk)
+    const unsigned v = lane >= (1 << k) ? 1u : 0u;
+    asm volatile("mov.u32 %0, %1;" : "=r"(scan_on[k]) : "r"(v));
+  }
 
+  // it_tail (32-bit, loop invariant) is the chunk that reaches past n_bytes
+  const long long tail_chunk = (n_bytes + mis) / kChunk;      // first chunk whose end is beyond n_bytes
+  const unsigned it_tail = tail_chunk < c_begin ? 0u : (tail_chunk - c_begin >= (long long)n_it ? kNoRel : (unsigned)(tail_chunk - c_begin));
+  const bool head_edge = pos0 < 0;
   int s = 0;
   unsigned parity = 0, crel = 0;      // stage index, its mbarrier phase, chunk start relative to pos0
   long long cs = pos0;
   for (unsigned it = 0; it < n_it; ++it, cs += kChunk, crel += kChunk) {
     const long long ce = cs + kChunk;   // chunk = positions [cs,ce) relative to bytes
-    const bool by_tma = c_begin + it < n_tma_chunks;
+    const bool by_tma = it < it_tma;
 
     // (a) the lane's 128 bytes -> WS / LETTER masks, 32 bytes at a time
     uint32_t ws[NW], L[NW];
@@ -320,7 +344,7 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
         classify32(w, mu, ws[g], L[g]);
       }
     }
-    if (cs < 0 || ce > n_bytes) {       // bytes outside [0,n_bytes) count as whitespace
+    if ((head_edge && it == 0) || it >= it_tail) {   // cs < 0 or ce > n_bytes: bytes outside [0,n_bytes) count as whitespace
 #pragma unroll
       for (int g = 0; g < NW; ++g) {
         const long long sp = cs + (long long)lane * kSeg + 32 * g;
@@ -446,7 +470,7 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
     __syncwarp();
 
     // (f) the stage (text and table) is dead: refill it with the chunk kStages ahead
-    if (lane == 0 && it + kStages < n_it) {
+    if (lane == 0 && it + kStages < it_tma) {
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       issue(it + kStages, s);
     }
@@ -486,7 +510,7 @@ extern "C" int ds_characterize(const uint8_t* bytes, int64_t n_bytes, const int6
                                int32_t* words_out, int32_t* tokens_out, void* workspace, size_t workspace_bytes, void* stream) {
   using namespace ds;
   (void)workspace; (void)workspace_bytes;
-  if (n_bytes < 0 || n_prompts < 0 || n_bytes > (1ll << 44)) return DS_EINVAL;
+  if (n_bytes < 0 || n_prompts < 0 || n_bytes > (1ll << 37)) return DS_EINVAL;   // 128 GiB: TMA row index stays below 2^31
   if (n_prompts > 0 && (!offsets || !words_out || !tokens_out)) return DS_EINVAL;
   if (n_bytes > 0 && !bytes) return DS_EINVAL;
   if (n_prompts == 0) return DS_OK;
@@ -521,7 +545,7 @@ extern "C" int ds_characterize(const uint8_t* bytes, int64_t n_bytes, const int6
   long long grid = (long long)kNumSMs * k1::kCtasPerSM;
   const long long need = (n_chunks + k1::kWarps - 1) / k1::kWarps;
   if (grid > need) grid = need;
-  const k1::Mul mu = {2u, 4u, 16u, 1u << 31, 1u << 30, 1u << 28};
+  const k1::Mul mu = {2u, 4u, 16u, 1u << 31, 1u << 30, 1u << 28, 1u << 16, 0u - (1u << 16)};
   k1::characterize_kernel<<<(unsigned)grid, k1::kThreads, sizeof(k1::Smem), st>>>(tmap, bytes, n_bytes, offsets, n_prompts, words_out,
                                                                                tokens_out, n_chunks, n_tma_chunks, status, mu);
   note_launch();
