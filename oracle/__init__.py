@@ -50,6 +50,8 @@ def _o():
         lib.oracle_simulate.argtypes = [p, p, p, C.c_int64, p, p, p, p, p, p, p]
         lib.oracle_estimation_error.argtypes = [p, p, C.c_int64, p, p, p, p, C.c_int32, p, p]
         lib.oracle_estimation_error.restype = C.c_int
+        lib.oracle_queue_depth.argtypes = [p, p, C.c_int64, p, p, C.c_int64, C.c_int64, C.c_int64, p]
+        lib.oracle_queue_depth.restype = C.c_int
         lib.oracle_latencies.argtypes = [p, p, C.c_int64, p, p, p, p, p, p, p, p, p]
         lib.oracle_tail_stats.argtypes = [p, p, C.c_int64, C.c_int32, p, C.c_int32, p, p]
         for f in (lib.oracle_characterize, lib.oracle_simulate, lib.oracle_latencies, lib.oracle_tail_stats):
@@ -175,3 +177,17 @@ def estimation_error(trace_off, arrival, tier, words, tokens, out_len, instances
     if rc:
         raise ValueError("oracle_estimation_error: contract violation")
     return (out, seg) if want_class_seg else out
+
+
+def queue_depth(trace_off, arrival, tier, words, tokens, out_len, instances, out_off, start, t0, dt, n_samples):
+    """-> depth int32[n_inst, n_samples, 3]: requests of each tier queued (arrival <= t < start) at t = t0 + j*dt."""
+    tr, keep = _traces(trace_off, arrival, tier, words, tokens, out_len)
+    inst = _c(instances, INSTANCE_DTYPE)
+    out_off = _c(out_off, np.int64)
+    start = _c(start, np.int64)
+    depth = np.zeros((len(inst), int(n_samples), 3), np.int32)
+    rc = _o().oracle_queue_depth(C.byref(tr), _p(inst), len(inst), _p(out_off), _p(start), int(t0), int(dt), int(n_samples),
+                                 _p(depth))
+    if rc:
+        raise ValueError("oracle_queue_depth: contract violation")
+    return depth

@@ -264,3 +264,24 @@ extern "C" int oracle_estimation_error(const oracle_traces* tr, const oracle_ins
   }
   return 0;
 }
+
+// Per-tenant queue depth over time (Fig. 8): a request is queued from
+// its arrival tick until the tick it is admitted to the batch. depth[i][j][k] = #{r of tier k : arrival <= t_j < start},
+// t_j = t0 + j*dt. Written as the definition: every request increments the samples it covers.
+extern "C" int oracle_queue_depth(const oracle_traces* tr, const oracle_instance* inst, int64_t n_inst, const int64_t* out_off,
+                                  const int64_t* start_tick, int64_t t0, int64_t dt, int64_t n_samples, int32_t* depth) {
+  if (dt < 1 || n_samples < 0) return -1;
+  for (int64_t k = 0; k < n_inst * n_samples * 3; ++k) depth[k] = 0;
+  for (int64_t ii = 0; ii < n_inst; ++ii) {
+    int64_t t = inst[ii].trace, lo = tr->trace_off[t], n = tr->trace_off[t + 1] - lo;
+    for (int64_t r = 0; r < n; ++r) {
+      int64_t a = tr->arrival_tick[lo + r], st = start_tick[out_off[ii] + r];
+      for (int64_t j = 0; j < n_samples; ++j) {
+        int64_t tj = t0 + j * dt;
+        if (tj >= st) break;
+        if (tj >= a) depth[(ii * n_samples + j) * 3 + tr->tier[lo + r]] += 1;
+      }
+    }
+  }
+  return 0;
+}

@@ -57,6 +57,11 @@ int oracle_estimation_error(const oracle_traces* tr, const oracle_instance* inst
                             const int64_t* est, const int64_t* start_tick, const int32_t* group, int32_t n_groups,
                             int64_t* out, int32_t* class_seg);
 
+/* Queue depth per tenant tier over time (Fig. 8): depth[(i*n_samples + j)*3 + k] =
+ * #{requests r of instance i with tier k : arrival <= t0 + j*dt < start_tick}. dt >= 1. */
+int oracle_queue_depth(const oracle_traces* tr, const oracle_instance* inst, int64_t n_inst, const int64_t* out_off,
+                       const int64_t* start_tick, int64_t t0, int64_t dt, int64_t n_samples, int32_t* depth);
+
 /* PAPER.md:270 (queue wait vs end-to-end latency). seg outputs nullable. */
 int oracle_latencies(const oracle_traces* tr, const oracle_instance* inst, int64_t n_inst, const int64_t* out_off,
                      const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, const int64_t* t_mid,
