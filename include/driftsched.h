@@ -136,6 +136,14 @@ int ds_estimation_error(const ds_traces* tr, const ds_instance* inst, int64_t n_
                         const int64_t* est, const int64_t* start_tick, const int32_t* group, int32_t n_groups,
                         int64_t* out, int32_t* class_seg, void* stream);
 
+/* Queue depth per tenant tier over time (Fig. 8: "per-tenant queue depth"):
+ * a request is queued from its arrival tick until the tick it is admitted to the batch (start_tick).
+ *   depth[(i*n_samples + j)*3 + k] = #{requests r of instance i with tier k : arrival_r <= t0 + j*dt < start_tick_r}
+ * depth [n_inst*n_samples*3] int32 device (written); t0 any tick, dt >= 1, n_samples >= 0 (host values).
+ * Launches: 1 memset + 2 kernels. */
+int ds_queue_depth(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, const int64_t* out_off,
+                   const int64_t* start_tick, int64_t t0, int64_t dt, int64_t n_samples, int32_t* depth, void* stream);
+
 /* ---------------------------------------------------------------------------------------------- (c)
  * Latency derivation (worker timestamps separate queueing from inference):
  *   e2e = done - arrival, qdelay = start - arrival, per simulated request (same indexing as start/done).

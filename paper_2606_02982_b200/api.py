@@ -198,3 +198,15 @@ def latency_stats(trace_off, arrival, tier, words, tokens, out_len, inst, out_of
                                                      _ptr(group), n_groups, _ptr(t_mid), arr, n_pct, _ptr(e2e_out), _ptr(qdelay_out),
                                                      _ptr(count_out), _ptr(workspace), workspace.numel(), _stream()))
     return e2e_out, qdelay_out, count_out
+
+
+def queue_depth(trace_off, arrival, tier, words, tokens, out_len, inst, out_off, start, t0, dt, n_samples, out=None):
+    """ds_queue_depth -> depth int32[n_inst, n_samples, 3]."""
+    tr = _traces(trace_off, arrival, tier, words, tokens, out_len)
+    _need_cuda(inst, out_off, start, out)
+    n_inst = inst.numel() // INSTANCE_BYTES
+    if out is None:
+        out = torch.empty((n_inst, int(n_samples), 3), dtype=torch.int32, device=start.device)
+    check("ds_queue_depth", lib().ds_queue_depth(C.byref(tr), _ptr(inst), n_inst, _ptr(out_off), _ptr(start), int(t0), int(dt),
+                                                 int(n_samples), _ptr(out), _stream()))
+    return out

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdriftsched.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
-SOURCES = ["api.cu", "characterize.cu", "simulate.cu", "tail_stats.cu", "esterr.cu"]
+SOURCES = ["api.cu", "characterize.cu", "simulate.cu", "tail_stats.cu", "esterr.cu", "queue_depth.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", INCLUDE]
 # the EMA path must never be contracted into FMAs (0-ulp parity with the oracle): whole TU built with -fmad=false
