@@ -38,6 +38,10 @@ class _Server(C.Structure):
                 ("traj_every", C.c_int32)]
 
 
+class _Budget(C.Structure):
+    _fields_ = [("t_base", C.c_double * 4), ("s_tenant", C.c_double * 3), ("f_slope", C.c_double), ("f_max", C.c_double)]
+
+
 _lib = None
 
 
@@ -52,6 +56,8 @@ def _o():
         lib.oracle_estimation_error.restype = C.c_int
         lib.oracle_queue_depth.argtypes = [p, p, C.c_int64, p, p, C.c_int64, C.c_int64, C.c_int64, p]
         lib.oracle_queue_depth.restype = C.c_int
+        lib.oracle_simulate_budget.argtypes = [p, p, p, p, p, C.c_int64, p, p, p, p, p, p, p]
+        lib.oracle_simulate_budget.restype = C.c_int
         lib.oracle_latencies.argtypes = [p, p, C.c_int64, p, p, p, p, p, p, p, p, p]
         lib.oracle_tail_stats.argtypes = [p, p, C.c_int64, C.c_int32, p, C.c_int32, p, p]
         for f in (lib.oracle_characterize, lib.oracle_simulate, lib.oracle_latencies, lib.oracle_tail_stats):
@@ -191,3 +197,34 @@ def queue_depth(trace_off, arrival, tier, words, tokens, out_len, instances, out
     if rc:
         raise ValueError("oracle_queue_depth: contract violation")
     return depth
+
+
+def simulate_budget(trace_off, arrival, tier, words, tokens, out_len, category, budget, server, instances, out_off=None,
+                    want_traj=False, want_est=False):
+    """Full Eq. 1-2 estimator with per-category feedback. budget: object with t_base[4], s_tenant[3], f_slope, f_max.
+    Returns start_tick, done_tick, ema_final[n_inst,4] (then ema_traj[samples,4] if want_traj, then est if want_est)."""
+    tr, keep = _traces(trace_off, arrival, tier, words, tokens, out_len)
+    cat = _c(category, np.uint8)
+    assert cat.size == keep[1].size
+    bp = _Budget((C.c_double * 4)(*budget.t_base), (C.c_double * 3)(*budget.s_tenant), budget.f_slope, budget.f_max)
+    sv = _server(server)
+    inst = _c(instances, INSTANCE_DTYPE)
+    n_inst = len(inst)
+    if out_off is None:
+        sizes = np.array([keep[0][i["trace"] + 1] - keep[0][i["trace"]] for i in inst], np.int64)
+        out_off = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int64)
+    out_off = _c(out_off, np.int64)
+    total = int(out_off[-1])
+    start = np.full(total, -1, np.int64)
+    done = np.full(total, -1, np.int64)
+    ema = np.zeros((n_inst, 4), np.float64)
+    toff = traj = None
+    if want_traj and server.traj_every > 0:
+        toff = traj_offsets(keep[0], inst, server.traj_every)
+        traj = np.zeros((int(toff[-1]), 4), np.float64)
+    est = np.full(total, -1, np.int64) if want_est else None
+    rc = _o().oracle_simulate_budget(C.byref(tr), _p(cat), C.byref(bp), C.byref(sv), _p(inst), n_inst, _p(out_off), _p(start),
+                                     _p(done), _p(ema), _p(toff), _p(traj), _p(est))
+    if rc:
+        raise ValueError("oracle_simulate_budget: contract violation")
+    return (start, done, ema) + ((traj,) if want_traj else ()) + ((est,) if want_est else ())

@@ -55,30 +55,55 @@ extern "C" int oracle_characterize(const uint8_t* bytes, int64_t n_bytes, const 
 namespace {
 
 enum { FIFO = 0, PRIORITY = 1, WEIGHTED = 2, SJF = 3, AGING = 4 };
-enum { SPLIT = 0, EXACT = 1 };
+enum { SPLIT = 0, EXACT = 1, BUDGET_SPLIT = 2, BUDGET_EXACT = 3 };
 
 struct Sim {
   // inputs for one instance (local request index r in [0,n))
   const int64_t* arr; const uint8_t* tier; const int32_t* W; const int32_t* P; const int32_t* O;
   int64_t n; const oracle_server* sv; int policy, estimator; double alpha;
+  const uint8_t* cat = nullptr; const oracle_budget* bp = nullptr;   // budget estimators only (Eq. 1-2 in full)
   // state (SURVEY.md §8(c) C.2 "State per instance")
   int64_t now = 0, next = 0, kv_used = 0, done = 0;
-  double B[3] = {1.0, 1.0, 1.0};
+  double B[4] = {1.0, 1.0, 1.0, 1.0};   // per tier (estimators 0/1) or per semantic category (budget estimators)
   int cur = 0;                       // Weighted slot cursor
   std::vector<int64_t> queued;       // all queued requests, arrival (= index) order
   std::vector<int64_t> R;            // running set, ascending request index
   std::vector<int64_t> est, g;
 
-  int64_t base(int64_t r) const { return estimator == SPLIT ? (int64_t)W[r] : (int64_t)P[r]; }
+  bool budget() const { return estimator >= BUDGET_SPLIT; }
+  int64_t base(int64_t r) const { return (estimator == SPLIT || estimator == BUDGET_SPLIT) ? (int64_t)W[r] : (int64_t)P[r]; }
 
   // admit_to_queue(r): estimate frozen at arrival (A5), Eq. 1-2 reduced form (A1).
   void admit_to_queue(int64_t r) {
     int64_t b = base(r);
-    if (b > 0) est[r] = (int64_t)std::ceil(B[tier[r]] * (double)b); else est[r] = 0;
+    if (budget()) {
+      // Eq. 1-2; Alg. 1: T_budget = T_input + T_base * B_runtime * S_tenant * F_input,
+      // factors multiplied left to right, each product rounded; F_input = min(f_max, 1 + f_slope*T_input) (B3).
+      int c = cat[r];
+      double F = 1.0 + bp->f_slope * (double)b;
+      if (F > bp->f_max) F = bp->f_max;
+      double x = bp->t_base[c] * B[c];
+      x = x * bp->s_tenant[tier[r]];
+      x = x * F;
+      est[r] = b + (int64_t)std::ceil(x);
+    } else if (b > 0) est[r] = (int64_t)std::ceil(B[tier[r]] * (double)b); else est[r] = 0;
     queued.push_back(r);
   }
   // ema_update(k,r): Eq. 5/6 with T_actual = tokens, T_base = base (A3); four separate roundings.
   void ema_update(int k, int64_t r) {
+    if (budget()) {
+      // Eq. 5-6, PAPER.md:278-286 as printed: B_measured = T_actual / T_base with T_actual the observed output length and
+      // T_base the category baseline; one factor per workload category.
+      int c = cat[r];
+      if (alpha > 0.0 && bp->t_base[c] > 0.0) {
+        double m = (double)O[r] / bp->t_base[c];
+        double t1 = 1.0 - alpha;
+        double t2 = t1 * B[c];
+        double t3 = alpha * m;
+        B[c] = t2 + t3;
+      }
+      return;
+    }
     int64_t b = base(r);
     if (alpha > 0.0 && b > 0) {
       double m = (double)P[r] / (double)b;
@@ -124,25 +149,37 @@ struct Sim {
 
 }  // namespace
 
-extern "C" int oracle_simulate(const oracle_traces* tr, const oracle_server* sv, const oracle_instance* inst,
-                               int64_t n_inst, const int64_t* out_off, int64_t* start_tick, int64_t* done_tick,
-                               double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out) {
+static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const oracle_budget* bp, const oracle_server* sv,
+                         const oracle_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t* start_tick,
+                         int64_t* done_tick, double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out) {
+  const int nb = bp ? 4 : 3;   // factors per instance: semantic categories (budget estimators) or tenant tiers
+  if (bp) {
+    if (!category) return -1;
+    for (int c = 0; c < 4; ++c) if (!(bp->t_base[c] >= 0.0)) return -1;
+    for (int t = 0; t < 3; ++t) if (!(bp->s_tenant[t] > 0.0)) return -1;
+    if (!(bp->f_slope >= 0.0) || !(bp->f_max >= 1.0)) return -1;
+  }
   if (sv->max_batch < 1) return -1;
   if (sv->weight[0] < 1 || sv->weight[1] < 1 || sv->weight[2] < 1) return -1;
   if (sv->aging_step < 1) return -1;
   for (int64_t ii = 0; ii < n_inst; ++ii) {
     const oracle_instance& in = inst[ii];
-    if (in.trace < 0 || in.trace >= tr->n_traces || in.policy < 0 || in.policy > 4 || in.estimator < 0 ||
-        in.estimator > 1 || !(in.ema_alpha >= 0.0 && in.ema_alpha <= 1.0)) return -1;
+    if (in.trace < 0 || in.trace >= tr->n_traces || in.policy < 0 || in.policy > 4 || !(in.ema_alpha >= 0.0 && in.ema_alpha <= 1.0))
+      return -1;
+    if (bp ? (in.estimator != BUDGET_SPLIT && in.estimator != BUDGET_EXACT) : (in.estimator != SPLIT && in.estimator != EXACT)) return -1;
     int64_t lo = tr->trace_off[in.trace], n = tr->trace_off[in.trace + 1] - lo;
     Sim s;
     s.arr = tr->arrival_tick + lo; s.tier = tr->tier + lo; s.W = tr->words + lo; s.P = tr->tokens + lo;
     s.O = tr->out_len + lo; s.n = n; s.sv = sv; s.policy = in.policy; s.estimator = in.estimator; s.alpha = in.ema_alpha;
     s.est.assign(n, 0); s.g.assign(n, 0);
+    if (bp) {
+      s.cat = category + lo; s.bp = bp;
+      for (int64_t r = 0; r < n; ++r) if (s.cat[r] > 3) return -1;
+    }
     int64_t* st = start_tick + out_off[ii];
     int64_t* dn = done_tick + out_off[ii];
     // instance ii owns samples [traj_off[ii], traj_off[ii+1]) of ema_traj, floor(n/traj_every) of them, 3 doubles each
-    double* traj = (ema_traj && traj_off && sv->traj_every > 0) ? ema_traj + traj_off[ii] * 3 : nullptr;
+    double* traj = (ema_traj && traj_off && sv->traj_every > 0) ? ema_traj + traj_off[ii] * nb : nullptr;
 
     bool skip_to_ingest_now = false;
     for (;;) {
@@ -159,8 +196,8 @@ extern "C" int oracle_simulate(const oracle_traces* tr, const oracle_server* sv,
             s.ema_update(s.tier[r], r);
             ++s.done;
             if (traj && sv->traj_every > 0 && s.done % sv->traj_every == 0) {
-              double* q = traj + (s.done / sv->traj_every - 1) * 3;
-              q[0] = s.B[0]; q[1] = s.B[1]; q[2] = s.B[2];
+              double* q = traj + (s.done / sv->traj_every - 1) * nb;
+              for (int k = 0; k < nb; ++k) q[k] = s.B[k];
             }
           } else ++i;
         }
@@ -197,10 +234,24 @@ extern "C" int oracle_simulate(const oracle_traces* tr, const oracle_server* sv,
       s.kv_used += (int64_t)s.R.size();
       s.now += dt;
     }
-    ema_final[ii * 3 + 0] = s.B[0]; ema_final[ii * 3 + 1] = s.B[1]; ema_final[ii * 3 + 2] = s.B[2];
+    for (int k = 0; k < nb; ++k) ema_final[ii * nb + k] = s.B[k];
     if (est_out) for (int64_t r = 0; r < n; ++r) est_out[out_off[ii] + r] = s.est[r];   // frozen at arrival (A5)
   }
   return 0;
+}
+
+extern "C" int oracle_simulate(const oracle_traces* tr, const oracle_server* sv, const oracle_instance* inst,
+                               int64_t n_inst, const int64_t* out_off, int64_t* start_tick, int64_t* done_tick,
+                               double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out) {
+  return simulate_impl(tr, nullptr, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out);
+}
+
+extern "C" int oracle_simulate_budget(const oracle_traces* tr, const uint8_t* category, const oracle_budget* bp,
+                                      const oracle_server* sv, const oracle_instance* inst, int64_t n_inst, const int64_t* out_off,
+                                      int64_t* start_tick, int64_t* done_tick, double* ema_final, const int64_t* traj_off,
+                                      double* ema_traj, int64_t* est_out) {
+  if (!bp) return -1;
+  return simulate_impl(tr, category, bp, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out);
 }
 
 extern "C" int oracle_latencies(const oracle_traces* tr, const oracle_instance* inst, int64_t n_inst,
@@ -254,6 +305,7 @@ extern "C" int oracle_estimation_error(const oracle_traces* tr, const oracle_ins
     int64_t* o = out + (int64_t)g * 11;
     for (int64_t r = 0; r < n; ++r) {
       int64_t e = est[out_off[ii] + r], P = tr->tokens[lo + r];
+      if (inst[ii].estimator >= 2) P += tr->out_len[lo + r];   // budget estimators predict input + output tokens (Eq. 1)
       int64_t err = e - P;                                  // estimate minus observed length (A3: T_actual = tokens)
       int cls = e <= 128 ? 0 : (e <= 512 ? 1 : 2);          // Eq. 4
       o[0] += 1; o[1] += err < 0 ? -err : err; o[2] += err * err; o[3] += e; o[4] += P;

@@ -38,6 +38,13 @@ typedef struct {
 
 typedef struct { int32_t trace, policy, estimator, _pad; double ema_alpha; } oracle_instance;
 
+/* Budget estimators (estimator 2: T_input = words, 3: T_input = tokens), Eq. 1-2 of the paper in full. */
+typedef struct {
+  double t_base[4];    /* baseline output-token estimate per semantic category short_qa/summary/technical/report */
+  double s_tenant[3];  /* tenant-aware safety scaling per tier */
+  double f_slope, f_max; /* prompt complexity scaling F_input = min(f_max, 1 + f_slope * T_input) */
+} oracle_budget;
+
 /* PAPER.md:35,114 (split() proxy vs tokenizer-aware count); SURVEY.md §8(c) C.1. */
 int oracle_characterize(const uint8_t* bytes, int64_t n_bytes, const int64_t* offsets, int64_t n_prompts,
                         int32_t* words_out, int32_t* tokens_out);
@@ -48,6 +55,13 @@ int oracle_simulate(const oracle_traces* tr, const oracle_server* sv, const orac
                     double* ema_final /*[n_inst*3]*/,
                     const int64_t* traj_off /*nullable; [n_inst+1] sample ranges*/, double* ema_traj /*nullable; [samples][3]*/,
                     int64_t* est_out /*nullable; frozen admission-time estimate per simulated request*/);
+
+/* Same loop with the paper's full estimator (Eq. 1-2, Alg. 1) and per-category feedback (Eq. 5-6 as printed,
+ * PAPER.md:276-286): est = T_input + ceil(((t_base[c]*B[c])*s_tenant[tier])*F_input); on completion
+ * B[c] <- (1-a)*B[c] + a*(out_len / t_base[c]). category: per request, 0..3. ema_final [n_inst*4], ema_traj [samples][4]. */
+int oracle_simulate_budget(const oracle_traces* tr, const uint8_t* category, const oracle_budget* bp, const oracle_server* sv,
+                           const oracle_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t* start_tick,
+                           int64_t* done_tick, double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out);
 
 /* Estimation fidelity (Eq. 3-4 job classes; Tables IV, IX, X): per reporting group, exact integer sums
  * over its simulated requests: out[g*11 + ..] = { n, sum|est-P|, sum(est-P)^2, sum est, sum P, n_short, n_medium, n_long,

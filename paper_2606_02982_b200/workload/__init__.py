@@ -20,6 +20,7 @@ _SRC = os.path.join(_HERE, "gen.cpp")
 
 FIFO, PRIORITY, WEIGHTED, SJF, AGING = 0, 1, 2, 3, 4
 SPLIT, EXACT = 0, 1
+BUDGET_SPLIT, BUDGET_EXACT = 2, 3
 POLICY_NAMES = ["FIFO", "PRIORITY", "WEIGHTED", "SJF", "AGING"]
 
 # layout of ds_instance in include/driftsched.h (24 bytes)
@@ -138,6 +139,31 @@ class Server:
     weight: tuple = (4, 2, 1)
     aging_step: int = 500_000
     traj_every: int = 0
+
+
+@dataclass
+class Budget:
+    """Mirror of ds_budget (include/driftsched.h): parameters of the paper's full estimator, Eq. 1-2.
+    The paper prints none of these constants; the defaults put T_base 25 % above each category's mean synthetic output
+    so that the feedback factor settles near 0.8, the range of Fig. 5."""
+    t_base: tuple = (38.0, 113.0, 189.0, 265.0)     # short_qa, summary, technical, report
+    s_tenant: tuple = (1.0, 1.0, 1.0)
+    f_slope: float = 0.0
+    f_max: float = 1.0
+
+
+CATEGORY_OUT_SCALE = (0.25, 0.75, 1.25, 1.75)       # mean output of a category relative to the trace's output law
+
+
+def assign_categories(seed, out_len, cap=512):
+    """Synthetic semantic categories (the paper's corpus, ~295 prompts per category, is not available):
+    each request gets one of four categories uniformly (seeded), and its decode length is rescaled by the category's
+    factor so that categories differ in output length as in Table I. Returns (category u8, out_len i32)."""
+    rng = np.random.default_rng([int(seed), 0xC47])
+    cat = rng.integers(0, 4, size=out_len.shape[0]).astype(np.uint8)
+    scale = np.asarray(CATEGORY_OUT_SCALE)[cat]
+    o = np.clip(np.rint(out_len.astype(np.float64) * scale), 1, cap).astype(np.int32)
+    return cat, o
 
 
 def mean_interarrival_ticks(rho, tokens, out_len, sv: Server):
