@@ -89,11 +89,13 @@ typedef struct {              /* continuous-batching server model, BASELINE.json
 #define DS_AGING 4    /* PAPER.md:242 */
 #define DS_SPLIT 0    /* estimate base = words  (split() proxy) */
 #define DS_EXACT 1    /* estimate base = tokens (tokenizer-aware) */
+#define DS_BUDGET_SPLIT 2 /* ds_simulate_budget only: full Eq. 1-2 estimator, T_input = words  */
+#define DS_BUDGET_EXACT 3 /* ds_simulate_budget only: full Eq. 1-2 estimator, T_input = tokens */
 
 typedef struct {
   int32_t trace;     /* index into ds_traces */
   int32_t policy;    /* DS_FIFO .. DS_AGING */
-  int32_t estimator; /* DS_SPLIT / DS_EXACT */
+  int32_t estimator; /* DS_SPLIT / DS_EXACT (ds_simulate, ds_simulate_est); DS_BUDGET_* (ds_simulate_budget) */
   int32_t _pad;
   double ema_alpha;  /* EMA learning rate in [0,1] (Eq. 5, PAPER.md:278-286); 0 = BIAS OFF */
 } ds_instance;
@@ -123,12 +125,36 @@ int ds_simulate_est(const ds_traces* tr, const ds_server* sv, const ds_instance*
                     const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace, size_t workspace_bytes,
                     void* stream);
 
+/* The paper's estimator in full (Eq. 1-2 and Alg. 1; semantic categories
+ * short_qa / summary / technical / report; one feedback factor per workload category):
+ *   T_budget = T_input + ceil(((t_base[c] * B[c]) * s_tenant[tier]) * F_input),   F_input = min(f_max, 1 + f_slope * T_input)
+ *   (fp64, the three products and F's multiply-add rounded separately, in that order), T_input = words (DS_BUDGET_SPLIT)
+ *   or tokens (DS_BUDGET_EXACT), c = category[r]; frozen at arrival; used as the SJF key, by KV admission and as est_out.
+ * Feedback on completion of r (Eq. 5-6 as printed: T_actual = observed output length, T_base = the
+ * category baseline): if ema_alpha > 0 and t_base[c] > 0:  B[c] <- (1-a)*B[c] + a*(out_len[r] / t_base[c]), B[] = 1.0 initially.
+ * Everything else (queues, policies, server model, same-tick ordering) is ds_simulate's. The paper prints none of the
+ * constants; they are parameters (DESIGN.md §4 B1-B4).
+ * category [same indexing as tr->tier] uint8 device, values 0..3 (larger: DS_DEV_BAD_TRACE); bp: HOST struct, t_base >= 0,
+ * s_tenant > 0, f_slope >= 0, f_max >= 1 (DS_EINVAL otherwise); every instance must use DS_BUDGET_SPLIT or DS_BUDGET_EXACT
+ * (DS_DEV_BAD_INSTANCE otherwise). ema_final [n_inst*4], ema_traj [samples][4] (one factor per category). est_out nullable. */
+typedef struct {
+  double t_base[4];   /* baseline output-token estimate per semantic category */
+  double s_tenant[3]; /* tenant-aware safety scaling per tier */
+  double f_slope;     /* prompt complexity scaling: F_input = min(f_max, 1 + f_slope * T_input) */
+  double f_max;
+} ds_budget;
+int ds_simulate_budget(const ds_traces* tr, const uint8_t* category, const ds_budget* bp, const ds_server* sv,
+                       const ds_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t* start_tick, int64_t* done_tick,
+                       double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace,
+                       size_t workspace_bytes, void* stream);
+
 /* Estimation fidelity: job classes of Eq. 3-4 (short est<=128, medium
  * est<=512, long otherwise), token-estimation error (Tables IV, X) and queue wait by job class
  * (Table IX), per reporting group g = group[instance] (nullable -> 0) in [0, n_groups).
  * out [n_groups*11] int64 device, exact integer sums over the group's simulated requests:
  *   { n, sum|est-P|, sum(est-P)^2, sum est, sum P, n_short, n_medium, n_long, sum qdelay_short, _medium, _long }
- *   with P = tokens (the observed length, reading A3) and qdelay = start_tick - arrival (0 if start_tick is NULL).
+ *   with P = tokens (the observed length, reading A3; tokens + out_len for the DS_BUDGET_* estimators, which predict
+ *   input + output tokens, Eq. 1) and qdelay = start_tick - arrival (0 if start_tick is NULL).
  *   MAE = out[1]/out[0], RMSE = sqrt(out[2]/out[0]), mean bias = out[4]/out[3] are left to the caller (fp64).
  * class_seg (nullable) [out_off[n_inst]] int32 device: 3*g + class, usable as seg_id for ds_tail_stats.
  * A group outside [0, n_groups) sets DS_DEV_BAD_INSTANCE. Launches: 1 memset + 1 kernel. */

@@ -10,7 +10,7 @@ LIB_PATH = os.path.join(_HERE, "libdriftsched.so")
 DS_OK, DS_EINVAL, DS_ECUDA, DS_ENOMEM = 0, -1, -2, -3
 WS_CHARACTERIZE, WS_SIMULATE, WS_TAIL_STATS = 0, 1, 2
 
-EXPORTS = ["ds_characterize", "ds_simulate", "ds_simulate_est", "ds_estimation_error", "ds_queue_depth", "ds_latencies", "ds_tail_stats",
+EXPORTS = ["ds_characterize", "ds_simulate", "ds_simulate_est", "ds_simulate_budget", "ds_estimation_error", "ds_queue_depth", "ds_latencies", "ds_tail_stats",
            "ds_latency_stats", "ds_workspace_bytes", "ds_device_status",
            "ds_strerror", "ds_last_cuda_error", "ds_launch_count"]
 
@@ -24,6 +24,10 @@ class DsServer(C.Structure):
     _fields_ = [("max_batch", C.c_int32), ("kv_budget", C.c_int64), ("c_base", C.c_int64), ("c_batch", C.c_int64),
                 ("c_ctx", C.c_int64), ("c_prefill", C.c_int64), ("weight", C.c_int32 * 3), ("aging_step", C.c_int64),
                 ("traj_every", C.c_int32)]
+
+
+class DsBudget(C.Structure):
+    _fields_ = [("t_base", C.c_double * 4), ("s_tenant", C.c_double * 3), ("f_slope", C.c_double), ("f_max", C.c_double)]
 
 
 class DsError(RuntimeError):
@@ -47,6 +51,7 @@ def lib():
         L.ds_characterize.argtypes = [p, i64, p, i64, p, p, p, sz, p]
         L.ds_simulate.argtypes = [C.POINTER(DsTraces), C.POINTER(DsServer), p, i64, p, p, p, p, p, p, p, sz, p]
         L.ds_simulate_est.argtypes = [C.POINTER(DsTraces), C.POINTER(DsServer), p, i64, p, p, p, p, p, p, p, p, sz, p]
+        L.ds_simulate_budget.argtypes = [C.POINTER(DsTraces), p, C.POINTER(DsBudget), C.POINTER(DsServer), p, i64, p, p, p, p, p, p, p, p, sz, p]
         L.ds_estimation_error.argtypes = [C.POINTER(DsTraces), p, i64, p, p, p, p, i32, p, p, p]
         L.ds_queue_depth.argtypes = [C.POINTER(DsTraces), p, i64, p, p, i64, i64, i64, p, p]
         L.ds_latencies.argtypes = [C.POINTER(DsTraces), p, i64, p, i64, p, p, p, p, p, p, p, p, p]
@@ -59,7 +64,7 @@ def lib():
         L.ds_strerror.restype = C.c_char_p
         L.ds_last_cuda_error.restype = C.c_char_p
         L.ds_launch_count.restype = i64
-        for f in ("ds_characterize", "ds_simulate", "ds_simulate_est", "ds_estimation_error", "ds_queue_depth", "ds_latencies", "ds_tail_stats", "ds_latency_stats", "ds_device_status"):
+        for f in ("ds_characterize", "ds_simulate", "ds_simulate_est", "ds_simulate_budget", "ds_estimation_error", "ds_queue_depth", "ds_latencies", "ds_tail_stats", "ds_latency_stats", "ds_device_status"):
             getattr(L, f).restype = C.c_int
         _lib = L
     return _lib

@@ -7,7 +7,7 @@ import numpy as np
 import torch
 
 from . import _lib
-from ._lib import DsServer, DsTraces, check, lib
+from ._lib import DsBudget, DsServer, DsTraces, check, lib
 
 INSTANCE_BYTES = 24
 
@@ -210,3 +210,28 @@ def queue_depth(trace_off, arrival, tier, words, tokens, out_len, inst, out_off,
     check("ds_queue_depth", lib().ds_queue_depth(C.byref(tr), _ptr(inst), n_inst, _ptr(out_off), _ptr(start), int(t0), int(dt),
                                                  int(n_samples), _ptr(out), _stream()))
     return out
+
+
+def simulate_budget(trace_off, arrival, tier, words, tokens, out_len, category, budget, server, inst, out_off, n_total,
+                    start=None, done=None, ema_final=None, traj_off=None, ema_traj=None, est_out=None, workspace=None):
+    """ds_simulate_budget. category uint8 CUDA tensor (per request); budget: object with t_base[4], s_tenant[3], f_slope,
+    f_max. Returns (start_tick, done_tick, ema_final[n_inst,4])."""
+    tr = _traces(trace_off, arrival, tier, words, tokens, out_len)
+    sv = _server(server)
+    bp = DsBudget((C.c_double * 4)(*budget.t_base), (C.c_double * 3)(*budget.s_tenant), budget.f_slope, budget.f_max)
+    _need_cuda(category, inst, out_off, start, done, ema_final, traj_off, ema_traj, est_out)
+    assert category.dtype == torch.uint8 and category.numel() == tier.numel()
+    n_inst = inst.numel() // INSTANCE_BYTES
+    dev = arrival.device
+    if start is None:
+        start = torch.empty(n_total, dtype=torch.int64, device=dev)
+    if done is None:
+        done = torch.empty(n_total, dtype=torch.int64, device=dev)
+    if ema_final is None:
+        ema_final = torch.empty((n_inst, 4), dtype=torch.float64, device=dev)
+    if workspace is None:
+        workspace = _workspace(_lib.WS_SIMULATE, n_total, n_inst, dev)
+    check("ds_simulate_budget", lib().ds_simulate_budget(C.byref(tr), _ptr(category), C.byref(bp), C.byref(sv), _ptr(inst), n_inst,
+                                                         _ptr(out_off), _ptr(start), _ptr(done), _ptr(ema_final), _ptr(traj_off),
+                                                         _ptr(ema_traj), _ptr(est_out), _ptr(workspace), workspace.numel(), _stream()))
+    return start, done, ema_final

@@ -43,6 +43,7 @@ struct Params {
   int32_t traj_every;
   const ds_instance* inst; int64_t n_inst; const int64_t* out_off; int64_t* start_tick; int64_t* done_tick;
   double* ema_final; const int64_t* traj_off; double* ema_traj; int64_t* est_out;
+  const uint8_t* category; ds_budget bp;   // budget estimators only (ds_simulate_budget)
   unsigned long long* heap_ws; unsigned int* counter; unsigned int* status; const unsigned int* perm;
 };
 
@@ -111,7 +112,9 @@ struct TierCursor {
 
 // kSmall: every per-iteration quantity of this trace (kv_used, dt, prefill) is proven < 2^31 and out_len <= 65535 by
 // trace_is_small(), so they are kept in 32-bit registers and the closed-form jump is two IMAD.WIDE; `now` stays 64-bit.
-template <int kSlots, int kPolicy, bool kSmall>
+// kBudget: the paper's full estimator (Eq. 1-2) with one feedback factor per semantic category (lanes 0..3) instead of
+// the reduced per-tier one (lanes 0..2); a separate instantiation so that the benchmarked path is not touched.
+template <int kSlots, int kPolicy, bool kSmall, bool kBudget>
 __device__ __forceinline__ void run_instance(const Params& p, const unsigned inst_id, const int trace, const bool split, const double alpha,
                                           unsigned long long* heap_sm, const int lane) {
   constexpr bool kCursor = kPolicy == DS_PRIORITY || kPolicy == DS_WEIGHTED || kPolicy == DS_AGING;
@@ -136,8 +139,10 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   const bool need_est = use_kv || kPolicy == DS_SJF || est_o != nullptr;
   // EXACT estimator: m = P/P = 1.0, and (1-a)*1 + a*1 rounds to exactly 1.0 for every a in [0,1] (DESIGN.md §4 A4),
   // so B stays 1.0 and est = base: no fp64 work at all on that path.
-  const bool ema_on = split && alpha > 0.0;
-  double* traj = (p.ema_traj && p.traj_off && p.traj_every > 0) ? p.ema_traj + 3 * p.traj_off[inst_id] : nullptr;
+  const bool ema_on = (kBudget || split) && alpha > 0.0;
+  constexpr int kFac = kBudget ? 4 : 3;           // feedback factors per instance
+  const uint8_t* __restrict__ cat = kBudget ? p.category + lo : nullptr;
+  double* traj = (p.ema_traj && p.traj_off && p.traj_every > 0) ? p.ema_traj + kFac * p.traj_off[inst_id] : nullptr;
   const int max_batch = p.max_batch;
 
   // ---- state (warp-uniform unless noted) ----
@@ -157,10 +162,14 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   const int wtot = p.w0 + p.w1 + p.w2;
 
   // arrival window: lane holds request wb+lane
-  int wb = 0; long long w_arr = kInf; int w_tier = 0, w_base = 0;
+  int wb = 0; long long w_arr = kInf; int w_tier = 0, w_base = 0, w_cat = 0;
   auto load_window = [&]() {
     const int i = wb + lane;
     if (i < n) { w_arr = arr[i]; w_tier = tier[i]; w_base = BASE[i]; } else { w_arr = kInf; w_tier = 0; w_base = 0; }
+    if (kBudget) {
+      w_cat = i < n ? (int)cat[i] : 0;
+      if (w_cat > 3) { atomicOr(p.status, DS_DEV_BAD_TRACE); w_cat = 3; }
+    }
     const long long prev = __shfl_up_sync(kFull, w_arr, 1);
     const bool bad = (i < n) && (w_tier > 2 || w_base < 0 || w_arr < 0 || (lane > 0 && w_arr < prev));
     if (bad) atomicOr(p.status, DS_DEV_BAD_TRACE);
@@ -199,7 +208,18 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       if (m == 0) break;
       const int c = __popc(m);
       long long est = 0;
-      if (need_est) {
+      if (kBudget) {
+        if (need_est) {                                       // Eq. 1-2 in full, frozen at arrival (A5)
+          const double tb = w_cat == 0 ? p.bp.t_base[0] : w_cat == 1 ? p.bp.t_base[1] : w_cat == 2 ? p.bp.t_base[2] : p.bp.t_base[3];
+          const double sc = w_tier == 0 ? p.bp.s_tenant[0] : w_tier == 1 ? p.bp.s_tenant[1] : p.bp.s_tenant[2];
+          double F = __dadd_rn(1.0, __dmul_rn(p.bp.f_slope, (double)w_base));
+          if (F > p.bp.f_max) F = p.bp.f_max;
+          double x = __dmul_rn(tb, shfl_f64(Bl, w_cat));
+          x = __dmul_rn(x, sc);
+          x = __dmul_rn(x, F);
+          est = (long long)w_base + (long long)ceil(x);
+        }
+      } else if (need_est) {
         if (ema_on) {                                         // Eq. 1-2 reduced (A1), frozen at arrival (A5)
           const double Bt = shfl_f64(Bl, w_tier);
           if (w_base > 0) est = (long long)ceil(__dmul_rn(Bt, (double)w_base));
@@ -252,7 +272,20 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       dn[r] = now;                                            // every lane, same address and value: one store, no branch
       kv_used -= (acc_t)Pr + (acc_t)Or;
       --b;
-      if (ema_on) {                                           // Eq. 5-6 (A3): four separately rounded operations
+      if (kBudget) {
+        if (ema_on) {                                         // Eq. 5-6 as printed: T_actual = observed output length, per category
+          const int cr = min((int)cat[r], 3);
+          const double tb = cr == 0 ? p.bp.t_base[0] : cr == 1 ? p.bp.t_base[1] : cr == 2 ? p.bp.t_base[2] : p.bp.t_base[3];
+          if (tb > 0.0) {
+            const double m = __ddiv_rn((double)Or, tb);
+            const double t1 = __dsub_rn(1.0, alpha);
+            const double t2 = __dmul_rn(t1, shfl_f64(Bl, cr));
+            const double t3 = __dmul_rn(alpha, m);
+            const double Bn = __dadd_rn(t2, t3);
+            if (lane == cr) Bl = Bn;
+          }
+        }
+      } else if (ema_on) {                                    // Eq. 5-6 (A3): four separately rounded operations
         const int br = W[r], tr = min((int)tier[r], 2);
         if (br > 0) {
           const double m = __ddiv_rn((double)Pr, (double)br);
@@ -264,7 +297,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
         }
       }
       ++done;
-      if (traj && done % p.traj_every == 0 && lane < 3) traj[3 * (done / p.traj_every - 1) + lane] = Bl;
+      if (traj && done % p.traj_every == 0 && lane < kFac) traj[kFac * (done / p.traj_every - 1) + lane] = Bl;
     }
     blocked = false;
     unsigned d = 0xffffffffu;
@@ -402,7 +435,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       }
     }
   }
-  if (lane < 3) p.ema_final[3 * (size_t)inst_id + lane] = Bl;
+  if (lane < kFac) p.ema_final[kFac * (size_t)inst_id + lane] = Bl;
   __syncwarp();
 }
 
@@ -466,8 +499,9 @@ __global__ void __launch_bounds__(1024) order_kernel(const ds_instance* __restri
   }
 }
 
-template <int kSlots>
+template <int kSlots, bool kBudget = false>
 __global__ void __launch_bounds__(k2::kWarpsPerBlock * 32) simulate_kernel(const __grid_constant__ Params p) {
+  constexpr int kFac = kBudget ? 4 : 3;
   __shared__ unsigned long long heap_sm[kWarpsPerBlock][kHeapSmem];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   // Policy affinity per SM: every warp of an SM starts on the same bucket and, when it is empty, moves to the bucket
@@ -498,19 +532,20 @@ __global__ void __launch_bounds__(k2::kWarpsPerBlock * 32) simulate_kernel(const
     }
     const unsigned inst_id = p.perm[b0 + k];
     const ds_instance in = p.inst[inst_id];
-    const bool bad_inst = in.trace < 0 || in.trace >= p.n_traces || in.policy < 0 || in.policy > 4 || in.estimator < 0 ||
-                          in.estimator > 1 || !(in.ema_alpha >= 0.0 && in.ema_alpha <= 1.0);
+    const int est_lo = kBudget ? DS_BUDGET_SPLIT : DS_SPLIT;          // this kernel's pair of estimators
+    const bool bad_inst = in.trace < 0 || in.trace >= p.n_traces || in.policy < 0 || in.policy > 4 || in.estimator < est_lo ||
+                          in.estimator > est_lo + 1 || !(in.ema_alpha >= 0.0 && in.ema_alpha <= 1.0);
     if (bad_inst) {
       if (lane == 0) atomicOr(p.status, DS_DEV_BAD_INSTANCE);
-      if (lane < 3) p.ema_final[3 * (size_t)inst_id + lane] = 1.0;
+      if (lane < kFac) p.ema_final[kFac * (size_t)inst_id + lane] = 1.0;
       continue;
     }
-    const bool split = in.estimator == DS_SPLIT;
-    if (lane < 3) p.ema_final[3 * (size_t)inst_id + lane] = 1.0;   // overwritten unless the trace is rejected
+    const bool split = in.estimator == est_lo;                         // T_input = words (else tokens)
+    if (lane < kFac) p.ema_final[kFac * (size_t)inst_id + lane] = 1.0;   // overwritten unless the trace is rejected
     const bool small = trace_is_small(p, in.trace, lane);
 #define DS_RUN(POL)                                                                                             \
-  if (small) run_instance<kSlots, POL, true>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane);    \
-  else run_instance<kSlots, POL, false>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane)
+  if (small) run_instance<kSlots, POL, true, kBudget>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane);    \
+  else run_instance<kSlots, POL, false, kBudget>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane)
     switch (in.policy) {
       case DS_FIFO: DS_RUN(DS_FIFO); break;
       case DS_PRIORITY: DS_RUN(DS_PRIORITY); break;
@@ -530,7 +565,7 @@ size_t ws_simulate(int64_t total_requests, int64_t n_inst) {
 }
 
 }  // namespace ds
-static int simulate_impl(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
+static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_budget* bp, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
                          const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
                          const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace, size_t workspace_bytes,
                          void* stream) {
@@ -544,6 +579,12 @@ static int simulate_impl(const ds_traces* tr, const ds_server* sv, const ds_inst
   if (sv->c_base < 0 || sv->c_batch < 0 || sv->c_ctx < 0 || sv->c_prefill < 0) return DS_EINVAL;
   if (sv->c_base > 0x7fffffff || sv->c_batch > 0x7fffffff || sv->c_ctx > 0x7fffffff || sv->c_prefill > 0x7fffffff) return DS_EINVAL;
   if (n_inst > 0x7fffffff) return DS_EINVAL;
+  if (bp) {
+    if (!category) return DS_EINVAL;
+    for (int c = 0; c < 4; ++c) if (!(bp->t_base[c] >= 0.0)) return DS_EINVAL;
+    for (int t = 0; t < 3; ++t) if (!(bp->s_tenant[t] > 0.0)) return DS_EINVAL;
+    if (!(bp->f_slope >= 0.0) || !(bp->f_max >= 1.0)) return DS_EINVAL;
+  }
   if (workspace_bytes < 256 + perm_bytes(n_inst)) return DS_ENOMEM;
   cudaStream_t s = (cudaStream_t)stream;
   k2::Params p;
@@ -554,6 +595,8 @@ static int simulate_impl(const ds_traces* tr, const ds_server* sv, const ds_inst
   p.traj_every = sv->traj_every;
   p.inst = inst; p.n_inst = n_inst; p.out_off = out_off; p.start_tick = start_tick; p.done_tick = done_tick;
   p.ema_final = ema_final; p.traj_off = traj_off; p.ema_traj = ema_traj; p.est_out = est_out;
+  p.category = category;
+  if (bp) p.bp = *bp; else memset(&p.bp, 0, sizeof(p.bp));
   p.counter = (unsigned int*)workspace;
   unsigned int* perm = (unsigned int*)((char*)workspace + 256);
   p.perm = perm;
@@ -578,6 +621,12 @@ static int simulate_impl(const ds_traces* tr, const ds_server* sv, const ds_inst
     DS_CUDA(cudaGetLastError());
     return DS_OK;
   };
+  if (bp) {
+    if (sv->max_batch <= 32) return launch(k2::simulate_kernel<1, true>);
+    if (sv->max_batch <= 64) return launch(k2::simulate_kernel<2, true>);
+    if (sv->max_batch <= 128) return launch(k2::simulate_kernel<4, true>);
+    return launch(k2::simulate_kernel<8, true>);
+  }
   if (sv->max_batch <= 32) return launch(k2::simulate_kernel<1>);
   if (sv->max_batch <= 64) return launch(k2::simulate_kernel<2>);
   if (sv->max_batch <= 128) return launch(k2::simulate_kernel<4>);
@@ -587,7 +636,7 @@ static int simulate_impl(const ds_traces* tr, const ds_server* sv, const ds_inst
 extern "C" int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
                            const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
                            const int64_t* traj_off, double* ema_traj, void* workspace, size_t workspace_bytes, void* stream) {
-  return simulate_impl(tr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, nullptr, workspace,
+  return simulate_impl(tr, nullptr, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, nullptr, workspace,
                        workspace_bytes, stream);
 }
 
@@ -596,6 +645,15 @@ extern "C" int ds_simulate_est(const ds_traces* tr, const ds_server* sv, const d
                                const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace,
                                size_t workspace_bytes, void* stream) {
   if (n_inst > 0 && !est_out) return DS_EINVAL;
-  return simulate_impl(tr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out, workspace,
+  return simulate_impl(tr, nullptr, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out, workspace,
                        workspace_bytes, stream);
+}
+
+extern "C" int ds_simulate_budget(const ds_traces* tr, const uint8_t* category, const ds_budget* bp, const ds_server* sv,
+                                  const ds_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t* start_tick,
+                                  int64_t* done_tick, double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out,
+                                  void* workspace, size_t workspace_bytes, void* stream) {
+  if (!bp) return DS_EINVAL;
+  return simulate_impl(tr, category, bp, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out,
+                       workspace, workspace_bytes, stream);
 }
