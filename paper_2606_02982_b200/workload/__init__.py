@@ -261,6 +261,33 @@ def _trace_workload(name, seed, n_traces, n_req, sv, combos, characterize, *, rh
                     {"post_drift": post, "combos": combos})
 
 
+def paper_phases(characterize, n_runs=3, seed=7, n_cal=1000, n_stress=2000, rho_cal=0.5, rho_stress=1.3):
+    """The paper's experiment shape: per run 1000 calibration requests followed by 2000 stress
+    requests, batch 32, feedback on throughout, three runs; Weighted 50/30/20 = weight {5,3,2}; the three
+    estimator modes of Table IX (split() OFF, split() ON, tokenizer-aware ON) for all five policies, with the full
+    estimator of Eq. 1-2 over four synthetic semantic categories. The paper's arrivals are closed-loop (50 clients);
+    here they stay an open-loop input (reading A12): the calibration phase arrives at offered load rho_cal, the stress
+    phase at rho_stress. t_mid[run] = arrival of the first stress request, so ds_latencies' phases = calibration/stress.
+    Returns (Workload, category u8, Budget); Workload.out_len already carries the per-category output scaling."""
+    n_req = n_cal + n_stress
+    sv = Server(max_batch=32, kv_budget=16384, weight=(5, 3, 2), aging_step=500_000, traj_every=100)
+    combos = [(p, e, a) for p in ALL_POLICIES for e, a in ((BUDGET_SPLIT, 0.0), (BUDGET_SPLIT, 0.1), (BUDGET_EXACT, 0.1))]
+    c = _trace_workload("paper_phases", seed, n_runs, n_req, sv, combos, characterize, rho=1.0)
+    cat, out_len = assign_categories(seed, c.out_len)
+    _, _, expo = make_requests(seed, n_runs, n_req, 0)
+    arrival = np.empty(n_runs * n_req, np.int64)
+    t_mid = np.empty(n_runs, np.int64)
+    for t in range(n_runs):
+        sl = slice(t * n_req, (t + 1) * n_req)
+        s_bar = mean_interarrival_ticks(1.0, c.tokens[sl], out_len[sl], sv)
+        mean = np.concatenate([np.full(n_cal, s_bar / rho_cal), np.full(n_stress, s_bar / rho_stress)])
+        ia = np.maximum(0, np.rint(expo[sl] * mean)).astype(np.int64)
+        arrival[sl] = np.cumsum(ia)
+        t_mid[t] = arrival[t * n_req + n_cal]
+    c.arrival, c.out_len, c.t_mid = arrival, out_len, t_mid
+    return c, cat, Budget()
+
+
 def config0(characterize):
     """configs[0]: 1 trace, 200 requests, seed 0, 2 req/s, batch 8, KV unlimited, FIFO+SJF, split()+EMA 0.1."""
     sv = Server(max_batch=8, kv_budget=0)
