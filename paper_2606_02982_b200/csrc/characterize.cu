@@ -151,6 +151,11 @@ __device__ __forceinline__ void classify32(uint32_t (&w)[8], const Mul& mu, uint
   letter = ~nonletter;
 }
 
+__device__ __forceinline__ unsigned bfind(uint32_t x) {              // index of the most significant 1 bit, 0xffffffff for 0
+  unsigned r;
+  asm("bfind.u32 %0, %1;" : "=r"(r) : "r"(x));
+  return r;
+}
 __device__ __forceinline__ bool is_ws_scalar(uint32_t c) { return (c - 9u) <= 4u || c == 32u; }
 __device__ __forceinline__ bool is_letter_scalar(uint32_t c) {
   bool punct = (c - 0x21u) <= 0x0Eu || (c - 0x3Au) <= 6u || (c - 0x5Bu) <= 5u || (c - 0x7Bu) <= 3u;
@@ -284,15 +289,21 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
 
   // boundary window: lane holds off[kb + lane] as a 32-bit position relative to pos0 (kNoRel: none / beyond 4 GiB)
   unsigned orel = kNoRel;
+  // per-lane cursors instead of 64-bit index arithmetic in the loop: this lane's entry of offsets[], how many entries are
+  // left from it (<= 0: none), and the output slots of the prompt its boundary closes (boundary k closes prompt k-1)
+  const int64_t* optr = off + kb + lane;
+  long long left = nb_total - kb - lane;
+  int32_t* wp = words + kb + lane - 1;
+  int32_t* tp = tokens + kb + lane - 1;
+  bool at_first = kb == 0;            // the window starts with boundary 0, which closes no prompt
   auto load_window = [&]() {
-    const long long idx = kb + lane;
-    const bool have = idx < nb_total;
-    const long long o = have ? off[idx] : kInfOff;
-    const long long d = o - pos0;
-    orel = (d < 0 || d >= (long long)kNoRel) ? kNoRel : (unsigned)d;
+    const bool have = left > 0;
+    const long long o = have ? *optr : kInfOff;
+    const unsigned long long d = (unsigned long long)(o - pos0);
+    orel = d >= (unsigned long long)kNoRel ? kNoRel : (unsigned)d;   // negative differences wrap to huge values
     unsigned prev = __shfl_up_sync(kFull, orel, 1);
     if (lane == 0) prev = last_rel;
-    if (have && (o < 0 || o > n_bytes || d < 0 || orel < prev)) atomicOr(status, DS_DEV_BAD_OFFSETS);
+    if (have && ((unsigned long long)o > (unsigned long long)n_bytes || o < pos0 || orel < prev)) atomicOr(status, DS_DEV_BAD_OFFSETS);
   };
   load_window();
 
@@ -300,6 +311,7 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
   const uint8_t* lrow = &stage[0][0] + lane * kSeg;
   const unsigned lx = (unsigned)(lane & 7) << 4;
   const int lane_prev = (lane + 31) & 31;
+  const unsigned lanemask_lt = (1u << lane) - 1u;
   unsigned scan_on[5];                  // 1 if lane >= 2^k: this lane takes the scan's k-th partial sum
 #pragma unroll
   for (int k = 0; k < 5; ++k) {         // (asm volatile: keep them in registers instead of recomputing ISETP+SEL per chunk)
@@ -313,9 +325,7 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
   const bool head_edge = pos0 < 0;
   int s = 0;
   unsigned parity = 0, crel = 0;      // stage index, its mbarrier phase, chunk start relative to pos0
-  long long cs = pos0;
-  for (unsigned it = 0; it < n_it; ++it, cs += kChunk, crel += kChunk) {
-    const long long ce = cs + kChunk;   // chunk = positions [cs,ce) relative to bytes
+  for (unsigned it = 0; it < n_it; ++it, crel += kChunk) {   // chunk = positions [pos0 + crel, +kChunk) relative to bytes
     const bool by_tma = it < it_tma;
 
     // (a) the lane's 128 bytes -> WS / LETTER masks, 32 bytes at a time
@@ -347,7 +357,7 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
     if ((head_edge && it == 0) || it >= it_tail) {   // cs < 0 or ce > n_bytes: bytes outside [0,n_bytes) count as whitespace
 #pragma unroll
       for (int g = 0; g < NW; ++g) {
-        const long long sp = cs + (long long)lane * kSeg + 32 * g;
+        const long long sp = pos0 + crel + (long long)lane * kSeg + 32 * g;
         long long lo = -sp, hi = n_bytes - sp;
         lo = lo < 0 ? 0 : (lo > 32 ? 32 : lo);
         hi = hi < 0 ? 0 : (hi > 32 ? 32 : hi);
@@ -363,9 +373,12 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
     unsigned bm = __ballot_sync(kFull, inb);
     if (inb) atomicOr(&sb[rel >> 5], 1u << (rel & 31));
     if (bm == kFull) {                                   // rare: more than 32 boundaries may fall into one chunk
-      for (long long kk = kb + 32; kk < nb_total; kk += 32) {
-        const long long idx = kk + lane;
-        const long long o2 = idx < nb_total ? off[idx] : kInfOff;
+      const long long cs = pos0 + crel, ce = cs + kChunk;
+      const int64_t* o2p = optr;
+      for (long long l2 = left - 32; ; l2 -= 32) {
+        o2p += 32;
+        if (__ballot_sync(kFull, l2 > 0) == 0u) break;
+        const long long o2 = l2 > 0 ? *o2p : kInfOff;
         const bool in2 = o2 >= cs && o2 < ce;
         if (in2) atomicOr(&sb[(int)(o2 - cs) >> 5], 1u << ((int)(o2 - cs) & 31));
         if (__ballot_sync(kFull, in2) != kFull) break;
@@ -390,21 +403,23 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
 #pragma unroll
     for (int g = 0; g < NW; ++g) { C[g] = L[g] & pl[g] & ~S[g]; call &= C[g]; }
     const bool has_break = call != ~0u;
-    unsigned cnt_out = 0;
-    if (has_break) {
-      // highest byte that does not continue its predecessor's run: the trailing run starts there (if a letter) or after it
-      int g = NW - 1;
-      uint32_t ct = C[g];
-      while (ct == ~0u) { --g; ct = g == 2 ? C[2] : g == 1 ? C[1] : C[0]; }
-      const uint32_t lt = g == 3 ? L[3] : g == 2 ? L[2] : g == 1 ? L[1] : L[0];
-      const int k = __clz((int)~ct);                                 // trailing continuation bytes (mod 32)
-      cnt_out = (unsigned)(k + (int)((lt >> (31 - k)) & 1u)) & 3u;    // lower words add multiples of 32 = 0 (mod 4)
+    // highest byte that does not continue its predecessor's run: the trailing run starts there (if a letter) or after it.
+    // Common case: it lies in the top word. kz = number of trailing continuation bytes (mod 32; lower words add
+    // multiples of 32 = 0 mod 4), the byte below them is bit 31-kz.
+    uint32_t ct = C[NW - 1], lt = L[NW - 1];
+    if (ct == ~0u && has_break) {                                    // rare: >= 32 trailing letters
+      ct = C[2]; lt = L[2];
+      if (ct == ~0u) { ct = C[1]; lt = L[1]; }
+      if (ct == ~0u) { ct = C[0]; lt = L[0]; }
     }
+    const unsigned hz = bfind(~ct);                                  // position of the highest 0 bit of ct
+    const unsigned cnt_out = ((31u - hz) + ((lt >> (hz & 31u)) & 1u)) & 3u;   // garbage if !has_break: never read then
     const unsigned brk_mask = __ballot_sync(kFull, has_break);
-    const unsigned below = brk_mask & ((1u << lane) - 1u);
-    const unsigned from_lane = __shfl_sync(kFull, cnt_out, below ? 31 - __clz(below) : 0);
+    const unsigned below = brk_mask & lanemask_lt;
+    const unsigned from_lane = __shfl_sync(kFull, cnt_out, bfind(below));      // bfind(0) = -1 -> lane 31, unused
     const unsigned cnt_in = below ? from_lane : c_cnt;
-    if (brk_mask) c_cnt = __shfl_sync(kFull, cnt_out, 31 - __clz(brk_mask));   // else unchanged: 4096 = 0 (mod 4)
+    const unsigned last_cnt = __shfl_sync(kFull, cnt_out, bfind(brk_mask));
+    c_cnt = brk_mask ? last_cnt : c_cnt;                             // no break in the chunk: unchanged, 4096 = 0 (mod 4)
 
     // (d) flags and their counts per 32-byte word, packed words | tokens << 16
     uint32_t fw[NW], ft[NW], cpk[NW];
@@ -443,20 +458,19 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
         if (lane == 0) prev = base_c;
         const unsigned dlt = cj - prev;                               // both fields are non-decreasing: no borrow
         unsigned nwd = dlt & 0xffffu, ntk = dlt >> 16;
-        const long long p = kb + lane - 1;                            // prompt closed by this lane's boundary
         if (lane == 0) { nwd += accW; ntk += accT; }
-        if (inb && p >= 0) {
+        if (inb && !(at_first && lane == 0)) {                        // *wp / *tp: the prompt closed by this lane's boundary
           if (lane == 0 && open_before_span) {
-            if (nwd) atomicAdd(words + p, (int)nwd);
-            if (ntk) atomicAdd(tokens + p, (int)ntk);
+            if (nwd) atomicAdd(wp, (int)nwd);
+            if (ntk) atomicAdd(tp, (int)ntk);
           } else {
-            words[p] = (int)nwd; tokens[p] = (int)ntk;
+            *wp = (int)nwd; *tp = (int)ntk;
           }
         }
-        accW = 0; accT = 0; open_before_span = false;
+        accW = 0; accT = 0; open_before_span = false; at_first = false;
         base_c = __shfl_sync(kFull, cj, nb - 1);
         last_rel = __shfl_sync(kFull, orel, nb - 1);
-        kb += nb;
+        optr += nb; left -= nb; wp += nb; tp += nb;
         load_window();
         if (nb < 32) break;
         rel = orel - crel;
@@ -478,9 +492,9 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
   }
 
   // the prompt still open at the span's end continues in the next warp's span
-  if (lane == 0 && kb >= 1 && kb <= n_prompts) {
-    if (accW) atomicAdd(words + (kb - 1), (int)accW);
-    if (accT) atomicAdd(tokens + (kb - 1), (int)accT);
+  if (lane == 0 && !at_first && left > 0) {             // lane 0: next boundary kb with 1 <= kb <= n_prompts; wp = words + kb - 1
+    if (accW) atomicAdd(wp, (int)accW);
+    if (accT) atomicAdd(tp, (int)accT);
   }
 }
 
