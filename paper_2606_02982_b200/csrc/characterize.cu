@@ -141,14 +141,26 @@ __device__ __forceinline__ void classify32(uint32_t (&w)[8], const Mul& mu, uint
   for (int i = 0; i < 8; i += 2) exchange<0x0f0f0f0fu>(w[i], w[i + 1], mu.l4, mu.r4); // a2 <-> position bit 2
   // register r now holds bit plane k with k2 = r&1, k1 = (r>>2)&1, k0 = (r>>1)&1
   const uint32_t b0 = w[0], b4 = w[1], b1 = w[2], b5 = w[3], b2 = w[4], b6 = w[5], b3 = w[6], b7 = w[7];
-  const uint32_t u9_13 = b3 & ((~b2 & (b1 | b0)) | (b2 & ~b1));                        // low nibble in 9..13
-  const uint32_t z0 = ~(b3 | b2 | b1 | b0);                                           // low nibble == 0
-  const uint32_t ge10 = b3 & (b2 | b1), ge11 = b3 & (b2 | (b1 & b0));
-  const uint32_t u11_14 = b3 & ((~b2 & b1 & b0) | (b2 & ~(b1 & b0)));                  // low nibble in 11..14
-  const uint32_t nonletter = ~b7 & ((~b6 & ~b5 & ~b4 & u9_13) | (~b6 & b5 & ~b4) | (~b6 & b5 & b4 & ge10) | (b6 & ~b4 & z0) |
-                                    (b6 & ~b5 & b4 & ge11) | (b6 & b5 & b4 & u11_14));
-  ws = ~b7 & ~b6 & ~b4 & ((~b5 & u9_13) | (b5 & z0));
-  letter = ~nonletter;
+  // Boolean network, written so that every line is one 3-input function (one LOP3): with m = (b2 b1 b0) the low nibble
+  // is (b3, m), and per row r = (b6 b5 b4) the non-LETTER set is  b3 ? G_r(m) : H_r(m):
+  //   r=0: G = m in 1..5 (9..13)   r=2: all 16          r=3: G = m >= 2 (58..63)   r=4,6: H = (m == 0) (64, 96)
+  //   r=5: G = m >= 3 (91..95)     r=7: G = m in 3..6 (123..126)                    r=1: none;  bytes >= 0x80: none.
+  const uint32_t p15 = (~b2 & (b1 | b0)) | (b2 & ~b1);      // m in 1..5
+  const uint32_t p3 = b2 | (b1 & b0);                        // m >= 3
+  const uint32_t p36 = b2 ^ (b1 & b0);                       // m in 3..6
+  const uint32_t pz = ~(b2 | b1 | b0);                       // m == 0
+  const uint32_t g_even = ~b6 & (b5 | p15);                  // G for rows 0, 2 (rows 4, 6: none)
+  const uint32_t u = (b5 & p36) | (~b5 & p3);                // G for rows 7 / 5
+  const uint32_t v = b5 & (b2 | b1);                         // G for row 3 (row 1: none)
+  const uint32_t g_odd = (b6 & u) | (~b6 & v);
+  const uint32_t x = (b6 & pz) | (~b6 & b5);                 // H for the rows with b4 = 0: rows 4, 6 / row 2
+  const uint32_t y0 = (b3 & g_even) | (~b3 & x);             // rows with b4 = 0
+  const uint32_t z = b3 & g_odd;                             // rows with b4 = 1 (H = none)
+  const uint32_t np = (b4 & z) | (~b4 & y0);                 // non-LETTER among bytes < 0x80
+  letter = b7 | ~np;
+  const uint32_t q = ~b5 | (~b3 & pz);                       // within rows 0 and 2: all of row 0's, only 0x20 of row 2's
+  const uint32_t t = np & ~b6 & ~b4;
+  ws = t & q & ~b7;
 }
 
 __device__ __forceinline__ unsigned bfind(uint32_t x) {              // index of the most significant 1 bit, 0xffffffff for 0
@@ -433,6 +445,18 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
     }
     const unsigned total = __reduce_add_sync(kFull, own);             // <= 4096 per field: no carry between the halves
 
+    // (f, placed inside e) the stage (text and table) is dead once the table has been read for the last time: refill it
+    // with the chunk kStages ahead BEFORE the next window of offsets is requested, so that the proxy fence (a CTA-level
+    // memory barrier) does not wait for that global load.
+    bool refilled = false;
+    auto refill = [&]() {
+      refilled = true;
+      __syncwarp();
+      if (lane == 0 && it + kStages < it_tma) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        issue(it + kStages, s);
+      }
+    };
     // (e) attribute to prompts: boundary k (= off[k]) closes prompt k-1
     unsigned base_c = 0;                                              // packed prefix count at the last boundary handled
     if (bm) {
@@ -471,8 +495,8 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
         base_c = __shfl_sync(kFull, cj, nb - 1);
         last_rel = __shfl_sync(kFull, orel, nb - 1);
         optr += nb; left -= nb; wp += nb; tp += nb;
+        if (nb < 32) { refill(); load_window(); break; }              // common case: this was the last pass over the table
         load_window();
-        if (nb < 32) break;
         rel = orel - crel;
         inb = rel < (unsigned)kChunk;
         bm = __ballot_sync(kFull, inb);
@@ -481,13 +505,8 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
     }
     const unsigned tail = total - base_c;
     accW += tail & 0xffffu; accT += tail >> 16;
+    if (!refilled) refill();
     __syncwarp();
-
-    // (f) the stage (text and table) is dead: refill it with the chunk kStages ahead
-    if (lane == 0 && it + kStages < it_tma) {
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      issue(it + kStages, s);
-    }
     if (++s == kStages) { s = 0; parity ^= 1u; }
   }
 

@@ -39,15 +39,19 @@ def _planes(w):
 def _classify(b):
     b0, b1, b2, b3, b4, b5, b6, b7 = b
     n = lambda x: ~x & M32
-    u9_13 = b3 & ((n(b2) & (b1 | b0)) | (b2 & n(b1)))
-    z0 = n(b3 | b2 | b1 | b0)
-    ge10 = b3 & (b2 | b1)
-    ge11 = b3 & (b2 | (b1 & b0))
-    u11_14 = b3 & ((n(b2) & b1 & b0) | (b2 & n(b1 & b0)))
-    nonletter = n(b7) & ((n(b6) & n(b5) & n(b4) & u9_13) | (n(b6) & b5 & n(b4)) | (n(b6) & b5 & b4 & ge10) | (b6 & n(b4) & z0)
-                         | (b6 & n(b5) & b4 & ge11) | (b6 & b5 & b4 & u11_14))
-    ws = n(b7) & n(b6) & n(b4) & ((n(b5) & u9_13) | (b5 & z0))
-    return ws, n(nonletter)
+    mux = lambda sel, a, c: (sel & a) | (n(sel) & c)
+    p15 = (n(b2) & (b1 | b0)) | (b2 & n(b1))
+    p3 = b2 | (b1 & b0)
+    p36 = b2 ^ (b1 & b0)
+    pz = n(b2 | b1 | b0)
+    g_even = n(b6) & (b5 | p15)
+    g_odd = mux(b6, mux(b5, p36, p3), b5 & (b2 | b1))
+    x = mux(b6, pz, b5)
+    np_ = mux(b4, b3 & g_odd, mux(b3, g_even, x))
+    letter = b7 | n(np_)
+    q = n(b5) | (n(b3) & pz)
+    ws = np_ & n(b6) & n(b4) & q & n(b7)
+    return ws, letter
 
 
 def test_transposition_and_class_network():
