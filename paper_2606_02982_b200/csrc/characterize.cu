@@ -59,6 +59,18 @@ __device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned coun
 __device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_wait_a(uint32_t bar, unsigned parity) {   // bar: shared-window address
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP_A:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra.uni WAIT_DONE_A;\n"
+      "bra.uni WAIT_LOOP_A;\n"
+      "WAIT_DONE_A:\n"
+      "}\n" ::"r"(bar), "r"(parity)
+      : "memory");
+}
 __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
   asm volatile(
       "{\n"
@@ -265,10 +277,16 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
   const unsigned n_it = (unsigned)(c_end - c_begin);
   const unsigned it_tma = n_tma_chunks <= c_begin ? 0u : (n_tma_chunks - c_begin >= (long long)n_it ? n_it : (unsigned)(n_tma_chunks - c_begin));
   const int row0 = (int)(c_begin * 32);   // first TMA row of the span (rows < 2^31: n_bytes <= 2^37 checked by the host)
+  // shared-window addresses of the stages and their barriers, computed once (the generic->shared conversion per use costs
+  // a dozen instructions in the loop)
+  const uint32_t stage_a0 = smem_u32(stage[0]), mbar_a0 = smem_u32(&mbar[0]);
   auto issue = [&](unsigned it, int s) {  // lane 0 only
     if (it < it_tma) {
-      mbar_expect_tx(&mbar[s], (unsigned)kChunk);
-      tma_load_rows(stage[s], &tmap, row0 + (int)it * 32, &mbar[s]);
+      const uint32_t bar = mbar_a0 + 8u * (unsigned)s, dst = stage_a0 + (unsigned)kChunk * (unsigned)s;
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"((unsigned)kChunk) : "memory");
+      asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
+                   "l"(&tmap), "r"(0), "r"(row0 + (int)it * 32), "r"(bar)
+                   : "memory");
     }
   };
   if (lane == 0)
@@ -343,7 +361,7 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
     // (a) the lane's 128 bytes -> WS / LETTER masks, 32 bytes at a time
     uint32_t ws[NW], L[NW];
     if (by_tma) {
-      mbar_wait(&mbar[s], parity);
+      mbar_wait_a(mbar_a0 + 8u * (unsigned)s, parity);
       const uint8_t* row = lrow + s * kChunk;
 #pragma unroll
       for (int g = 0; g < NW; ++g) {
