@@ -38,7 +38,8 @@ constexpr int NW = 4;                         // 32-byte groups (= 32-bit mask w
 constexpr int kSeg = 32 * NW;                 // 128 bytes per lane per chunk = one TMA box row
 constexpr int kChunk = 32 * kSeg;             // 4 KiB per warp per step
 constexpr int kStages = 2;
-constexpr int kCtasPerSM = 3;
+constexpr int kSub = 2;                       // chunks per boundary-attribution pass (amortises the window handling)
+constexpr int kCtasPerSM = 2;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr long long kInfOff = 0x7fffffffffffffffLL;
 constexpr unsigned kNoRel = 0xffffffffu;      // "no boundary" in span-relative 32-bit positions
@@ -46,7 +47,8 @@ static_assert(kChunk % 4 == 0 && kSeg == 128, "a TMA box row is one 128-byte swi
 
 struct Smem {
   alignas(1024) uint8_t data[kWarps][kStages][kChunk];   // SWIZZLE_128B needs 1024-byte aligned stages
-  unsigned int sbits[kWarps][kChunk / 32];               // prompt-start bit per byte of the warp's current chunk
+  uint4 att[kWarps][kSub * kChunk / 32];                 // per 32-byte word: {wordstart mask, token mask, packed count before it}
+  unsigned int sbits[kWarps][kSub * kChunk / 32];        // prompt-start bit per byte of the warp's current kSub chunks
   unsigned long long mbar[kWarps][kStages];
 };
 
@@ -270,7 +272,7 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
 #pragma unroll
-  for (int k = 0; k < kChunk / 32 / 32; ++k) sb[lane + 32 * k] = 0u;
+  for (int k = 0; k < kSub * kChunk / 32 / 32; ++k) sb[lane + 32 * k] = 0u;
   __syncwarp();
 
   // chunks [0, n_tma_chunks) lie wholly inside the readable range and come by TMA; the last, partial one is read directly
@@ -355,7 +357,34 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
   const bool head_edge = pos0 < 0;
   int s = 0;
   unsigned parity = 0, crel = 0;      // stage index, its mbarrier phase, chunk start relative to pos0
-  for (unsigned it = 0; it < n_it; ++it, crel += kChunk) {   // chunk = positions [pos0 + crel, +kChunk) relative to bytes
+  uint4* att = sm.att[warp];
+  for (unsigned it0 = 0; it0 < n_it; it0 += kSub, crel += kSub * kChunk) {   // kSub chunks: positions [pos0 + crel, +span)
+  const unsigned nsub = n_it - it0 < (unsigned)kSub ? n_it - it0 : (unsigned)kSub;
+  const unsigned span = nsub * (unsigned)kChunk;
+
+  // (b) prompt boundaries inside these chunks -> start bits (the window's lanes hold them in order)
+  unsigned rel = orel - crel;
+  bool inb = rel < span;
+  unsigned bm = __ballot_sync(kFull, inb);
+  if (inb) atomicOr(&sb[rel >> 5], 1u << (rel & 31));
+  if (bm == kFull) {                                     // rare: more than 32 boundaries may fall into the span
+    const long long cs = pos0 + crel, ce = cs + span;
+    const int64_t* o2p = optr;
+    for (long long l2 = left - 32; ; l2 -= 32) {
+      o2p += 32;
+      if (__ballot_sync(kFull, l2 > 0) == 0u) break;
+      const long long o2 = l2 > 0 ? *o2p : kInfOff;
+      const bool in2 = o2 >= cs && o2 < ce;
+      if (in2) atomicOr(&sb[(int)(o2 - cs) >> 5], 1u << ((int)(o2 - cs) & 31));
+      if (__ballot_sync(kFull, in2) != kFull) break;
+    }
+  }
+  __syncwarp();
+
+  unsigned total = 0;                                    // packed count of the chunks of this pass so far
+#pragma unroll 1
+  for (unsigned h = 0; h < nsub; ++h) {
+    const unsigned it = it0 + h;
     const bool by_tma = it < it_tma;
 
     // (a) the lane's 128 bytes -> WS / LETTER masks, 32 bytes at a time
@@ -387,7 +416,7 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
     if ((head_edge && it == 0) || it >= it_tail) {   // cs < 0 or ce > n_bytes: bytes outside [0,n_bytes) count as whitespace
 #pragma unroll
       for (int g = 0; g < NW; ++g) {
-        const long long sp = pos0 + crel + (long long)lane * kSeg + 32 * g;
+        const long long sp = pos0 + crel + (long long)(h * kChunk) + (long long)lane * kSeg + 32 * g;
         long long lo = -sp, hi = n_bytes - sp;
         lo = lo < 0 ? 0 : (lo > 32 ? 32 : lo);
         hi = hi < 0 ? 0 : (hi > 32 ? 32 : hi);
@@ -397,26 +426,11 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
       }
     }
 
-    // (b) prompt boundaries inside this chunk -> start bits (the window's lanes hold them in order)
-    unsigned rel = orel - crel;
-    bool inb = rel < (unsigned)kChunk;
-    unsigned bm = __ballot_sync(kFull, inb);
-    if (inb) atomicOr(&sb[rel >> 5], 1u << (rel & 31));
-    if (bm == kFull) {                                   // rare: more than 32 boundaries may fall into one chunk
-      const long long cs = pos0 + crel, ce = cs + kChunk;
-      const int64_t* o2p = optr;
-      for (long long l2 = left - 32; ; l2 -= 32) {
-        o2p += 32;
-        if (__ballot_sync(kFull, l2 > 0) == 0u) break;
-        const long long o2 = l2 > 0 ? *o2p : kInfOff;
-        const bool in2 = o2 >= cs && o2 < ce;
-        if (in2) atomicOr(&sb[(int)(o2 - cs) >> 5], 1u << ((int)(o2 - cs) & 31));
-        if (__ballot_sync(kFull, in2) != kFull) break;
-      }
-    }
+    // the stage's bytes are all in registers now: refill it with the chunk kStages ahead
     __syncwarp();
-    const uint4 S4 = reinterpret_cast<const uint4*>(sb)[lane];
-    reinterpret_cast<uint4*>(sb)[lane] = make_uint4(0u, 0u, 0u, 0u);
+    if (lane == 0 && it + kStages < it_tma) issue(it + kStages, s);
+    const uint4 S4 = reinterpret_cast<const uint4*>(sb)[h * 32 + lane];
+    reinterpret_cast<uint4*>(sb)[h * 32 + lane] = make_uint4(0u, 0u, 0u, 0u);
     const uint32_t S[NW] = {S4.x, S4.y, S4.z, S4.w};
 
     // (c) carries between lanes: one WS bit, one LETTER bit, the letter count (mod 4) of the run that is still open
@@ -461,35 +475,25 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
       cpk[g] = (unsigned)__popc(fw[g]) + ((unsigned)__popc(ft[g]) << 16);
       own += cpk[g];
     }
-    const unsigned total = __reduce_add_sync(kFull, own);             // <= 4096 per field: no carry between the halves
+    // table for the boundary pass: per 32-byte word {wordstart mask, token mask, packed count before the word}
+    unsigned incl = own;                                              // inclusive prefix over lanes (0/1 multipliers: IMAD)
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+      const unsigned y = __shfl_up_sync(kFull, incl, 1 << k);
+      asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(incl) : "r"(y), "r"(scan_on[k]));
+    }
+    unsigned run = total + incl - own;
+#pragma unroll
+    for (int g = 0; g < NW; ++g) { att[(h * 32 + lane) * NW + g] = make_uint4(fw[g], ft[g], run, 0u); run += cpk[g]; }
+    total += __reduce_add_sync(kFull, own);                           // <= 8192 per field: no carry between the halves
+    if (++s == kStages) { s = 0; parity ^= 1u; }
+  }
+  __syncwarp();
 
-    // (f, placed inside e) the stage (text and table) is dead once the table has been read for the last time: refill it
-    // with the chunk kStages ahead BEFORE the next window of offsets is requested, so that the proxy fence (a CTA-level
-    // memory barrier) does not wait for that global load.
-    bool refilled = false;
-    auto refill = [&]() {
-      refilled = true;
-      __syncwarp();
-      if (lane == 0 && it + kStages < it_tma) {
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        issue(it + kStages, s);
-      }
-    };
-    // (e) attribute to prompts: boundary k (= off[k]) closes prompt k-1
+  // (e) attribute to prompts: boundary k (= off[k]) closes prompt k-1
+  {
     unsigned base_c = 0;                                              // packed prefix count at the last boundary handled
     if (bm) {
-      unsigned incl = own;                                            // inclusive prefix over lanes (0/1 multipliers: IMAD)
-#pragma unroll
-      for (int k = 0; k < 5; ++k) {
-        const unsigned y = __shfl_up_sync(kFull, incl, 1 << k);
-        asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(incl) : "r"(y), "r"(scan_on[k]));
-      }
-      // table in the consumed stage: per 32-byte word {wordstart mask, token mask, packed count before the word}
-      uint4* att = reinterpret_cast<uint4*>(stage[s]);
-      unsigned run = incl - own;
-#pragma unroll
-      for (int g = 0; g < NW; ++g) { att[lane * NW + g] = make_uint4(fw[g], ft[g], run, 0u); run += cpk[g]; }
-      __syncwarp();
       for (;;) {
         const int nb = __popc(bm);
         const unsigned r = inb ? rel : 0u;
@@ -513,19 +517,18 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
         base_c = __shfl_sync(kFull, cj, nb - 1);
         last_rel = __shfl_sync(kFull, orel, nb - 1);
         optr += nb; left -= nb; wp += nb; tp += nb;
-        if (nb < 32) { refill(); load_window(); break; }              // common case: this was the last pass over the table
         load_window();
+        if (nb < 32) break;
         rel = orel - crel;
-        inb = rel < (unsigned)kChunk;
+        inb = rel < span;
         bm = __ballot_sync(kFull, inb);
         if (!bm) break;
       }
     }
     const unsigned tail = total - base_c;
     accW += tail & 0xffffu; accT += tail >> 16;
-    if (!refilled) refill();
     __syncwarp();
-    if (++s == kStages) { s = 0; parity ^= 1u; }
+  }
   }
 
   // the prompt still open at the span's end continues in the next warp's span
