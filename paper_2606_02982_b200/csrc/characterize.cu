@@ -382,8 +382,9 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
   __syncwarp();
 
   unsigned total = 0;                                    // packed count of the chunks of this pass so far
-#pragma unroll 1
-  for (unsigned h = 0; h < nsub; ++h) {
+#pragma unroll
+  for (unsigned h = 0; h < (unsigned)kSub; ++h) {
+    if (h >= nsub) break;
     const unsigned it = it0 + h;
     const bool by_tma = it < it_tma;
 
