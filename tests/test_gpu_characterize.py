@@ -108,3 +108,30 @@ def test_empty_inputs_and_bad_offsets(G):
     ds.characterize(text, torch.tensor([0, 12, 5, 18], dtype=torch.int64, device=G.DEV))
     assert ds.device_status() & 1                                        # DS_DEV_BAD_OFFSETS
     assert ds.device_status() == 0                                       # cleared by the read
+
+
+def test_sizes_around_chunk_seams(G):
+    # K1 v3 moves 4 KiB chunks by TMA (whole chunks only), reads the last partial chunk directly and handles boundaries
+    # once per two chunks: buffer sizes and base misalignments around every one of those seams, dense and sparse prompts
+    rng = np.random.default_rng(21)
+    alpha = np.frombuffer(b"  \t\nabcdefghijklmnopqrstuvwxyz,.;", np.uint8)
+    big = alpha[rng.integers(0, len(alpha), 3 * 8192 + 64)]
+    for n in (1, 15, 16, 17, 4095, 4096, 4097, 8191, 8192, 8193, 12287, 12288, 12289, 16384, 3 * 8192 + 5):
+        for mis in (0, 5):
+            buf = big[mis:mis + n]
+            dense = np.unique(np.concatenate([[0, n], rng.integers(0, n + 1, max(2, n // 3))]))
+            sparse = np.unique(np.concatenate([[0, n], rng.integers(0, n + 1, 3)]))
+            for off in (dense, sparse):
+                w, k = G.gpu_characterize(buf, off) if mis == 0 else _misaligned(G, big, mis, n, off)
+                ow, ok = oracle.characterize(buf, off)
+                assert np.array_equal(w, ow) and np.array_equal(k, ok), (n, mis, len(off))
+
+
+def _misaligned(G, big, mis, n, off):
+    import torch
+    import paper_2606_02982_b200 as ds
+    t = torch.from_numpy(np.ascontiguousarray(big)).to(G.DEV)
+    o = torch.from_numpy(np.ascontiguousarray(off, np.int64)).to(G.DEV)
+    w, k = ds.characterize(t[mis:mis + n], o)
+    assert ds.device_status() == 0
+    return w.cpu().numpy(), k.cpu().numpy()
