@@ -58,6 +58,8 @@ def _o():
         lib.oracle_queue_depth.restype = C.c_int
         lib.oracle_simulate_budget.argtypes = [p, p, p, p, p, C.c_int64, p, p, p, p, p, p, p]
         lib.oracle_simulate_budget.restype = C.c_int
+        lib.oracle_simulate_closed.argtypes = [p, p, p, p, C.c_int64, C.c_int64, p, C.c_int64, p, p, p, p, p, p, p, p]
+        lib.oracle_simulate_closed.restype = C.c_int
         lib.oracle_latencies.argtypes = [p, p, C.c_int64, p, p, p, p, p, p, p, p, p]
         lib.oracle_tail_stats.argtypes = [p, p, C.c_int64, C.c_int32, p, C.c_int32, p, p]
         for f in (lib.oracle_characterize, lib.oracle_simulate, lib.oracle_latencies, lib.oracle_tail_stats):
@@ -200,7 +202,7 @@ def queue_depth(trace_off, arrival, tier, words, tokens, out_len, instances, out
 
 
 def simulate_budget(trace_off, arrival, tier, words, tokens, out_len, category, budget, server, instances, out_off=None,
-                    want_traj=False, want_est=False):
+                    want_traj=False, want_est=False, n_clients=0, think_ticks=0):
     """Full Eq. 1-2 estimator with per-category feedback. budget: object with t_base[4], s_tenant[3], f_slope, f_max.
     Returns start_tick, done_tick, ema_final[n_inst,4] (then ema_traj[samples,4] if want_traj, then est if want_est)."""
     tr, keep = _traces(trace_off, arrival, tier, words, tokens, out_len)
@@ -223,6 +225,13 @@ def simulate_budget(trace_off, arrival, tier, words, tokens, out_len, category, 
         toff = traj_offsets(keep[0], inst, server.traj_every)
         traj = np.zeros((int(toff[-1]), 4), np.float64)
     est = np.full(total, -1, np.int64) if want_est else None
+    if n_clients > 0:   # closed loop: also returns the arrival tick of every simulated request (last element)
+        arr_out = np.full(total, -1, np.int64)
+        rc = _o().oracle_simulate_closed(C.byref(tr), _p(cat), C.byref(bp), C.byref(sv), int(n_clients), int(think_ticks), _p(inst),
+                                         n_inst, _p(out_off), _p(arr_out), _p(start), _p(done), _p(ema), _p(toff), _p(traj), _p(est))
+        if rc:
+            raise ValueError("oracle_simulate_closed: contract violation")
+        return (start, done, ema) + ((traj,) if want_traj else ()) + ((est,) if want_est else ()) + (arr_out,)
     rc = _o().oracle_simulate_budget(C.byref(tr), _p(cat), C.byref(bp), C.byref(sv), _p(inst), n_inst, _p(out_off), _p(start),
                                      _p(done), _p(ema), _p(toff), _p(traj), _p(est))
     if rc:

@@ -62,6 +62,8 @@ struct Sim {
   const int64_t* arr; const uint8_t* tier; const int32_t* W; const int32_t* P; const int32_t* O;
   int64_t n; const oracle_server* sv; int policy, estimator; double alpha;
   const uint8_t* cat = nullptr; const oracle_budget* bp = nullptr;   // budget estimators only (Eq. 1-2 in full)
+  // closed loop ("50 concurrent clients"): requests [released, n) have not been submitted yet
+  std::vector<int64_t> arr_dyn; int64_t released = 0, think = 0; bool closed = false;
   // state (SURVEY.md §8(c) C.2 "State per instance")
   int64_t now = 0, next = 0, kv_used = 0, done = 0;
   double B[4] = {1.0, 1.0, 1.0, 1.0};   // per tier (estimators 0/1) or per semantic category (budget estimators)
@@ -150,6 +152,7 @@ struct Sim {
 }  // namespace
 
 static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const oracle_budget* bp, const oracle_server* sv,
+                         int64_t n_clients, int64_t think_ticks, int64_t* arrival_out,
                          const oracle_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t* start_tick,
                          int64_t* done_tick, double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out) {
   const int nb = bp ? 4 : 3;   // factors per instance: semantic categories (budget estimators) or tenant tiers
@@ -159,6 +162,7 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
     for (int t = 0; t < 3; ++t) if (!(bp->s_tenant[t] > 0.0)) return -1;
     if (!(bp->f_slope >= 0.0) || !(bp->f_max >= 1.0)) return -1;
   }
+  if (n_clients < 0 || think_ticks < 0 || (n_clients > 0 && !arrival_out)) return -1;
   if (sv->max_batch < 1) return -1;
   if (sv->weight[0] < 1 || sv->weight[1] < 1 || sv->weight[2] < 1) return -1;
   if (sv->aging_step < 1) return -1;
@@ -172,6 +176,9 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
     s.arr = tr->arrival_tick + lo; s.tier = tr->tier + lo; s.W = tr->words + lo; s.P = tr->tokens + lo;
     s.O = tr->out_len + lo; s.n = n; s.sv = sv; s.policy = in.policy; s.estimator = in.estimator; s.alpha = in.ema_alpha;
     s.est.assign(n, 0); s.g.assign(n, 0);
+    // arrivals: the input array (open loop), or only its first n_clients entries (closed loop; the rest follow completions)
+    s.arr_dyn.assign(s.arr, s.arr + n); s.arr = s.arr_dyn.data();
+    s.closed = n_clients > 0; s.think = think_ticks; s.released = s.closed ? std::min<int64_t>(n_clients, n) : n;
     if (bp) {
       s.cat = category + lo; s.bp = bp;
       for (int64_t r = 0; r < n; ++r) if (s.cat[r] > 3) return -1;
@@ -185,7 +192,7 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
     for (;;) {
       if (!skip_to_ingest_now) {
         // 1. INGEST-EARLY: arrivals strictly before `now` use the factors before this tick's completions (R-ORD).
-        while (s.next < n && s.arr[s.next] < s.now) s.admit_to_queue(s.next++);
+        while (s.next < s.released && s.arr[s.next] < s.now) s.admit_to_queue(s.next++);
         // 2. RETIRE: completions at `now`, ascending request index.
         for (size_t i = 0; i < s.R.size();) {
           int64_t r = s.R[i];
@@ -195,6 +202,8 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
             s.R.erase(s.R.begin() + i);
             s.ema_update(s.tier[r], r);
             ++s.done;
+            // closed loop: the client whose request completed submits the next request after its think time
+            if (s.closed && s.released < n) s.arr_dyn[s.released++] = s.now + s.think;
             if (traj && sv->traj_every > 0 && s.done % sv->traj_every == 0) {
               double* q = traj + (s.done / sv->traj_every - 1) * nb;
               for (int k = 0; k < nb; ++k) q[k] = s.B[k];
@@ -204,7 +213,7 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
       }
       skip_to_ingest_now = false;
       // 3. INGEST-NOW: arrivals at exactly `now` see the updated factors.
-      while (s.next < n && s.arr[s.next] <= s.now) s.admit_to_queue(s.next++);
+      while (s.next < s.released && s.arr[s.next] <= s.now) s.admit_to_queue(s.next++);
       // 4. ADMIT
       int64_t prefill_new = 0;
       while ((int64_t)s.R.size() < sv->max_batch && !s.queued.empty()) {
@@ -222,6 +231,7 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
       // 5. IDLE / END
       if (s.R.empty()) {
         if (s.next == n) break;
+        if (s.next >= s.released) return -1;   // unreachable: an empty server means every submitted request completed
         s.now = s.arr[s.next];
         skip_to_ingest_now = true;
         continue;
@@ -236,6 +246,7 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
     }
     for (int k = 0; k < nb; ++k) ema_final[ii * nb + k] = s.B[k];
     if (est_out) for (int64_t r = 0; r < n; ++r) est_out[out_off[ii] + r] = s.est[r];   // frozen at arrival (A5)
+    if (arrival_out) for (int64_t r = 0; r < n; ++r) arrival_out[out_off[ii] + r] = s.arr_dyn[r];
   }
   return 0;
 }
@@ -243,7 +254,7 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
 extern "C" int oracle_simulate(const oracle_traces* tr, const oracle_server* sv, const oracle_instance* inst,
                                int64_t n_inst, const int64_t* out_off, int64_t* start_tick, int64_t* done_tick,
                                double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out) {
-  return simulate_impl(tr, nullptr, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out);
+  return simulate_impl(tr, nullptr, nullptr, sv, 0, 0, nullptr, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out);
 }
 
 extern "C" int oracle_simulate_budget(const oracle_traces* tr, const uint8_t* category, const oracle_budget* bp,
@@ -251,7 +262,17 @@ extern "C" int oracle_simulate_budget(const oracle_traces* tr, const uint8_t* ca
                                       int64_t* start_tick, int64_t* done_tick, double* ema_final, const int64_t* traj_off,
                                       double* ema_traj, int64_t* est_out) {
   if (!bp) return -1;
-  return simulate_impl(tr, category, bp, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out);
+  return simulate_impl(tr, category, bp, sv, 0, 0, nullptr, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out);
+}
+
+extern "C" int oracle_simulate_closed(const oracle_traces* tr, const uint8_t* category, const oracle_budget* bp,
+                                      const oracle_server* sv, int64_t n_clients, int64_t think_ticks, const oracle_instance* inst,
+                                      int64_t n_inst, const int64_t* out_off, int64_t* arrival_out, int64_t* start_tick,
+                                      int64_t* done_tick, double* ema_final, const int64_t* traj_off, double* ema_traj,
+                                      int64_t* est_out) {
+  if (!bp || n_clients < 1) return -1;
+  return simulate_impl(tr, category, bp, sv, n_clients, think_ticks, arrival_out, inst, n_inst, out_off, start_tick, done_tick,
+                       ema_final, traj_off, ema_traj, est_out);
 }
 
 extern "C" int oracle_latencies(const oracle_traces* tr, const oracle_instance* inst, int64_t n_inst,

@@ -63,6 +63,16 @@ int oracle_simulate_budget(const oracle_traces* tr, const uint8_t* category, con
                            const oracle_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t* start_tick,
                            int64_t* done_tick, double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out);
 
+/* Closed-loop arrivals ("50 concurrent clients", 3000 requests per run): only the first n_clients
+ * requests of a trace arrive at their input ticks; every completion (in completion order: tick, then request index) lets
+ * the next request of the trace arrive at  completion tick + think_ticks. Same-tick ordering as everywhere: completions,
+ * then same-tick arrivals (R-ORD). arrival_out [out_off[n_inst]]: the arrival tick of every simulated request (per
+ * instance: arrivals now depend on the policy). Estimator and feedback as in oracle_simulate_budget. */
+int oracle_simulate_closed(const oracle_traces* tr, const uint8_t* category, const oracle_budget* bp, const oracle_server* sv,
+                           int64_t n_clients, int64_t think_ticks, const oracle_instance* inst, int64_t n_inst,
+                           const int64_t* out_off, int64_t* arrival_out, int64_t* start_tick, int64_t* done_tick,
+                           double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out);
+
 /* Estimation fidelity (Eq. 3-4 job classes; Tables IV, IX, X): per reporting group, exact integer sums
  * over its simulated requests: out[g*11 + ..] = { n, sum|est-P|, sum(est-P)^2, sum est, sum P, n_short, n_medium, n_long,
  * sum qdelay_short, sum qdelay_medium, sum qdelay_long } with class short: est<=128, medium: est<=512, long: else.
