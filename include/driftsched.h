@@ -148,6 +148,19 @@ int ds_simulate_budget(const ds_traces* tr, const uint8_t* category, const ds_bu
                        double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace,
                        size_t workspace_bytes, void* stream);
 
+/* ds_simulate_budget with CLOSED-LOOP arrivals ("50 concurrent clients",
+ * 3000 requests per run): only the first n_clients requests of a trace arrive at their tr->arrival_tick; every completion
+ * (in completion order: tick, then request index) lets the next request of the trace arrive at completion tick +
+ * think_ticks. Same-tick order as everywhere (R-ORD): completions, then same-tick arrivals, which therefore see the updated
+ * factors. n_clients >= 1, think_ticks >= 0 (host values; DS_EINVAL otherwise); n_clients >= trace length = the open loop.
+ * arrival_out [out_off[n_inst]] int64 device (written): the arrival tick of every simulated request - per instance,
+ * because arrivals now depend on the policy; latencies are done_tick - arrival_out / start_tick - arrival_out.
+ * Everything else as ds_simulate_budget. */
+int ds_simulate_closed(const ds_traces* tr, const uint8_t* category, const ds_budget* bp, const ds_server* sv, int32_t n_clients,
+                       int64_t think_ticks, const ds_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t* arrival_out,
+                       int64_t* start_tick, int64_t* done_tick, double* ema_final, const int64_t* traj_off, double* ema_traj,
+                       int64_t* est_out, void* workspace, size_t workspace_bytes, void* stream);
+
 /* Estimation fidelity: job classes of Eq. 3-4 (short est<=128, medium
  * est<=512, long otherwise), token-estimation error (Tables IV, X) and queue wait by job class
  * (Table IX), per reporting group g = group[instance] (nullable -> 0) in [0, n_groups).

@@ -10,7 +10,7 @@ LIB_PATH = os.path.join(_HERE, "libdriftsched.so")
 DS_OK, DS_EINVAL, DS_ECUDA, DS_ENOMEM = 0, -1, -2, -3
 WS_CHARACTERIZE, WS_SIMULATE, WS_TAIL_STATS = 0, 1, 2
 
-EXPORTS = ["ds_characterize", "ds_simulate", "ds_simulate_est", "ds_simulate_budget", "ds_estimation_error", "ds_queue_depth", "ds_latencies", "ds_tail_stats",
+EXPORTS = ["ds_characterize", "ds_simulate", "ds_simulate_est", "ds_simulate_budget", "ds_simulate_closed", "ds_estimation_error", "ds_queue_depth", "ds_latencies", "ds_tail_stats",
            "ds_latency_stats", "ds_workspace_bytes", "ds_device_status",
            "ds_strerror", "ds_last_cuda_error", "ds_launch_count"]
 
@@ -52,6 +52,7 @@ def lib():
         L.ds_simulate.argtypes = [C.POINTER(DsTraces), C.POINTER(DsServer), p, i64, p, p, p, p, p, p, p, sz, p]
         L.ds_simulate_est.argtypes = [C.POINTER(DsTraces), C.POINTER(DsServer), p, i64, p, p, p, p, p, p, p, p, sz, p]
         L.ds_simulate_budget.argtypes = [C.POINTER(DsTraces), p, C.POINTER(DsBudget), C.POINTER(DsServer), p, i64, p, p, p, p, p, p, p, p, sz, p]
+        L.ds_simulate_closed.argtypes = [C.POINTER(DsTraces), p, C.POINTER(DsBudget), C.POINTER(DsServer), i32, i64, p, i64, p, p, p, p, p, p, p, p, p, sz, p]
         L.ds_estimation_error.argtypes = [C.POINTER(DsTraces), p, i64, p, p, p, p, i32, p, p, p]
         L.ds_queue_depth.argtypes = [C.POINTER(DsTraces), p, i64, p, p, i64, i64, i64, p, p]
         L.ds_latencies.argtypes = [C.POINTER(DsTraces), p, i64, p, i64, p, p, p, p, p, p, p, p, p]
@@ -64,7 +65,7 @@ def lib():
         L.ds_strerror.restype = C.c_char_p
         L.ds_last_cuda_error.restype = C.c_char_p
         L.ds_launch_count.restype = i64
-        for f in ("ds_characterize", "ds_simulate", "ds_simulate_est", "ds_simulate_budget", "ds_estimation_error", "ds_queue_depth", "ds_latencies", "ds_tail_stats", "ds_latency_stats", "ds_device_status"):
+        for f in ("ds_characterize", "ds_simulate", "ds_simulate_est", "ds_simulate_budget", "ds_simulate_closed", "ds_estimation_error", "ds_queue_depth", "ds_latencies", "ds_tail_stats", "ds_latency_stats", "ds_device_status"):
             getattr(L, f).restype = C.c_int
         _lib = L
     return _lib

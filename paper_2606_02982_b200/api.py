@@ -213,7 +213,8 @@ def queue_depth(trace_off, arrival, tier, words, tokens, out_len, inst, out_off,
 
 
 def simulate_budget(trace_off, arrival, tier, words, tokens, out_len, category, budget, server, inst, out_off, n_total,
-                    start=None, done=None, ema_final=None, traj_off=None, ema_traj=None, est_out=None, workspace=None):
+                    start=None, done=None, ema_final=None, traj_off=None, ema_traj=None, est_out=None, workspace=None,
+                    n_clients=0, think_ticks=0, arrival_out=None):
     """ds_simulate_budget. category uint8 CUDA tensor (per request); budget: object with t_base[4], s_tenant[3], f_slope,
     f_max. Returns (start_tick, done_tick, ema_final[n_inst,4])."""
     tr = _traces(trace_off, arrival, tier, words, tokens, out_len)
@@ -231,6 +232,15 @@ def simulate_budget(trace_off, arrival, tier, words, tokens, out_len, category, 
         ema_final = torch.empty((n_inst, 4), dtype=torch.float64, device=dev)
     if workspace is None:
         workspace = _workspace(_lib.WS_SIMULATE, n_total, n_inst, dev)
+    if n_clients > 0:   # ds_simulate_closed: closed-loop arrivals, returns arrival_out as a 4th element
+        if arrival_out is None:
+            arrival_out = torch.empty(n_total, dtype=torch.int64, device=dev)
+        _need_cuda(arrival_out)
+        check("ds_simulate_closed", lib().ds_simulate_closed(C.byref(tr), _ptr(category), C.byref(bp), C.byref(sv), int(n_clients),
+                                                             int(think_ticks), _ptr(inst), n_inst, _ptr(out_off), _ptr(arrival_out),
+                                                             _ptr(start), _ptr(done), _ptr(ema_final), _ptr(traj_off), _ptr(ema_traj),
+                                                             _ptr(est_out), _ptr(workspace), workspace.numel(), _stream()))
+        return start, done, ema_final, arrival_out
     check("ds_simulate_budget", lib().ds_simulate_budget(C.byref(tr), _ptr(category), C.byref(bp), C.byref(sv), _ptr(inst), n_inst,
                                                          _ptr(out_off), _ptr(start), _ptr(done), _ptr(ema_final), _ptr(traj_off),
                                                          _ptr(ema_traj), _ptr(est_out), _ptr(workspace), workspace.numel(), _stream()))

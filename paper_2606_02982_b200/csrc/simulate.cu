@@ -44,6 +44,7 @@ struct Params {
   const ds_instance* inst; int64_t n_inst; const int64_t* out_off; int64_t* start_tick; int64_t* done_tick;
   double* ema_final; const int64_t* traj_off; double* ema_traj; int64_t* est_out;
   const uint8_t* category; ds_budget bp;   // budget estimators only (ds_simulate_budget)
+  int32_t n_clients; int64_t think; int64_t* arrival_out;   // closed-loop arrivals (ds_simulate_closed), n_clients = 0: open loop
   unsigned long long* heap_ws; unsigned int* counter; unsigned int* status; const unsigned int* perm;
 };
 
@@ -161,11 +162,23 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   TierCursor tc[3];
   const int wtot = p.w0 + p.w1 + p.w2;
 
+  // Closed loop (ds_simulate_closed): arrivals live in arrival_out (per instance). The first n_clients
+  // entries are the trace's, the rest start at kInf ("not submitted yet") and are written when a completion releases them.
+  const bool closed = kBudget && p.n_clients > 0;
+  int64_t* arr_d = closed ? p.arrival_out + oo : nullptr;
+  int released = n;
+  if (closed) {
+    released = p.n_clients < n ? p.n_clients : n;
+    for (int i = lane; i < n; i += 32) __stcg(arr_d + i, i < released ? arr[i] : kInf);
+    __syncwarp();
+  }
+  auto arr_at = [&](const int i) -> long long { return closed ? (long long)__ldcg(arr_d + i) : (long long)arr[i]; };
+
   // arrival window: lane holds request wb+lane
   int wb = 0; long long w_arr = kInf; int w_tier = 0, w_base = 0, w_cat = 0;
   auto load_window = [&]() {
     const int i = wb + lane;
-    if (i < n) { w_arr = arr[i]; w_tier = tier[i]; w_base = BASE[i]; } else { w_arr = kInf; w_tier = 0; w_base = 0; }
+    if (i < n) { w_arr = arr_at(i); w_tier = tier[i]; w_base = BASE[i]; } else { w_arr = kInf; w_tier = 0; w_base = 0; }
     if (kBudget) {
       w_cat = i < n ? (int)cat[i] : 0;
       if (w_cat > 3) { atomicOr(p.status, DS_DEV_BAD_TRACE); w_cat = 3; }
@@ -192,7 +205,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
     c.head = c.blk * 32 + (__ffs(c.mask) - 1);
     if (c.head < next) {   // already arrived: its frozen estimate sits in the done_tick scratch
       if (use_kv) c.est = (long long)__ldcg(dn + c.head);
-      if (kPolicy == DS_AGING) c.arr = arr[c.head];
+      if (kPolicy == DS_AGING) c.arr = arr_at(c.head);
     }
   };
   if (kCursor)
@@ -297,6 +310,14 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
         }
       }
       ++done;
+      if (kBudget && closed && released < n) {                // the client whose request completed submits the next one
+        const long long t_new = now + p.think;
+        if (lane == 0) __stcg(arr_d + released, t_new);
+        if (lane == released - wb) w_arr = t_new;             // (unsigned compare not needed: released >= next >= wb)
+        if (released == next) an = t_new;
+        ++released;
+        __syncwarp();
+      }
       if (traj && done % p.traj_every == 0 && lane < kFac) traj[kFac * (done / p.traj_every - 1) + lane] = Bl;
     }
     blocked = false;
@@ -565,7 +586,8 @@ size_t ws_simulate(int64_t total_requests, int64_t n_inst) {
 }
 
 }  // namespace ds
-static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_budget* bp, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
+static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_budget* bp, int32_t n_clients, int64_t think_ticks,
+                         int64_t* arrival_out, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
                          const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
                          const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace, size_t workspace_bytes,
                          void* stream) {
@@ -595,7 +617,8 @@ static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_
   p.traj_every = sv->traj_every;
   p.inst = inst; p.n_inst = n_inst; p.out_off = out_off; p.start_tick = start_tick; p.done_tick = done_tick;
   p.ema_final = ema_final; p.traj_off = traj_off; p.ema_traj = ema_traj; p.est_out = est_out;
-  p.category = category;
+  p.category = category; p.n_clients = n_clients; p.think = think_ticks; p.arrival_out = arrival_out;
+  if (n_clients < 0 || think_ticks < 0 || (n_clients > 0 && (!bp || !arrival_out))) return DS_EINVAL;
   if (bp) p.bp = *bp; else memset(&p.bp, 0, sizeof(p.bp));
   p.counter = (unsigned int*)workspace;
   unsigned int* perm = (unsigned int*)((char*)workspace + 256);
@@ -636,7 +659,7 @@ static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_
 extern "C" int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
                            const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
                            const int64_t* traj_off, double* ema_traj, void* workspace, size_t workspace_bytes, void* stream) {
-  return simulate_impl(tr, nullptr, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, nullptr, workspace,
+  return simulate_impl(tr, nullptr, nullptr, 0, 0, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, nullptr, workspace,
                        workspace_bytes, stream);
 }
 
@@ -645,7 +668,7 @@ extern "C" int ds_simulate_est(const ds_traces* tr, const ds_server* sv, const d
                                const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace,
                                size_t workspace_bytes, void* stream) {
   if (n_inst > 0 && !est_out) return DS_EINVAL;
-  return simulate_impl(tr, nullptr, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out, workspace,
+  return simulate_impl(tr, nullptr, nullptr, 0, 0, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out, workspace,
                        workspace_bytes, stream);
 }
 
@@ -654,6 +677,16 @@ extern "C" int ds_simulate_budget(const ds_traces* tr, const uint8_t* category, 
                                   int64_t* done_tick, double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out,
                                   void* workspace, size_t workspace_bytes, void* stream) {
   if (!bp) return DS_EINVAL;
-  return simulate_impl(tr, category, bp, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out,
-                       workspace, workspace_bytes, stream);
+  return simulate_impl(tr, category, bp, 0, 0, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj,
+                       est_out, workspace, workspace_bytes, stream);
+}
+
+extern "C" int ds_simulate_closed(const ds_traces* tr, const uint8_t* category, const ds_budget* bp, const ds_server* sv,
+                                  int32_t n_clients, int64_t think_ticks, const ds_instance* inst, int64_t n_inst,
+                                  const int64_t* out_off, int64_t* arrival_out, int64_t* start_tick, int64_t* done_tick,
+                                  double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace,
+                                  size_t workspace_bytes, void* stream) {
+  if (!bp || n_clients < 1) return DS_EINVAL;
+  return simulate_impl(tr, category, bp, n_clients, think_ticks, arrival_out, sv, inst, n_inst, out_off, start_tick, done_tick,
+                       ema_final, traj_off, ema_traj, est_out, workspace, workspace_bytes, stream);
 }

@@ -136,3 +136,55 @@ def test_paper_phases_shape_end_to_end(G):
     assert med[sjf, 1] < 0.58 * med[fifo, 1]                           # paper: -42 % median
     tier_med = want["e2e"][0][:3 * G2, 0].reshape(G2, 3)
     assert tier_med[2 * prio + 1, 0] < tier_med[2 * prio + 1, 1] < tier_med[2 * prio + 1, 2]
+
+
+@pytest.mark.parametrize("n_clients,think,max_batch,kv", [(1, 0, 1, 0), (7, 0, 4, 0), (50, 0, 32, 16384), (50, 25_000, 32, 4000),
+                                                          (300, 0, 64, 9000), (40, 1000, 200, 30000)])
+def test_closed_loop(G, n_clients, think, max_batch, kv):
+    import paper_2606_02982_b200 as ds
+    sv = wl.Server(max_batch=max_batch, kv_budget=kv, aging_step=40_000, traj_every=41)
+    combos = [(p, e, a) for p in wl.ALL_POLICIES for e, a in ((wl.BUDGET_SPLIT, 0.1), (wl.BUDGET_EXACT, 0.0))]
+    c = wl._trace_workload("t", 51 + n_clients, 3, 700, sv, combos, oracle.characterize, rho=1.0)
+    cat, out_len = wl.assign_categories(51 + n_clients, c.out_len)
+    arrival = c.arrival.copy().reshape(3, 700)
+    arrival[:, n_clients:] = 0                       # ignored by the closed loop; must not matter
+    arrival[:, :n_clients] = np.minimum(arrival[:, :n_clients], 50_000)
+    arrival = arrival.reshape(-1)
+    bp = wl.Budget(s_tenant=(1.25, 1.0, 0.8), f_slope=0.001, f_max=1.3)
+    tr = (c.trace_off, arrival, c.tier, c.words, c.tokens, out_len)
+    ost, odn, oema, otraj, oest, oarr = oracle.simulate_budget(*tr, cat, bp, sv, c.instances, out_off=c.out_off, want_traj=True,
+                                                               want_est=True, n_clients=n_clients, think_ticks=think)
+    d = G.upload(c)
+    d["out_len"] = torch.from_numpy(out_len).to(G.DEV)
+    d["arrival"] = torch.from_numpy(arrival).to(G.DEV)
+    dcat = torch.from_numpy(cat).to(G.DEV)
+    n_total = int(c.out_off[-1])
+    targs = (d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"])
+    toff_h = oracle.traj_offsets(c.trace_off, c.instances, sv.traj_every)
+    toff = torch.from_numpy(toff_h).to(G.DEV)
+    traj = torch.zeros((int(toff_h[-1]), 4), dtype=torch.float64, device=G.DEV)
+    est = torch.full((n_total,), -1, dtype=torch.int64, device=G.DEV)
+    st, dn, ema, arr = ds.api.simulate_budget(*targs, dcat, bp, sv, d["inst"], d["out_off"], n_total, traj_off=toff, ema_traj=traj,
+                                              est_out=est, n_clients=n_clients, think_ticks=think)
+    assert ds.device_status() == 0
+    for name, a, b in (("arrival", arr, oarr), ("start", st, ost), ("done", dn, odn), ("est", est, oest)):
+        a = a.cpu().numpy()
+        bad = np.flatnonzero(a != b)
+        assert bad.size == 0, (name, bad[:5], a[bad[:5]], b[bad[:5]], c.instances[bad[:5] // 700])
+    assert np.array_equal(ema.cpu().numpy().view(np.uint64), oema.view(np.uint64))
+    assert np.array_equal(traj.cpu().numpy().view(np.uint64), otraj.view(np.uint64))
+
+
+def test_closed_loop_hand_trace_and_contract(G):
+    import paper_2606_02982_b200 as ds
+    req = [[0, 1, 1, 9, 1], [0, 1, 1, 5, 1], [0, 1, 1, 3, 1], [0, 1, 1, 1, 1]]
+    c = G.tiny_workload(wl, req, wl.Server(max_batch=1, kv_budget=0), [(wl.SJF, wl.BUDGET_EXACT, 0.0)])
+    d = G.upload(c)
+    targs = (d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"])
+    cat = torch.zeros(4, dtype=torch.uint8, device=G.DEV)
+    bp = wl.Budget(t_base=(0.0, 0.0, 0.0, 0.0))
+    st, dn, ema, arr = ds.api.simulate_budget(*targs, cat, bp, c.server, d["inst"], d["out_off"], 4, n_clients=3)
+    assert ds.device_status() == 0
+    assert arr.tolist() == [0, 0, 0, 2168] and st.tolist() == [6504, 4324, 0, 2168] and dn.tolist() == [8708, 6504, 2168, 4324]
+    with pytest.raises(ds.DsError):
+        ds.api.simulate_budget(*targs, cat, bp, c.server, d["inst"], d["out_off"], 4, n_clients=3, think_ticks=-5)
