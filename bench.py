@@ -3,7 +3,7 @@
 
 A step = one pass of every SURVEY.md §8(a) row over BASELINE.json:configs[1] (policy sweep: 1024 traces x 2000
 requests x 5 policies x 2 estimators = 10 240 instances, 20.48 M simulated requests, 1.13 GB of prompt text):
-ds_characterize -> ds_simulate -> ds_latencies -> 4 x ds_tail_stats.  Prints ONE JSON line.
+ds_characterize -> ds_simulate -> ds_latency_stats (fused latencies + percentiles).  Prints ONE JSON line.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--traces T]
 """
@@ -263,6 +263,13 @@ def run_ours(args):
         line["roofline"] = {"kernel": "simulate_kernel<1>", "bound": "alu", "achieved": ach, "peak": issue_peak,
                             "unit": "Gwarp-inst/s", "frac": ach / issue_peak, "traffic": _traffic().get("simulate_kernel"),
                             "note": "achieved = ncu-counted executed warp instructions per sim-request x sim-requests / live duration"}
+        alu = _k2_inst_per_simreq(1)
+        if alu is not None:
+            # DESIGN.md §6.1/§6.2: measured on this GPU, an ALU-pipe instruction (16 lanes/clk per scheduler) holds the issue
+            # port for two cycles, everything else for one: issue cycles per request = instructions + ALU instructions.
+            cyc = (ipr + alu) * n_sim / (sim_ms * 1e-3) / 1e9
+            line["roofline"]["issue_cycles"] = {"achieved": cyc, "peak": issue_peak, "unit": "Gcycle/s", "frac": cyc / issue_peak,
+                                                "alu_inst_per_request": alu}
     else:
         line["roofline"] = {"kernel": "simulate_kernel<1>", "bound": "alu", "achieved": None, "peak": issue_peak,
                             "unit": "Gwarp-inst/s", "frac": None, "traffic": None}
@@ -314,10 +321,11 @@ def scan_leg(dev, gib, hbm_peak):
             "algorithmic_bytes": int(nbytes)}
 
 
-def _k2_inst_per_simreq():
+def _k2_inst_per_simreq(col=0):
+    """col 0: executed warp instructions per simulated request; col 1: those of them on the ALU pipe (ncu SASS counts)."""
     p = os.path.join(ROOT, "paper_2606_02982_b200", "k2_inst_per_simreq.txt")
     try:
-        return float(open(p).read().split()[0])
+        return float(open(p).read().split()[col])
     except Exception:
         return None
 
