@@ -58,7 +58,7 @@ def _o():
         lib.oracle_queue_depth.restype = C.c_int
         lib.oracle_simulate_budget.argtypes = [p, p, p, p, p, C.c_int64, p, p, p, p, p, p, p]
         lib.oracle_simulate_budget.restype = C.c_int
-        lib.oracle_simulate_closed.argtypes = [p, p, p, p, C.c_int64, C.c_int64, p, C.c_int64, p, p, p, p, p, p, p, p]
+        lib.oracle_simulate_closed.argtypes = [p, p, p, p, C.c_int64, C.c_int64, C.c_int64, p, C.c_int64, p, p, p, p, p, p, p, p]
         lib.oracle_simulate_closed.restype = C.c_int
         lib.oracle_latencies.argtypes = [p, p, C.c_int64, p, p, p, p, p, p, p, p, p]
         lib.oracle_tail_stats.argtypes = [p, p, C.c_int64, C.c_int32, p, C.c_int32, p, p]
@@ -202,7 +202,7 @@ def queue_depth(trace_off, arrival, tier, words, tokens, out_len, instances, out
 
 
 def simulate_budget(trace_off, arrival, tier, words, tokens, out_len, category, budget, server, instances, out_off=None,
-                    want_traj=False, want_est=False, n_clients=0, think_ticks=0):
+                    want_traj=False, want_est=False, n_clients=0, think_ticks=0, batch_wait=0):
     """Full Eq. 1-2 estimator with per-category feedback. budget: object with t_base[4], s_tenant[3], f_slope, f_max.
     Returns start_tick, done_tick, ema_final[n_inst,4] (then ema_traj[samples,4] if want_traj, then est if want_est)."""
     tr, keep = _traces(trace_off, arrival, tier, words, tokens, out_len)
@@ -227,7 +227,8 @@ def simulate_budget(trace_off, arrival, tier, words, tokens, out_len, category, 
     est = np.full(total, -1, np.int64) if want_est else None
     if n_clients > 0:   # closed loop: also returns the arrival tick of every simulated request (last element)
         arr_out = np.full(total, -1, np.int64)
-        rc = _o().oracle_simulate_closed(C.byref(tr), _p(cat), C.byref(bp), C.byref(sv), int(n_clients), int(think_ticks), _p(inst),
+        rc = _o().oracle_simulate_closed(C.byref(tr), _p(cat), C.byref(bp), C.byref(sv), int(n_clients), int(think_ticks), int(batch_wait),
+                                         _p(inst),
                                          n_inst, _p(out_off), _p(arr_out), _p(start), _p(done), _p(ema), _p(toff), _p(traj), _p(est))
         if rc:
             raise ValueError("oracle_simulate_closed: contract violation")

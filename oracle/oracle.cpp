@@ -152,7 +152,7 @@ struct Sim {
 }  // namespace
 
 static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const oracle_budget* bp, const oracle_server* sv,
-                         int64_t n_clients, int64_t think_ticks, int64_t* arrival_out,
+                         int64_t n_clients, int64_t think_ticks, int64_t batch_wait, int64_t* arrival_out,
                          const oracle_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t* start_tick,
                          int64_t* done_tick, double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out) {
   const int nb = bp ? 4 : 3;   // factors per instance: semantic categories (budget estimators) or tenant tiers
@@ -162,6 +162,7 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
     for (int t = 0; t < 3; ++t) if (!(bp->s_tenant[t] > 0.0)) return -1;
     if (!(bp->f_slope >= 0.0) || !(bp->f_max >= 1.0)) return -1;
   }
+  if (batch_wait < 0) return -1;
   if (n_clients < 0 || think_ticks < 0 || (n_clients > 0 && !arrival_out)) return -1;
   if (sv->max_batch < 1) return -1;
   if (sv->weight[0] < 1 || sv->weight[1] < 1 || sv->weight[2] < 1) return -1;
@@ -216,7 +217,12 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
       while (s.next < s.released && s.arr[s.next] <= s.now) s.admit_to_queue(s.next++);
       // 4. ADMIT
       int64_t prefill_new = 0;
-      while ((int64_t)s.R.size() < sv->max_batch && !s.queued.empty()) {
+      // batch-wait ("batch wait interval of 0.01 seconds before dispatching"; reading B6): an IDLE server
+      // dispatches only once max_batch requests are queued or the oldest queued request has waited batch_wait ticks
+      bool gated = false;
+      if (batch_wait > 0 && s.R.empty() && !s.queued.empty() && (int64_t)s.queued.size() < sv->max_batch &&
+          s.now < s.arr[s.queued.front()] + batch_wait) gated = true;
+      while (!gated && (int64_t)s.R.size() < sv->max_batch && !s.queued.empty()) {
         int wpos = 0;
         size_t qi = s.peek(&wpos);
         int64_t c = s.queued[qi];
@@ -230,6 +236,13 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
       }
       // 5. IDLE / END
       if (s.R.empty()) {
+        if (gated) {                             // wake at the gate's deadline or at the next arrival, whichever is first
+          int64_t t = s.arr[s.queued.front()] + batch_wait;
+          if (s.next < s.released && s.arr[s.next] < t) t = s.arr[s.next];
+          s.now = t;
+          skip_to_ingest_now = true;
+          continue;
+        }
         if (s.next == n) break;
         if (s.next >= s.released) return -1;   // unreachable: an empty server means every submitted request completed
         s.now = s.arr[s.next];
@@ -254,7 +267,7 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
 extern "C" int oracle_simulate(const oracle_traces* tr, const oracle_server* sv, const oracle_instance* inst,
                                int64_t n_inst, const int64_t* out_off, int64_t* start_tick, int64_t* done_tick,
                                double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out) {
-  return simulate_impl(tr, nullptr, nullptr, sv, 0, 0, nullptr, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out);
+  return simulate_impl(tr, nullptr, nullptr, sv, 0, 0, 0, nullptr, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out);
 }
 
 extern "C" int oracle_simulate_budget(const oracle_traces* tr, const uint8_t* category, const oracle_budget* bp,
@@ -262,16 +275,17 @@ extern "C" int oracle_simulate_budget(const oracle_traces* tr, const uint8_t* ca
                                       int64_t* start_tick, int64_t* done_tick, double* ema_final, const int64_t* traj_off,
                                       double* ema_traj, int64_t* est_out) {
   if (!bp) return -1;
-  return simulate_impl(tr, category, bp, sv, 0, 0, nullptr, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out);
+  return simulate_impl(tr, category, bp, sv, 0, 0, 0, nullptr, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out);
 }
 
 extern "C" int oracle_simulate_closed(const oracle_traces* tr, const uint8_t* category, const oracle_budget* bp,
-                                      const oracle_server* sv, int64_t n_clients, int64_t think_ticks, const oracle_instance* inst,
+                                      const oracle_server* sv, int64_t n_clients, int64_t think_ticks, int64_t batch_wait,
+                                      const oracle_instance* inst,
                                       int64_t n_inst, const int64_t* out_off, int64_t* arrival_out, int64_t* start_tick,
                                       int64_t* done_tick, double* ema_final, const int64_t* traj_off, double* ema_traj,
                                       int64_t* est_out) {
   if (!bp || n_clients < 1) return -1;
-  return simulate_impl(tr, category, bp, sv, n_clients, think_ticks, arrival_out, inst, n_inst, out_off, start_tick, done_tick,
+  return simulate_impl(tr, category, bp, sv, n_clients, think_ticks, batch_wait, arrival_out, inst, n_inst, out_off, start_tick, done_tick,
                        ema_final, traj_off, ema_traj, est_out);
 }
 

@@ -92,3 +92,49 @@ def test_sjf_lowers_the_median_under_the_paper_setup():
 def test_contract():
     with pytest.raises(ValueError):
         _run([[0, 0, 1, 1, 1]], server(), wl.FIFO, n_clients=1, think=-1)
+
+
+def test_batch_wait_hand_trace():
+    # PAPER.md:302 batch wait (reading B6). max_batch 2, W = 10000, O = 1, kv off. S(alone) = 2150 + 6P; pair: 2300 + 6(P1+P2).
+    # r0 @0, r1 @3000: the batch fills at 3000 (< 0 + W) -> both start at 3000, done 3000 + 2300 + 6*3 = 5318.
+    # r2 @20000 alone: idle server waits until 30000, done 30000 + 2150 + 18 = 32168.
+    # r3 @32168 arrives on the completion tick of r2: idle again -> waits for r4 @33000 (fills the batch) -> both at 33000.
+    req = [[0, 1, 1, 1, 1], [3000, 1, 1, 2, 1], [20000, 1, 1, 3, 1], [32168, 1, 1, 4, 1], [33000, 1, 1, 5, 1]]
+    req = np.asarray(req, np.int64)
+    inst = np.zeros(1, wl.INSTANCE_DTYPE); inst[0] = (0, wl.FIFO, wl.BUDGET_EXACT, 0, 0.0)
+    tr = ([0, 5], req[:, 0], req[:, 1], req[:, 2], req[:, 3], req[:, 4])
+    bp = wl.Budget(t_base=(0.0, 0.0, 0.0, 0.0))
+    st, dn, ema, arr = oracle.simulate_budget(*tr, np.zeros(5, np.uint8), bp, server(max_batch=2), inst, n_clients=5, batch_wait=10_000)
+    assert arr.tolist() == req[:, 0].tolist()
+    assert st.tolist() == [3000, 3000, 30000, 33000, 33000]
+    assert dn.tolist() == [5318, 5318, 32168, 33000 + 2300 + 54, 33000 + 2300 + 54]
+    # W = 0: no gate
+    st0, dn0, _, _ = oracle.simulate_budget(*tr, np.zeros(5, np.uint8), bp, server(max_batch=2), inst, n_clients=5)
+    assert st0.tolist() == [0, 3000, 20000, 32168, 34342]          # r4 joins at the boundary after r3's only iteration (2150 + 24)
+
+
+@pytest.mark.parametrize("policy", wl.ALL_POLICIES)
+def test_batch_wait_gate_property(policy):
+    # checked from the outputs alone: whenever requests start on an idle server (nothing running across tick t), either the
+    # batch was full or the oldest queued request had waited W; and such a start happens exactly at that deadline, at the
+    # arrival that filled the batch, or at a completion tick (the server went idle with requests already queued)
+    sv = wl.Server(max_batch=4, kv_budget=0, aging_step=30_000)
+    c = wl._trace_workload("t", 29, 1, 500, sv, [(policy, wl.BUDGET_SPLIT, 0.1)], oracle.characterize, rho=0.3)   # often idle
+    cat, out_len = wl.assign_categories(29, c.out_len)
+    tr = (c.trace_off, c.arrival, c.tier, c.words, c.tokens, out_len)
+    W = 10_000
+    st, dn, ema, arr = oracle.simulate_budget(*tr, cat, wl.Budget(), sv, c.instances, n_clients=500, batch_wait=W)
+    assert np.array_equal(arr, c.arrival) and (st >= arr).all()
+    n_idle = 0
+    for t in np.unique(st):
+        if ((st < t) & (dn > t)).any():
+            continue                                           # server busy across t: continuous batching, no gate
+        n_idle += 1
+        q = np.flatnonzero((arr <= t) & (st >= t))             # queued at t (completions at t have retired)
+        oldest = arr[q].min()
+        assert len(q) >= sv.max_batch or t >= oldest + W
+        fill = np.sort(arr[q])[sv.max_batch - 1] if len(q) >= sv.max_batch else -1
+        assert t == oldest + W or t == fill or (dn == t).any()
+    assert n_idle > 50
+    st0 = oracle.simulate_budget(*tr, cat, wl.Budget(), sv, c.instances, n_clients=500)[0]
+    assert (st != st0).any()
