@@ -155,9 +155,12 @@ int ds_simulate_budget(const ds_traces* tr, const uint8_t* category, const ds_bu
  * factors. n_clients >= 1, think_ticks >= 0 (host values; DS_EINVAL otherwise); n_clients >= trace length = the open loop.
  * arrival_out [out_off[n_inst]] int64 device (written): the arrival tick of every simulated request - per instance,
  * because arrivals now depend on the policy; latencies are done_tick - arrival_out / start_tick - arrival_out.
+ * batch_wait_ticks >= 0 ("batch wait interval of 0.01 seconds before dispatching"; 0 = none; reading B6): an
+ * IDLE server does not start at the first queued request's arrival a but when max_batch requests are queued or at
+ * a + batch_wait_ticks, whichever is first; a busy server admits at every iteration boundary as before.
  * Everything else as ds_simulate_budget. */
 int ds_simulate_closed(const ds_traces* tr, const uint8_t* category, const ds_budget* bp, const ds_server* sv, int32_t n_clients,
-                       int64_t think_ticks, const ds_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t* arrival_out,
+                       int64_t think_ticks, int64_t batch_wait_ticks, const ds_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t* arrival_out,
                        int64_t* start_tick, int64_t* done_tick, double* ema_final, const int64_t* traj_off, double* ema_traj,
                        int64_t* est_out, void* workspace, size_t workspace_bytes, void* stream);
 

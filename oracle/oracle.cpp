@@ -64,6 +64,7 @@ struct Sim {
   const uint8_t* cat = nullptr; const oracle_budget* bp = nullptr;   // budget estimators only (Eq. 1-2 in full)
   // closed loop ("50 concurrent clients"): requests [released, n) have not been submitted yet
   std::vector<int64_t> arr_dyn; int64_t released = 0, think = 0; bool closed = false;
+  int64_t collect_start = -1;        // batch-wait: tick at which the idle dispatcher started collecting (-1: not collecting)
   // state (SURVEY.md §8(c) C.2 "State per instance")
   int64_t now = 0, next = 0, kv_used = 0, done = 0;
   double B[4] = {1.0, 1.0, 1.0, 1.0};   // per tier (estimators 0/1) or per semantic category (budget estimators)
@@ -217,11 +218,16 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
       while (s.next < s.released && s.arr[s.next] <= s.now) s.admit_to_queue(s.next++);
       // 4. ADMIT
       int64_t prefill_new = 0;
-      // batch-wait ("batch wait interval of 0.01 seconds before dispatching"; reading B6): an IDLE server
-      // dispatches only once max_batch requests are queued or the oldest queued request has waited batch_wait ticks
+      // batch-wait ("batch wait interval of 0.01 seconds before dispatching"; reading B6): when the server is
+      // IDLE and a request is queued, the dispatcher collects for at most batch_wait ticks: it dispatches as soon as
+      // max_batch requests are queued or batch_wait ticks after the collection started (= the first boundary at which
+      // the server is idle with a non-empty queue: the tick it went idle, or the first arrival after that)
       bool gated = false;
-      if (batch_wait > 0 && s.R.empty() && !s.queued.empty() && (int64_t)s.queued.size() < sv->max_batch &&
-          s.now < s.arr[s.queued.front()] + batch_wait) gated = true;
+      if (batch_wait > 0 && s.R.empty() && !s.queued.empty()) {
+        if (s.collect_start < 0) s.collect_start = s.now;
+        if ((int64_t)s.queued.size() < sv->max_batch && s.now < s.collect_start + batch_wait) gated = true;
+        else s.collect_start = -1;
+      }
       while (!gated && (int64_t)s.R.size() < sv->max_batch && !s.queued.empty()) {
         int wpos = 0;
         size_t qi = s.peek(&wpos);
@@ -237,7 +243,7 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
       // 5. IDLE / END
       if (s.R.empty()) {
         if (gated) {                             // wake at the gate's deadline or at the next arrival, whichever is first
-          int64_t t = s.arr[s.queued.front()] + batch_wait;
+          int64_t t = s.collect_start + batch_wait;
           if (s.next < s.released && s.arr[s.next] < t) t = s.arr[s.next];
           s.now = t;
           skip_to_ingest_now = true;

@@ -68,8 +68,9 @@ int oracle_simulate_budget(const oracle_traces* tr, const uint8_t* category, con
  * the next request of the trace arrive at  completion tick + think_ticks. Same-tick ordering as everywhere: completions,
  * then same-tick arrivals (R-ORD). arrival_out [out_off[n_inst]]: the arrival tick of every simulated request (per
  * instance: arrivals now depend on the policy). Estimator and feedback as in oracle_simulate_budget.
- * batch_wait ("batch wait interval of 0.01 seconds before dispatching"; 0 = none): an IDLE server does not
- * start at the first arrival a but at min(a + batch_wait, arrival of the max_batch-th request from there). */
+ * batch_wait ("batch wait interval of 0.01 seconds before dispatching"; 0 = none): an IDLE server with a
+ * queued request collects for at most batch_wait ticks: it dispatches when max_batch requests are queued or batch_wait
+ * ticks after the collection started (the tick it went idle with a non-empty queue, else the first arrival after). */
 int oracle_simulate_closed(const oracle_traces* tr, const uint8_t* category, const oracle_budget* bp, const oracle_server* sv,
                            int64_t n_clients, int64_t think_ticks, int64_t batch_wait, const oracle_instance* inst, int64_t n_inst,
                            const int64_t* out_off, int64_t* arrival_out, int64_t* start_tick, int64_t* done_tick,

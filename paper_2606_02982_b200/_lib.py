@@ -52,7 +52,7 @@ def lib():
         L.ds_simulate.argtypes = [C.POINTER(DsTraces), C.POINTER(DsServer), p, i64, p, p, p, p, p, p, p, sz, p]
         L.ds_simulate_est.argtypes = [C.POINTER(DsTraces), C.POINTER(DsServer), p, i64, p, p, p, p, p, p, p, p, sz, p]
         L.ds_simulate_budget.argtypes = [C.POINTER(DsTraces), p, C.POINTER(DsBudget), C.POINTER(DsServer), p, i64, p, p, p, p, p, p, p, p, sz, p]
-        L.ds_simulate_closed.argtypes = [C.POINTER(DsTraces), p, C.POINTER(DsBudget), C.POINTER(DsServer), i32, i64, p, i64, p, p, p, p, p, p, p, p, p, sz, p]
+        L.ds_simulate_closed.argtypes = [C.POINTER(DsTraces), p, C.POINTER(DsBudget), C.POINTER(DsServer), i32, i64, i64, p, i64, p, p, p, p, p, p, p, p, p, sz, p]
         L.ds_estimation_error.argtypes = [C.POINTER(DsTraces), p, i64, p, p, p, p, i32, p, p, p]
         L.ds_queue_depth.argtypes = [C.POINTER(DsTraces), p, i64, p, p, i64, i64, i64, p, p]
         L.ds_latencies.argtypes = [C.POINTER(DsTraces), p, i64, p, i64, p, p, p, p, p, p, p, p, p]

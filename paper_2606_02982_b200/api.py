@@ -214,7 +214,7 @@ def queue_depth(trace_off, arrival, tier, words, tokens, out_len, inst, out_off,
 
 def simulate_budget(trace_off, arrival, tier, words, tokens, out_len, category, budget, server, inst, out_off, n_total,
                     start=None, done=None, ema_final=None, traj_off=None, ema_traj=None, est_out=None, workspace=None,
-                    n_clients=0, think_ticks=0, arrival_out=None):
+                    n_clients=0, think_ticks=0, arrival_out=None, batch_wait=0):
     """ds_simulate_budget. category uint8 CUDA tensor (per request); budget: object with t_base[4], s_tenant[3], f_slope,
     f_max. Returns (start_tick, done_tick, ema_final[n_inst,4])."""
     tr = _traces(trace_off, arrival, tier, words, tokens, out_len)
@@ -237,7 +237,7 @@ def simulate_budget(trace_off, arrival, tier, words, tokens, out_len, category, 
             arrival_out = torch.empty(n_total, dtype=torch.int64, device=dev)
         _need_cuda(arrival_out)
         check("ds_simulate_closed", lib().ds_simulate_closed(C.byref(tr), _ptr(category), C.byref(bp), C.byref(sv), int(n_clients),
-                                                             int(think_ticks), _ptr(inst), n_inst, _ptr(out_off), _ptr(arrival_out),
+                                                             int(think_ticks), int(batch_wait), _ptr(inst), n_inst, _ptr(out_off), _ptr(arrival_out),
                                                              _ptr(start), _ptr(done), _ptr(ema_final), _ptr(traj_off), _ptr(ema_traj),
                                                              _ptr(est_out), _ptr(workspace), workspace.numel(), _stream()))
         return start, done, ema_final, arrival_out

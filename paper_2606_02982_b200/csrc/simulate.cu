@@ -45,6 +45,7 @@ struct Params {
   double* ema_final; const int64_t* traj_off; double* ema_traj; int64_t* est_out;
   const uint8_t* category; ds_budget bp;   // budget estimators only (ds_simulate_budget)
   int32_t n_clients; int64_t think; int64_t* arrival_out;   // closed-loop arrivals (ds_simulate_closed), n_clients = 0: open loop
+  int64_t batch_wait;                                        // ds_simulate_closed: dispatch gate of an idle server (0 = none)
   unsigned long long* heap_ws; unsigned int* counter; unsigned int* status; const unsigned int* perm;
 };
 
@@ -154,6 +155,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   long long fifo_est = 0;
   unsigned iter = 0, dist = 0xffffffffu;
   bool blocked = false;
+  long long collect = -1;                // batch-wait: tick at which the idle dispatcher started collecting (-1: not collecting)
   double Bl = 1.0;                       // lane t < 3 holds B[t]
   int s_idx[kSlots]; unsigned s_fin[kSlots];   // per lane: running requests
 #pragma unroll
@@ -336,6 +338,14 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
 
   // 4. ADMIT: while a slot is free, peek(policy, now); KV check on the estimate (A8); pop
   auto admit = [&]() {
+    // batch-wait gate (reading B6): an idle server with a queued request collects for at most batch_wait
+    // ticks from `collect` (the first boundary at which it is idle with a non-empty queue) and dispatches as soon as
+    // max_batch requests are queued. Idle => everything started has completed, so next - done requests are queued.
+    if (kBudget && p.batch_wait > 0 && b == 0) {
+      if (collect < 0) collect = now;
+      if (next - done < max_batch && now < collect + p.batch_wait) return;
+      collect = -1;
+    }
     while (b < max_batch) {
       int c = -1, ct = 0, wpos = 0; long long est_c = 0;
       if (kPolicy == DS_FIFO) {
@@ -411,6 +421,17 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
     }
     if (!blocked && b < max_batch && queue_nonempty()) admit();           // 4. ADMIT
     if (b == 0) {                                                         // 5. IDLE / END
+      if (kBudget && p.batch_wait > 0) {
+        // the gate's closed form: first queued (or next arriving) request q0 -> dispatch at min(arrival[q0] + wait,
+        // arrival of the request that fills the batch); unsubmitted requests of a closed loop read as +inf
+        const int qc = next - done;                                       // queued (gated) requests
+        if (qc == 0) { if (next >= n) break; collect = an; }              // collection starts at the first arrival
+        long long t = collect + p.batch_wait;
+        const int kf = next + (max_batch - qc) - 1;                       // the arrival that fills the batch
+        if (kf < n) { const long long tf = arr_at(kf); if (tf < t) t = tf; }
+        now = t > now ? t : now;
+        continue;
+      }
       if (next >= n) break;
       now = an;
       continue;
@@ -587,7 +608,7 @@ size_t ws_simulate(int64_t total_requests, int64_t n_inst) {
 
 }  // namespace ds
 static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_budget* bp, int32_t n_clients, int64_t think_ticks,
-                         int64_t* arrival_out, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
+                         int64_t batch_wait, int64_t* arrival_out, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
                          const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
                          const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace, size_t workspace_bytes,
                          void* stream) {
@@ -617,8 +638,8 @@ static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_
   p.traj_every = sv->traj_every;
   p.inst = inst; p.n_inst = n_inst; p.out_off = out_off; p.start_tick = start_tick; p.done_tick = done_tick;
   p.ema_final = ema_final; p.traj_off = traj_off; p.ema_traj = ema_traj; p.est_out = est_out;
-  p.category = category; p.n_clients = n_clients; p.think = think_ticks; p.arrival_out = arrival_out;
-  if (n_clients < 0 || think_ticks < 0 || (n_clients > 0 && (!bp || !arrival_out))) return DS_EINVAL;
+  p.category = category; p.n_clients = n_clients; p.think = think_ticks; p.arrival_out = arrival_out; p.batch_wait = batch_wait;
+  if (batch_wait < 0 || n_clients < 0 || think_ticks < 0 || (n_clients > 0 && (!bp || !arrival_out))) return DS_EINVAL;
   if (bp) p.bp = *bp; else memset(&p.bp, 0, sizeof(p.bp));
   p.counter = (unsigned int*)workspace;
   unsigned int* perm = (unsigned int*)((char*)workspace + 256);
@@ -659,7 +680,7 @@ static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_
 extern "C" int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
                            const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
                            const int64_t* traj_off, double* ema_traj, void* workspace, size_t workspace_bytes, void* stream) {
-  return simulate_impl(tr, nullptr, nullptr, 0, 0, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, nullptr, workspace,
+  return simulate_impl(tr, nullptr, nullptr, 0, 0, 0, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, nullptr, workspace,
                        workspace_bytes, stream);
 }
 
@@ -668,7 +689,7 @@ extern "C" int ds_simulate_est(const ds_traces* tr, const ds_server* sv, const d
                                const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace,
                                size_t workspace_bytes, void* stream) {
   if (n_inst > 0 && !est_out) return DS_EINVAL;
-  return simulate_impl(tr, nullptr, nullptr, 0, 0, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out, workspace,
+  return simulate_impl(tr, nullptr, nullptr, 0, 0, 0, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out, workspace,
                        workspace_bytes, stream);
 }
 
@@ -677,16 +698,17 @@ extern "C" int ds_simulate_budget(const ds_traces* tr, const uint8_t* category, 
                                   int64_t* done_tick, double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out,
                                   void* workspace, size_t workspace_bytes, void* stream) {
   if (!bp) return DS_EINVAL;
-  return simulate_impl(tr, category, bp, 0, 0, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj,
+  return simulate_impl(tr, category, bp, 0, 0, 0, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj,
                        est_out, workspace, workspace_bytes, stream);
 }
 
 extern "C" int ds_simulate_closed(const ds_traces* tr, const uint8_t* category, const ds_budget* bp, const ds_server* sv,
-                                  int32_t n_clients, int64_t think_ticks, const ds_instance* inst, int64_t n_inst,
+                                  int32_t n_clients, int64_t think_ticks, int64_t batch_wait_ticks, const ds_instance* inst,
+                                  int64_t n_inst,
                                   const int64_t* out_off, int64_t* arrival_out, int64_t* start_tick, int64_t* done_tick,
                                   double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace,
                                   size_t workspace_bytes, void* stream) {
   if (!bp || n_clients < 1) return DS_EINVAL;
-  return simulate_impl(tr, category, bp, n_clients, think_ticks, arrival_out, sv, inst, n_inst, out_off, start_tick, done_tick,
+  return simulate_impl(tr, category, bp, n_clients, think_ticks, batch_wait_ticks, arrival_out, sv, inst, n_inst, out_off, start_tick, done_tick,
                        ema_final, traj_off, ema_traj, est_out, workspace, workspace_bytes, stream);
 }

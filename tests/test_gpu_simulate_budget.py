@@ -188,3 +188,49 @@ def test_closed_loop_hand_trace_and_contract(G):
     assert arr.tolist() == [0, 0, 0, 2168] and st.tolist() == [6504, 4324, 0, 2168] and dn.tolist() == [8708, 6504, 2168, 4324]
     with pytest.raises(ds.DsError):
         ds.api.simulate_budget(*targs, cat, bp, c.server, d["inst"], d["out_off"], 4, n_clients=3, think_ticks=-5)
+
+
+@pytest.mark.parametrize("rho,n_clients,W,max_batch", [(0.3, 600, 10_000, 4), (0.6, 600, 10_000, 32), (0.3, 600, 3_000, 1),
+                                                      (1.0, 40, 10_000, 32), (0.5, 600, 50_000, 64)])
+def test_batch_wait(G, rho, n_clients, W, max_batch):
+    import paper_2606_02982_b200 as ds
+    sv = wl.Server(max_batch=max_batch, kv_budget=6000, aging_step=40_000)
+    combos = [(p, wl.BUDGET_SPLIT, 0.1) for p in wl.ALL_POLICIES]
+    c = wl._trace_workload("t", 61 + max_batch, 2, 600, sv, combos, oracle.characterize, rho=rho)
+    cat, out_len = wl.assign_categories(61, c.out_len)
+    arrival = c.arrival.copy()
+    if n_clients < 600:
+        arrival[:] = 0
+    tr = (c.trace_off, arrival, c.tier, c.words, c.tokens, out_len)
+    ost, odn, oema, oest, oarr = oracle.simulate_budget(*tr, cat, wl.Budget(), sv, c.instances, out_off=c.out_off, want_est=True,
+                                                        n_clients=n_clients, batch_wait=W)
+    ost0 = oracle.simulate_budget(*tr, cat, wl.Budget(), sv, c.instances, out_off=c.out_off, n_clients=n_clients)[0]
+    if n_clients >= 600:
+        assert (ost != ost0).any() == (max_batch > 1)  # the gate changes something on this shape (never with batch 1)
+    d = G.upload(c)
+    d["out_len"] = torch.from_numpy(out_len).to(G.DEV)
+    d["arrival"] = torch.from_numpy(arrival).to(G.DEV)
+    targs = (d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"])
+    n_total = int(c.out_off[-1])
+    est = torch.full((n_total,), -1, dtype=torch.int64, device=G.DEV)
+    st, dn, ema, arr = ds.api.simulate_budget(*targs, torch.from_numpy(cat).to(G.DEV), wl.Budget(), sv, d["inst"], d["out_off"], n_total,
+                                              est_out=est, n_clients=n_clients, batch_wait=W)
+    assert ds.device_status() == 0
+    for name, a, b in (("arrival", arr, oarr), ("start", st, ost), ("done", dn, odn), ("est", est, oest)):
+        a = a.cpu().numpy()
+        bad = np.flatnonzero(a != b)
+        assert bad.size == 0, (name, bad[:5], a[bad[:5]], b[bad[:5]], c.instances[bad[:5] // 600])
+    assert np.array_equal(ema.cpu().numpy().view(np.uint64), oema.view(np.uint64))
+
+
+def test_batch_wait_hand_trace(G):
+    import paper_2606_02982_b200 as ds
+    req = [[0, 1, 1, 1, 1], [3000, 1, 1, 2, 1], [20000, 1, 1, 3, 1], [32168, 1, 1, 4, 1], [33000, 1, 1, 5, 1]]
+    c = G.tiny_workload(wl, req, wl.Server(max_batch=2, kv_budget=0), [(wl.FIFO, wl.BUDGET_EXACT, 0.0)])
+    d = G.upload(c)
+    targs = (d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"])
+    cat = torch.zeros(5, dtype=torch.uint8, device=G.DEV)
+    st, dn, ema, arr = ds.api.simulate_budget(*targs, cat, wl.Budget(t_base=(0.0, 0.0, 0.0, 0.0)), c.server, d["inst"], d["out_off"], 5,
+                                              n_clients=5, batch_wait=10_000)
+    assert ds.device_status() == 0
+    assert st.tolist() == [3000, 3000, 30000, 33000, 33000] and dn.tolist() == [5318, 5318, 32168, 35354, 35354]

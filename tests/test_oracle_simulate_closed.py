@@ -116,8 +116,8 @@ def test_batch_wait_hand_trace():
 @pytest.mark.parametrize("policy", wl.ALL_POLICIES)
 def test_batch_wait_gate_property(policy):
     # checked from the outputs alone: whenever requests start on an idle server (nothing running across tick t), either the
-    # batch was full or the oldest queued request had waited W; and such a start happens exactly at that deadline, at the
-    # arrival that filled the batch, or at a completion tick (the server went idle with requests already queued)
+    # batch was full or W ticks had passed since the collection started (the later of: the tick the server went idle, the
+    # oldest queued arrival); and such a start happens exactly at that deadline or when the batch filled
     sv = wl.Server(max_batch=4, kv_budget=0, aging_step=30_000)
     c = wl._trace_workload("t", 29, 1, 500, sv, [(policy, wl.BUDGET_SPLIT, 0.1)], oracle.characterize, rho=0.3)   # often idle
     cat, out_len = wl.assign_categories(29, c.out_len)
@@ -131,10 +131,11 @@ def test_batch_wait_gate_property(policy):
             continue                                           # server busy across t: continuous batching, no gate
         n_idle += 1
         q = np.flatnonzero((arr <= t) & (st >= t))             # queued at t (completions at t have retired)
-        oldest = arr[q].min()
-        assert len(q) >= sv.max_batch or t >= oldest + W
+        went_idle = dn[st < t].max() if (st < t).any() else 0  # tick at which the server last went idle
+        cs = max(arr[q].min(), went_idle)                      # collection start: idle with a non-empty queue
+        assert len(q) >= sv.max_batch or t >= cs + W
         fill = np.sort(arr[q])[sv.max_batch - 1] if len(q) >= sv.max_batch else -1
-        assert t == oldest + W or t == fill or (dn == t).any()
+        assert t == cs + W or t == max(fill, went_idle)
     assert n_idle > 50
     st0 = oracle.simulate_budget(*tr, cat, wl.Budget(), sv, c.instances, n_clients=500)[0]
     assert (st != st0).any()
