@@ -234,3 +234,37 @@ def test_batch_wait_hand_trace(G):
                                               n_clients=5, batch_wait=10_000)
     assert ds.device_status() == 0
     assert st.tolist() == [3000, 3000, 30000, 33000, 33000] and dn.tolist() == [5318, 5318, 32168, 35354, 35354]
+
+
+def test_paper_setup_closed_loop_tables(G):
+    # 3000 requests, 50 concurrent clients, batch 32, batch wait 0.01 s, three runs; five policies x the three
+    # estimator modes of Table IX. End-to-end on the GPU: closed-loop simulation -> P50/P95/P99 of the end-to-end latency
+    # per (policy, mode) (Table VI's columns) -> error sums; all bit-exact against the oracle.
+    import paper_2606_02982_b200 as ds
+    c, cat, bp = wl.paper_phases(oracle.characterize)
+    arrival = np.zeros_like(c.arrival)
+    tr = (c.trace_off, arrival, c.tier, c.words, c.tokens, c.out_len)
+    ost, odn, oema, oest, oarr = oracle.simulate_budget(*tr, cat, bp, c.server, c.instances, out_off=c.out_off, want_est=True,
+                                                        n_clients=50, batch_wait=10_000)
+    d = G.upload(c)
+    d["arrival"] = torch.from_numpy(arrival).to(G.DEV)
+    targs = (d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"])
+    n_total = int(c.out_off[-1])
+    est = torch.empty(n_total, dtype=torch.int64, device=G.DEV)
+    st, dn, ema, arr = ds.api.simulate_budget(*targs, torch.from_numpy(cat).to(G.DEV), bp, c.server, d["inst"], d["out_off"], n_total,
+                                              est_out=est, n_clients=50, batch_wait=10_000)
+    assert ds.device_status() == 0
+    assert np.array_equal(arr.cpu().numpy(), oarr) and np.array_equal(st.cpu().numpy(), ost) and np.array_equal(dn.cpu().numpy(), odn)
+    assert np.array_equal(ema.cpu().numpy().view(np.uint64), oema.view(np.uint64))
+    seg_h = np.repeat(c.group, c.n_req).astype(np.int32)                # one segment per (policy, mode), runs pooled
+    pct = (50, 95, 99)
+    want, wcnt = oracle.tail_stats(odn - oarr, seg_h, c.n_groups, pct)
+    got, gcnt = ds.tail_stats(dn - arr, torch.from_numpy(seg_h).to(G.DEV), c.n_groups, pct)
+    assert np.array_equal(got.cpu().numpy(), want) and np.array_equal(gcnt.cpu().numpy(), wcnt)
+    osum = oracle.estimation_error(*tr, c.instances, c.out_off, oest, ost, c.group, c.n_groups)
+    gsum = ds.api.estimation_error(*targs, d["inst"], d["out_off"], n_total, est, st, d["group"], c.n_groups)
+    assert np.array_equal(gsum.cpu().numpy()[:, :8], osum[:, :8])       # (queue-wait sums use tr.arrival: not the closed-loop ones)
+    # the paper's headline on its own setup: SJF lowers the median end-to-end latency against FIFO
+    g = {c.extra["combos"][k]: k for k in range(c.n_groups)}
+    fifo, sjf = g[(wl.FIFO, wl.BUDGET_SPLIT, 0.1)], g[(wl.SJF, wl.BUDGET_SPLIT, 0.1)]
+    assert want[sjf, 0] < 0.8 * want[fifo, 0]
