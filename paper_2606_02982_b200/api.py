@@ -245,3 +245,12 @@ def simulate_budget(trace_off, arrival, tier, words, tokens, out_len, category, 
                                                          _ptr(out_off), _ptr(start), _ptr(done), _ptr(ema_final), _ptr(traj_off),
                                                          _ptr(ema_traj), _ptr(est_out), _ptr(workspace), workspace.numel(), _stream()))
     return start, done, ema_final
+
+
+def simulate_closed(trace_off, arrival, tier, words, tokens, out_len, category, budget, server, n_clients, think_ticks, batch_wait,
+                    inst, out_off, n_total, **kw):
+    """ds_simulate_closed -> (start_tick, done_tick, ema_final[n_inst,4], arrival_out)."""
+    if n_clients < 1:
+        raise ValueError("ds_simulate_closed: n_clients >= 1")
+    return simulate_budget(trace_off, arrival, tier, words, tokens, out_len, category, budget, server, inst, out_off, n_total,
+                           n_clients=n_clients, think_ticks=think_ticks, batch_wait=batch_wait, **kw)
