@@ -32,6 +32,10 @@ namespace ds {
 namespace k2 {
 
 constexpr int kWarpsPerBlock = 4;
+#ifndef DS_K2_MIN_BLOCKS
+#define DS_K2_MIN_BLOCKS 6   // resident 128-thread blocks per SM the register allocation is bounded for (measured: 7 and 8
+                             // spill and gain nothing: 13.27 / 13.62 ms against 13.26 ms; 5, 4, 3 blocks: 14.9 / 17.2 / 20.7 ms)
+#endif
 constexpr int kHeapSmem = 256;  // heap entries cached in shared memory per warp
 constexpr long long kInf = 0x7fffffffffffffffLL;
 constexpr unsigned kFull = 0xffffffffu;
@@ -542,7 +546,7 @@ __global__ void __launch_bounds__(1024) order_kernel(const ds_instance* __restri
 }
 
 template <int kSlots, bool kBudget = false>
-__global__ void __launch_bounds__(k2::kWarpsPerBlock * 32) simulate_kernel(const __grid_constant__ Params p) {
+__global__ void __launch_bounds__(k2::kWarpsPerBlock * 32, DS_K2_MIN_BLOCKS) simulate_kernel(const __grid_constant__ Params p) {
   constexpr int kFac = kBudget ? 4 : 3;
   __shared__ unsigned long long heap_sm[kWarpsPerBlock][kHeapSmem];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
