@@ -423,7 +423,13 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       if (an <= limit) ingest(limit);                                     // 1. INGEST-EARLY / 3. INGEST-NOW
       if (ph == 0 && dist == 0) retire();                                 // 2. RETIRE
     }
-    if (!blocked && b < max_batch && queue_nonempty()) admit();           // 4. ADMIT
+    // 4. ADMIT. admit() returns with the batch full, the queue empty or (every policy but AGING) `blocked` set, so
+    // afterwards something can still be admitted at the next boundary only under AGING (levels change with time)
+    bool can_admit = !blocked && b < max_batch && queue_nonempty();
+    if (can_admit) {
+      admit();
+      can_admit = kPolicy == DS_AGING && !blocked && b < max_batch && queue_nonempty();
+    }
     if (b == 0) {                                                         // 5. IDLE / END
       if (kBudget && p.batch_wait > 0) {
         // the gate's closed form: first queued (or next arriving) request q0 -> dispatch at min(arrival[q0] + wait,
@@ -447,7 +453,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
     prefill_new = 0;
     kv_used += (unsigned)b; dt += cb; --dist; ++iter;
     // boundaries at which nothing can happen: no completion, and no arrival that could be admitted
-    if (dist != 0 && !(!blocked && b < max_batch && queue_nonempty())) {
+    if (dist != 0 && !can_admit) {
       const bool arrivals_matter = b < max_batch && !(kPolicy == DS_FIFO && blocked) && next < n;
       // tick of the last boundary before the completion boundary: the stepping loop "while (an > now) step" runs all
       // `dist` iterations iff an > t_last
