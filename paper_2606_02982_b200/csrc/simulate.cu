@@ -283,8 +283,8 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       int lm = 0x7fffffff;
 #pragma unroll
       for (int s = 0; s < kSlots; ++s) if (s_idx[s] >= 0 && s_fin[s] == iter) lm = min(lm, s_idx[s]);
-      const int r = __reduce_min_sync(kFull, lm);
-      if (r == 0x7fffffff) break;
+      const int r = __reduce_min_sync(kFull, lm);             // called with dist == 0: at least one request completes now
+      if (r == 0x7fffffff) { dist = 0xffffffffu; break; }     // (defensive: cannot happen; never spin or index with it)
 #pragma unroll
       for (int s = 0; s < kSlots; ++s) if (s_idx[s] == r) s_idx[s] = -1;
       const int Pr = P[r], Or = max(O[r], 1);
@@ -325,12 +325,15 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
         __syncwarp();
       }
       if (traj && done % p.traj_every == 0 && lane < kFac) traj[kFac * (done / p.traj_every - 1) + lane] = Bl;
+      // distance to the next completion; 0 = another request completes at this same boundary (one reduction serves as
+      // both the loop test and the result)
+      unsigned d = 0xffffffffu;
+#pragma unroll
+      for (int s = 0; s < kSlots; ++s) if (s_idx[s] >= 0) d = min(d, s_fin[s] - iter);
+      dist = __reduce_min_sync(kFull, d);
+      if (dist != 0) break;
     }
     blocked = false;
-    unsigned d = 0xffffffffu;
-#pragma unroll
-    for (int s = 0; s < kSlots; ++s) if (s_idx[s] >= 0) d = min(d, s_fin[s] - iter);
-    dist = __reduce_min_sync(kFull, d);
     __syncwarp();
   };
 
