@@ -25,7 +25,7 @@ sys.path.insert(0, ROOT)
 METRIC = "simulated requests/sec (policy x trace)"
 UNIT = "req/s"
 # The issue-slot roofline of ds_simulate uses the executed warp instructions per simulated request measured with ncu
-# (paper_2606_02982_b200/k2_inst_per_simreq.txt, from profiles/r01_ncu_k2_v3.txt); DRAM traffic per launch comes from
+# (paper_2606_02982_b200/k2_inst_per_simreq.txt, from profiles/r01_ncu_k2_v4.txt); DRAM traffic per launch comes from
 # the same captures (profiles/r01_traffic.json.txt).
 
 
