@@ -18,6 +18,19 @@ struct Ws {               // header at the start of the workspace
   unsigned long long and_bits, or_bits;
   unsigned int any;
 };
+// Digits are aligned to the highest bit on which the keys differ (diff = AND ^ OR of all keys): pass j = 0, 1, ... covers
+// bits [top - 8(j+1), top - 8j) clamped at 0, top = number of low bits that vary. A fixed alignment (bits 56-63, 48-55, ...)
+// wastes a full-cost pass on a top digit that carries one or two bits (25-bit latencies: bits 24-31 hold one bit).
+struct DigitPos { int lo, width; bool active; };
+__device__ __forceinline__ int vary_top(unsigned long long diff) { return diff ? 64 - __clzll((long long)diff) : 0; }
+__device__ __forceinline__ DigitPos digit_pos(unsigned long long diff, int j) {
+  DigitPos p;
+  const int hi_end = vary_top(diff) - 8 * j;
+  p.active = hi_end > 0;
+  p.lo = hi_end > 8 ? hi_end - 8 : 0;
+  p.width = p.active ? hi_end - p.lo : 0;
+  return p;
+}
 // layout: Ws | counts[n_seg] u64 | prefix[n_seg*n_pct] u64 | rank[n_seg*n_pct] u64 | hist[n_seg*n_pct*256] u32
 struct Layout {
   Ws* hdr; unsigned long long* counts; unsigned long long* prefix; unsigned long long* rank; unsigned int* hist;
@@ -103,7 +116,7 @@ __global__ void __launch_bounds__(512) count_kernel(const int64_t* __restrict__ 
 
 struct Pcts { int p[kMaxPct]; };
 
-__global__ void init_kernel(const unsigned long long* counts, int n_seg, int n_pct, Pcts pc, unsigned long long* prefix,
+__global__ void init_kernel(const unsigned long long* counts, int n_seg, int n_pct, Pcts pc, const Ws* hdr, unsigned long long* prefix,
                             unsigned long long* rank, int64_t* count_out) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n_seg * n_pct) return;
@@ -112,7 +125,8 @@ __global__ void init_kernel(const unsigned long long* counts, int n_seg, int n_p
   unsigned long long r = ((unsigned long long)pc.p[q] * c + 99ull) / 100ull;   // nearest rank (A13)
   if (r < 1) r = 1;
   if (r > c) r = c;
-  prefix[i] = 0; rank[i] = r;
+  const int top = vary_top(hdr->and_bits ^ hdr->or_bits);           // the bits above `top` are common to all keys
+  prefix[i] = (hdr->any && top < 64) ? hdr->and_bits >> top : 0ull; rank[i] = r;
   if (q == 0 && count_out) count_out[s] = (int64_t)c;
 }
 
@@ -120,13 +134,14 @@ __global__ void init_kernel(const unsigned long long* counts, int n_seg, int n_p
 template <bool kPriv>
 __global__ void __launch_bounds__(512) hist_kernel(const int64_t* __restrict__ v, const int32_t* __restrict__ seg, long long n, int n_seg,
                             int n_pct, int d, const Ws* hdr, const unsigned long long* __restrict__ prefix, unsigned int* hist) {
-  const unsigned long long diff = hdr->and_bits ^ hdr->or_bits;
-  if (!hdr->any || ((diff >> (8 * d)) & 0xffull) == 0) return;   // every key has the same digit here: skipped
+  const DigitPos dp = digit_pos(hdr->and_bits ^ hdr->or_bits, 7 - d);
+  if (!hdr->any || !dp.active) return;                           // no varying bits left for this pass
   extern __shared__ unsigned int sh[];
   const int nb = n_seg * n_pct * 256;
   if (kPriv) { for (int i = threadIdx.x; i < nb; i += blockDim.x) sh[i] = 0; __syncthreads(); }
   unsigned int* bins = kPriv ? sh : hist;
-  const int shift = 8 * d;
+  const int shift = dp.lo, hshift = dp.lo + dp.width;
+  const unsigned dmask = (1u << dp.width) - 1u;
   const long long stride = (long long)gridDim.x * blockDim.x;
   for (long long base = blockIdx.x * (long long)blockDim.x; base < n; base += stride * kUnroll) {   // block-uniform trip count
     int sv[kUnroll]; unsigned long long kv[kUnroll];
@@ -140,8 +155,8 @@ __global__ void __launch_bounds__(512) hist_kernel(const int64_t* __restrict__ v
     for (int u = 0; u < kUnroll; ++u) {
       const bool ok = sv[u] >= 0 && sv[u] < n_seg;
       const int s = ok ? sv[u] : 0;
-      const unsigned long long hi = d == 7 ? 0ull : (kv[u] >> (shift + 8));
-      const unsigned dig = (unsigned)(kv[u] >> shift) & 0xffu;
+      const unsigned long long hi = hshift >= 64 ? 0ull : (kv[u] >> hshift);
+      const unsigned dig = (unsigned)(kv[u] >> shift) & dmask;
       for (int q = 0; q < n_pct; ++q)
         agg_add(bins, ok && hi == prefix[s * n_pct + q], (unsigned)((s * n_pct + q) * 256) + dig);
     }
@@ -154,11 +169,10 @@ __global__ void select_kernel(int n_seg, int n_pct, int d, const Ws* hdr, const 
                               unsigned long long* prefix, unsigned long long* rank, unsigned int* hist, int64_t* out) {
   const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (i >= n_seg * n_pct) return;
-  const unsigned long long diff = hdr->and_bits ^ hdr->or_bits;
-  const bool skip = !hdr->any || ((diff >> (8 * d)) & 0xffull) == 0;
+  const DigitPos dp = digit_pos(hdr->and_bits ^ hdr->or_bits, 7 - d);
+  const bool skip = !hdr->any || !dp.active;
   unsigned long long pf = prefix[i];
-  if (skip) pf = (pf << 8) | ((hdr->and_bits >> (8 * d)) & 0xffull);
-  else {
+  if (!skip) {
     uint4* h4 = reinterpret_cast<uint4*>(hist + (size_t)i * 256 + lane * 8);
     const uint4 x = h4[0], y = h4[1];
     h4[0] = make_uint4(0, 0, 0, 0); h4[1] = make_uint4(0, 0, 0, 0);   // ready for the next digit
@@ -189,7 +203,7 @@ __global__ void select_kernel(int n_seg, int n_pct, int d, const Ws* hdr, const 
     const int digit = __shfl_sync(0xffffffffu, lane * 8 + dig, src);
     const unsigned long long bef = __shfl_sync(0xffffffffu, before, src);
     if (lane == 0) rank[i] = r - bef;
-    pf = (pf << 8) | (unsigned long long)digit;
+    pf = (pf << dp.width) | (unsigned long long)digit;
   }
   if (lane == 0) {
     prefix[i] = pf;
@@ -213,14 +227,16 @@ __global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pc
   extern __shared__ unsigned int sh[];
   const int n_seg = 4 * a.n_groups;
   const int nb = kCount ? n_seg : n_seg * n_pct * 256;
+  DigitPos dp; dp.lo = 0; dp.width = 0; dp.active = true;
   if (!kCount) {
-    const unsigned long long diff = hdr->and_bits ^ hdr->or_bits;
-    if (!hdr->any || ((diff >> (8 * d)) & 0xffull) == 0) return;   // every key has the same digit here: skipped
+    dp = digit_pos(hdr->and_bits ^ hdr->or_bits, 7 - d);
+    if (!hdr->any || !dp.active) return;                           // no varying bits left for this pass
   }
   for (int i = threadIdx.x; i < nb; i += blockDim.x) sh[i] = 0;
   __syncthreads();
   unsigned long long kand = ~0ull, kor = 0ull; bool any = false;
-  const int shift = 8 * d;
+  const int shift = dp.lo, hshift = dp.lo + dp.width;
+  const unsigned dmask = (1u << dp.width) - 1u;
   // one WARP per instance: the dependent header loads (instance -> trace -> offsets) of 16 warps per block overlap
   const int lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
   for (long long ii = (long long)blockIdx.x * nwarp + (threadIdx.x >> 5); ii < a.n_inst; ii += (long long)gridDim.x * nwarp) {
@@ -249,8 +265,8 @@ __global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pc
           agg_add(sh, ok, s_t);
           agg_add(sh, ok, s_a);
         } else {
-          const unsigned long long hi = d == 7 ? 0ull : (k >> (shift + 8));
-          const unsigned dig = (unsigned)(k >> shift) & 0xffu;
+          const unsigned long long hi = hshift >= 64 ? 0ull : (k >> hshift);
+          const unsigned dig = (unsigned)(k >> shift) & dmask;
           for (int q = 0; q < n_pct; ++q) {
             agg_add(sh, ok && hi == prefix[s_t * n_pct + q], (s_t * n_pct + q) * 256 + dig);
             agg_add(sh, ok && hi == prefix[s_a * n_pct + q], (s_a * n_pct + q) * 256 + dig);
@@ -310,7 +326,7 @@ extern "C" int ds_tail_stats(const int64_t* values, const int32_t* seg_id, int64
   if (blocks < 1) blocks = 1;
   const size_t csm = n_segments <= 4096 ? sizeof(unsigned) * (size_t)n_segments : 0;
   k3::count_kernel<<<(unsigned)blocks, threads, csm, s>>>(values, seg_id, n, n_segments, L.hdr, L.counts);
-  k3::init_kernel<<<(nsq + 255) / 256, 256, 0, s>>>(L.counts, n_segments, n_pct, pc, L.prefix, L.rank, count_out);
+  k3::init_kernel<<<(nsq + 255) / 256, 256, 0, s>>>(L.counts, n_segments, n_pct, pc, L.hdr, L.prefix, L.rank, count_out);
   note_launch(2);
   const size_t hsm = sizeof(unsigned) * 256 * (size_t)nsq;
   const bool priv = hsm <= 160 * 1024;
@@ -368,7 +384,7 @@ extern "C" int ds_latency_stats(const ds_traces* tr, const ds_instance* inst, in
     DS_CUDA(cudaMemsetAsync(workspace, 0, L.total, s));
     DS_CUDA(cudaMemsetAsync(&L.hdr->and_bits, 0xff, 8, s));
     if (n_inst == 0) {   // all segments empty
-      k3::init_kernel<<<(nsq + 255) / 256, 256, 0, s>>>(L.counts, n_seg, n_pct, pc, L.prefix, L.rank, count_out);
+      k3::init_kernel<<<(nsq + 255) / 256, 256, 0, s>>>(L.counts, n_seg, n_pct, pc, L.hdr, L.prefix, L.rank, count_out);
       k3::select_kernel<<<(nsq + 3) / 4, 128, 0, s>>>(n_seg, n_pct, 0, L.hdr, L.counts, L.prefix, L.rank, L.hist, out);
       note_launch(2);
       continue;
@@ -376,7 +392,7 @@ extern "C" int ds_latency_stats(const ds_traces* tr, const ds_instance* inst, in
     k3::LatArgs a{tr->trace_off, tr->arrival_tick, tr->tier, inst, out_off, metric == 0 ? done_tick : start_tick, group, t_mid,
                   (long long)n_inst, G};
     k3::lat_pass_kernel<true><<<(unsigned)blocks, 512, sizeof(unsigned) * (size_t)n_seg, s>>>(a, n_pct, 0, L.hdr, L.counts, L.prefix, L.hist);
-    k3::init_kernel<<<(nsq + 255) / 256, 256, 0, s>>>(L.counts, n_seg, n_pct, pc, L.prefix, L.rank, count_out);
+    k3::init_kernel<<<(nsq + 255) / 256, 256, 0, s>>>(L.counts, n_seg, n_pct, pc, L.hdr, L.prefix, L.rank, count_out);
     note_launch(2);
     for (int d = 7; d >= 0; --d) {
       k3::lat_pass_kernel<false><<<(unsigned)blocks, 512, hsm, s>>>(a, n_pct, d, L.hdr, L.counts, L.prefix, L.hist);
