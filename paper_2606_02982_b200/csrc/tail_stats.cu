@@ -83,6 +83,7 @@ __device__ __forceinline__ void agg_add(unsigned int* bins, bool pred, unsigned 
   else if (pred && bin != lead_bin) atomicAdd(&bins[bin], 1u);
 }
 
+constexpr int kMaxSegPct = 200;   // (segments x percentiles) of the fused pass: 200 KB of shared-memory histograms at most
 constexpr int kUnroll = 4;   // independent 12-byte loads in flight per thread
 
 __global__ void __launch_bounds__(512) count_kernel(const int64_t* __restrict__ v, const int32_t* __restrict__ seg, long long n, int n_seg,
@@ -233,6 +234,8 @@ __global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pc
     if (!hdr->any || !dp.active) return;                           // no varying bits left for this pass
   }
   for (int i = threadIdx.x; i < nb; i += blockDim.x) sh[i] = 0;
+  __shared__ unsigned long long pfx_s[kMaxSegPct];                  // the prefixes, read 2 x n_pct times per key
+  if (!kCount) for (int i = threadIdx.x; i < n_seg * n_pct; i += blockDim.x) pfx_s[i] = prefix[i];
   __syncthreads();
   unsigned long long kand = ~0ull, kor = 0ull; bool any = false;
   const int shift = dp.lo, hshift = dp.lo + dp.width;
@@ -267,9 +270,17 @@ __global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pc
         } else {
           const unsigned long long hi = hshift >= 64 ? 0ull : (k >> hshift);
           const unsigned dig = (unsigned)(k >> shift) & dmask;
+          // which of the key's (segment, percentile) prefixes it matches: bit q = tier segment, bit 8+q = "all" segment.
+          // After the first pass almost no key matches anything: one vote rejects the whole warp.
+          unsigned mm = 0;
           for (int q = 0; q < n_pct; ++q) {
-            agg_add(sh, ok && hi == prefix[s_t * n_pct + q], (s_t * n_pct + q) * 256 + dig);
-            agg_add(sh, ok && hi == prefix[s_a * n_pct + q], (s_a * n_pct + q) * 256 + dig);
+            mm |= (ok && hi == pfx_s[s_t * n_pct + q]) ? (1u << q) : 0u;
+            mm |= (ok && hi == pfx_s[s_a * n_pct + q]) ? (256u << q) : 0u;
+          }
+          if (!__any_sync(0xffffffffu, mm != 0u)) continue;
+          for (int q = 0; q < n_pct; ++q) {
+            agg_add(sh, (mm >> q) & 1u, (s_t * n_pct + q) * 256 + dig);
+            agg_add(sh, (mm >> (8 + q)) & 1u, (s_a * n_pct + q) * 256 + dig);
           }
         }
       }
