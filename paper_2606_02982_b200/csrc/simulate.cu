@@ -190,7 +190,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       if (w_cat > 3) { atomicOr(p.status, DS_DEV_BAD_TRACE); w_cat = 3; }
     }
     const long long prev = __shfl_up_sync(kFull, w_arr, 1);
-    const bool bad = (i < n) && (w_tier > 2 || w_base < 0 || w_arr < 0 || (lane > 0 && w_arr < prev));
+    const bool bad = (i < n) && (w_tier > 2 || w_base < 0 || w_arr < 0 || (lane > 0 && w_arr < prev) || O[i] < 1);   // (out_len checked here, 32 at a time)
     if (bad) atomicOr(p.status, DS_DEV_BAD_TRACE);
     if (w_tier > 2) w_tier = 2;
     if (w_base < 0) w_base = 0;
@@ -401,8 +401,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
         if (kPolicy == DS_WEIGHTED) { cur = wpos + 1; if (cur >= wtot) cur = 0; }
       }
       const int Pc = P[c];
-      int Oc = O[c];
-      if (Oc < 1) { Oc = 1; if (lane == 0) atomicOr(p.status, DS_DEV_BAD_TRACE); }
+      const int Oc = max(O[c], 1);                             // (a bad out_len was reported when its window was loaded)
       st[c] = now;                                             // every lane, same address and value
       bool has_free = false;                                   // first lane with a free slot takes the request
 #pragma unroll
