@@ -54,7 +54,7 @@ extern "C" int oracle_characterize(const uint8_t* bytes, int64_t n_bytes, const 
 
 namespace {
 
-enum { FIFO = 0, PRIORITY = 1, WEIGHTED = 2, SJF = 3, AGING = 4 };
+enum { FIFO = 0, PRIORITY = 1, WEIGHTED = 2, SJF = 3, AGING = 4, AGING_UNCLAMPED = 5 };
 enum { SPLIT = 0, EXACT = 1, BUDGET_SPLIT = 2, BUDGET_EXACT = 3 };
 
 struct Sim {
@@ -139,8 +139,11 @@ struct Sim {
         case PRIORITY: k0 = tier[r]; break;                         // (tier, seq)
         case SJF: k0 = est[r]; break;                               // (est, seq)
         default: {                                                  // AGING (A10)
+          // PAPER.md:242 "waiting time progressively reduces the effective scheduling score". AGING clamps the score
+          // at Premium's level (A10); AGING_UNCLAMPED (reading A15) lets it fall below 0, so
+          // among long waiters the tier order survives instead of degenerating to arrival order.
           int64_t lv = (now - arr[r]) / sv->aging_step;
-          int64_t eff = (int64_t)tier[r] - lv; if (eff < 0) eff = 0;
+          int64_t eff = (int64_t)tier[r] - lv; if (eff < 0 && policy == AGING) eff = 0;
           k0 = eff;
         }
       }
@@ -170,7 +173,7 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
   if (sv->aging_step < 1) return -1;
   for (int64_t ii = 0; ii < n_inst; ++ii) {
     const oracle_instance& in = inst[ii];
-    if (in.trace < 0 || in.trace >= tr->n_traces || in.policy < 0 || in.policy > 4 || !(in.ema_alpha >= 0.0 && in.ema_alpha <= 1.0))
+    if (in.trace < 0 || in.trace >= tr->n_traces || in.policy < 0 || in.policy > AGING_UNCLAMPED || !(in.ema_alpha >= 0.0 && in.ema_alpha <= 1.0))
       return -1;
     if (bp ? (in.estimator != BUDGET_SPLIT && in.estimator != BUDGET_EXACT) : (in.estimator != SPLIT && in.estimator != EXACT)) return -1;
     int64_t lo = tr->trace_off[in.trace], n = tr->trace_off[in.trace + 1] - lo;

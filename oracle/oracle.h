@@ -36,6 +36,8 @@ typedef struct {
   int32_t traj_every;
 } oracle_server;
 
+/* policy: 0 FIFO, 1 PRIORITY, 2 WEIGHTED, 3 SJF, 4 AGING (score clamped at Premium's level, A10),
+ *         5 AGING_UNCLAMPED (A15: score = tier - floor(waited/aging_step), no clamp) */
 typedef struct { int32_t trace, policy, estimator, _pad; double ema_alpha; } oracle_instance;
 
 /* Budget estimators (estimator 2: T_input = words, 3: T_input = tokens), Eq. 1-2 of the paper in full. */

@@ -19,9 +19,10 @@ _SO = os.path.join(_HERE, "libdsgen.so")
 _SRC = os.path.join(_HERE, "gen.cpp")
 
 FIFO, PRIORITY, WEIGHTED, SJF, AGING = 0, 1, 2, 3, 4
+AGING_UNCLAMPED = 5   # NEXT-4 variant (A15): the aging score is not clamped at Premium's level
 SPLIT, EXACT = 0, 1
 BUDGET_SPLIT, BUDGET_EXACT = 2, 3
-POLICY_NAMES = ["FIFO", "PRIORITY", "WEIGHTED", "SJF", "AGING"]
+POLICY_NAMES = ["FIFO", "PRIORITY", "WEIGHTED", "SJF", "AGING", "AGING_UNCLAMPED"]
 
 # layout of ds_instance in include/driftsched.h (24 bytes)
 INSTANCE_DTYPE = np.dtype(
