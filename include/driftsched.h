@@ -86,7 +86,8 @@ typedef struct {              /* continuous-batching server model, BASELINE.json
 #define DS_PRIORITY 1 /* PAPER.md:202-204, 228-230 */
 #define DS_WEIGHTED 2 /* PAPER.md:232-240 */
 #define DS_SJF 3      /* PAPER.md:231 */
-#define DS_AGING 4    /* PAPER.md:242 */
+#define DS_AGING 4    /* PAPER.md:242; score max(0, tier - floor(waited/aging_step)) (DESIGN.md A10) */
+#define DS_AGING_UNCLAMPED 5 /* PAPER.md:242, variant (A15): score tier - floor(waited/aging_step), no clamp */
 #define DS_SPLIT 0    /* estimate base = words  (split() proxy) */
 #define DS_EXACT 1    /* estimate base = tokens (tokenizer-aware) */
 #define DS_BUDGET_SPLIT 2 /* ds_simulate_budget only: full Eq. 1-2 estimator, T_input = words  */
@@ -94,7 +95,7 @@ typedef struct {              /* continuous-batching server model, BASELINE.json
 
 typedef struct {
   int32_t trace;     /* index into ds_traces */
-  int32_t policy;    /* DS_FIFO .. DS_AGING */
+  int32_t policy;    /* DS_FIFO .. DS_AGING_UNCLAMPED */
   int32_t estimator; /* DS_SPLIT / DS_EXACT (ds_simulate, ds_simulate_est); DS_BUDGET_* (ds_simulate_budget) */
   int32_t _pad;
   double ema_alpha;  /* EMA learning rate in [0,1] (Eq. 5); 0 = BIAS OFF */

@@ -123,7 +123,8 @@ struct TierCursor {
 template <int kSlots, int kPolicy, bool kSmall, bool kBudget>
 __device__ __forceinline__ void run_instance(const Params& p, const unsigned inst_id, const int trace, const bool split, const double alpha,
                                           unsigned long long* heap_sm, const int lane) {
-  constexpr bool kCursor = kPolicy == DS_PRIORITY || kPolicy == DS_WEIGHTED || kPolicy == DS_AGING;
+  constexpr bool kAging = kPolicy == DS_AGING || kPolicy == DS_AGING_UNCLAMPED;   // both read the heads' arrival ticks
+  constexpr bool kCursor = kPolicy == DS_PRIORITY || kPolicy == DS_WEIGHTED || kAging;
   const long long lo = p.trace_off[trace];
   const long long n64 = p.trace_off[trace + 1] - lo;
   if (n64 < 0 || n64 > 0x7ffffff0ll || (kPolicy == DS_SJF && n64 > (1 << 24))) {   // local indices are 32-bit (SJF keys: 24-bit)
@@ -211,7 +212,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
     c.head = c.blk * 32 + (__ffs(c.mask) - 1);
     if (c.head < next) {   // already arrived: its frozen estimate sits in the done_tick scratch
       if (use_kv) c.est = (long long)__ldcg(dn + c.head);
-      if (kPolicy == DS_AGING) c.arr = arr_at(c.head);
+      if (kAging) c.arr = arr_at(c.head);
     }
   };
   if (kCursor)
@@ -264,7 +265,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
           for (int t = 0; t < 3; ++t) {
             if (tc[t].head >= next && tc[t].head < last) {   // warp-uniform
               if (use_kv) tc[t].est = shfl_i64(est, tc[t].head - wb);
-              if (kPolicy == DS_AGING) tc[t].arr = shfl_i64(w_arr, tc[t].head - wb);
+              if (kAging) tc[t].arr = shfl_i64(w_arr, tc[t].head - wb);
             }
           }
         }
@@ -375,6 +376,15 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
         }
 #pragma unroll
         for (int t = 0; t < 3; ++t) if (t == ct) { c = tc[t].head; est_c = tc[t].est; }
+      } else if (kPolicy == DS_AGING_UNCLAMPED) {  // A15: eff = tier - floor(waited/aging_step), not clamped; key (eff, seq)
+        long long best_eff = 0;
+#pragma unroll
+        for (int t = 0; t < 3; ++t) {
+          if (tc[t].head < next) {                 // a head has the longest wait of its tier, so the minimum is among the heads
+            const long long eff = (long long)t - (now - tc[t].arr) / p.aging_step;
+            if (c < 0 || eff < best_eff || (eff == best_eff && tc[t].head < c)) { best_eff = eff; c = tc[t].head; est_c = tc[t].est; ct = t; }
+          }
+        }
       } else {  // AGING (A10): eff = max(0, tier - floor(waited/aging_step)); key (eff, seq)
         int best_eff = 99;
 #pragma unroll
@@ -389,7 +399,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
         }
       }
       if (c < 0) break;
-      if (b > 0 && use_kv && (long long)kv_used + est_c > p.kv_budget) { blocked = kPolicy != DS_AGING; break; }   // deferred (A8)
+      if (b > 0 && use_kv && (long long)kv_used + est_c > p.kv_budget) { blocked = !kAging; break; }   // deferred (A8)
       // pop
       if (kPolicy == DS_FIFO) {
         ++fifo_head;
@@ -430,7 +440,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
     bool can_admit = !blocked && b < max_batch && queue_nonempty();
     if (can_admit) {
       admit();
-      can_admit = kPolicy == DS_AGING && !blocked && b < max_batch && queue_nonempty();
+      can_admit = kAging && !blocked && b < max_batch && queue_nonempty();
     }
     if (b == 0) {                                                         // 5. IDLE / END
       if (kBudget && p.batch_wait > 0) {
@@ -518,7 +528,7 @@ __global__ void __launch_bounds__(1024) order_kernel(const ds_instance* __restri
   __shared__ unsigned int cnt[6], pos[6];
   if (threadIdx.x < 6) cnt[threadIdx.x] = 0;
   __syncthreads();
-  auto bucket = [](int policy) { return policy == DS_SJF ? 0 : policy == DS_AGING ? 1 : policy == DS_WEIGHTED ? 2 :
+  auto bucket = [](int policy) { return policy == DS_SJF ? 0 : (policy == DS_AGING || policy == DS_AGING_UNCLAMPED) ? 1 : policy == DS_WEIGHTED ? 2 :
                                         policy == DS_PRIORITY ? 3 : policy == DS_FIFO ? 4 : 5; };
   for (long long i = threadIdx.x; i < n_inst; i += blockDim.x) atomicAdd(&cnt[bucket(inst[i].policy)], 1u);
   __syncthreads();
@@ -587,7 +597,7 @@ __global__ void __launch_bounds__(k2::kWarpsPerBlock * 32, DS_K2_MIN_BLOCKS) sim
     const unsigned inst_id = p.perm[b0 + k];
     const ds_instance in = p.inst[inst_id];
     const int est_lo = kBudget ? DS_BUDGET_SPLIT : DS_SPLIT;          // this kernel's pair of estimators
-    const bool bad_inst = in.trace < 0 || in.trace >= p.n_traces || in.policy < 0 || in.policy > 4 || in.estimator < est_lo ||
+    const bool bad_inst = in.trace < 0 || in.trace >= p.n_traces || in.policy < 0 || in.policy > DS_AGING_UNCLAMPED || in.estimator < est_lo ||
                           in.estimator > est_lo + 1 || !(in.ema_alpha >= 0.0 && in.ema_alpha <= 1.0);
     if (bad_inst) {
       if (lane == 0) atomicOr(p.status, DS_DEV_BAD_INSTANCE);
@@ -605,7 +615,8 @@ __global__ void __launch_bounds__(k2::kWarpsPerBlock * 32, DS_K2_MIN_BLOCKS) sim
       case DS_PRIORITY: DS_RUN(DS_PRIORITY); break;
       case DS_WEIGHTED: DS_RUN(DS_WEIGHTED); break;
       case DS_SJF: DS_RUN(DS_SJF); break;
-      default: DS_RUN(DS_AGING); break;
+      case DS_AGING: DS_RUN(DS_AGING); break;
+      default: DS_RUN(DS_AGING_UNCLAMPED); break;
     }
 #undef DS_RUN
   }
