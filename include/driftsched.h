@@ -154,6 +154,9 @@ int ds_simulate_budget(const ds_traces* tr, const uint8_t* category, const ds_bu
  * (in completion order: tick, then request index) lets the next request of the trace arrive at completion tick +
  * think_ticks. Same-tick order as everywhere (R-ORD): completions, then same-tick arrivals, which therefore see the updated
  * factors. n_clients >= 1, think_ticks >= 0 (host values; DS_EINVAL otherwise); n_clients >= trace length = the open loop.
+ * Contract: the arrival sequence the loop produces must be non-decreasing in request index like every trace's, i.e. the
+ * first n_clients arrival ticks must not lie after the first release (they are all 0 when the paper's clients start
+ * together); a later one sets DS_DEV_BAD_TRACE and the instance's outputs are unspecified.
  * arrival_out [out_off[n_inst]] int64 device (written): the arrival tick of every simulated request - per instance,
  * because arrivals now depend on the policy; latencies are done_tick - arrival_out / start_tick - arrival_out.
  * batch_wait_ticks >= 0 ("batch wait interval of 0.01 seconds before dispatching"; 0 = none; reading B6): an

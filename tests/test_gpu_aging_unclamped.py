@@ -80,6 +80,7 @@ def test_budget_estimator_and_closed_loop(G):
     c = wl._trace_workload("t", 80, 3, 1500, sv, [(wl.AGING_UNCLAMPED, wl.BUDGET_SPLIT, 0.1), (wl.AGING_UNCLAMPED, wl.BUDGET_EXACT, 0.0)],
                            oracle.characterize, rho=1.0)
     cat, out_len = wl.assign_categories(80, c.out_len)
+    arrival = np.zeros_like(c.arrival)               # closed loop: the 50 clients start together; later entries are ignored
     tr = (c.trace_off, c.arrival, c.tier, c.words, c.tokens, out_len)
     d = G.upload(c)
     d["out_len"] = torch.from_numpy(out_len).to(G.DEV)
@@ -87,6 +88,10 @@ def test_budget_estimator_and_closed_loop(G):
     targs = tuple(d[k] for k in ("trace_off", "arrival", "tier", "words", "tokens", "out_len"))
     n_total = int(c.out_off[-1])
     for n_clients, wait in ((0, 0), (50, 0), (50, 10_000)):
+        if n_clients:
+            tr = (c.trace_off, arrival, c.tier, c.words, c.tokens, out_len)
+            d["arrival"] = torch.from_numpy(arrival).to(G.DEV)
+            targs = tuple(d[k] for k in ("trace_off", "arrival", "tier", "words", "tokens", "out_len"))
         o = oracle.simulate_budget(*tr, cat, bp, c.server, c.instances, n_clients=n_clients, batch_wait=wait)
         arr_out = torch.zeros(n_total, dtype=torch.int64, device=G.DEV) if n_clients else None
         r = ds.api.simulate_budget(*targs, dcat, bp, c.server, d["inst"], d["out_off"], n_total, n_clients=n_clients,
