@@ -218,7 +218,11 @@ int ds_tail_stats(const int64_t* values, const int32_t* seg_id, int64_t n, int32
  *   count_out [4*G] nullable: segment sizes in the same order.
  * Same nearest-rank definition and results as the unfused calls (bit-exact). pct: HOST array, n_pct <= 8.
  * Requires 4*G*n_pct <= 200 histograms (shared memory); DS_EINVAL otherwise: use the unfused calls then.
- * workspace: ds_workspace_bytes(DS_WS_TAIL_STATS, 4*G, n_pct). Launches per wanted metric: 2 memsets + 2 + up to 8 x 2 kernels. */
+ * workspace: ds_workspace_bytes(DS_WS_TAIL_STATS, 4*G, n_pct), optionally followed by a staging area of
+ *   ds_workspace_bytes(DS_WS_LATENCY_STAGE, n_total, 0) bytes (n_total = out_off[n_inst]; 5 bytes per simulated request): when
+ *   it is there, out_off tiles [0, n_total) in instance order and every latency is below 2^32 ticks, the count pass stages
+ *   32-bit keys + segment codes and the digit passes stream those instead of recomputing tick - arrival (same results,
+ *   bit-exact; any other case silently takes the unstaged passes). Launches per wanted metric: 2 memsets + 2 + up to 8 x 2 kernels. */
 int ds_latency_stats(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, const int64_t* out_off,
                      const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, int32_t n_groups,
                      const int64_t* t_mid, const int32_t* pct, int32_t n_pct, int64_t* e2e_out, int64_t* qdelay_out,
@@ -227,6 +231,7 @@ int ds_latency_stats(const ds_traces* tr, const ds_instance* inst, int64_t n_ins
 #define DS_WS_CHARACTERIZE 0
 #define DS_WS_SIMULATE 1
 #define DS_WS_TAIL_STATS 2
+#define DS_WS_LATENCY_STAGE 3 /* n = simulated requests over all instances; m unused: optional staging area of ds_latency_stats */
 /* Workspace size in bytes for call `which` with the two size arguments named at that call. Never 0. */
 size_t ds_workspace_bytes(int which, int64_t n, int64_t m);
 

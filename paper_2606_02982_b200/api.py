@@ -176,7 +176,7 @@ def tail_stats(values, seg_id, n_segments, pct=(50, 99), out=None, count_out=Non
 
 
 def latency_stats(trace_off, arrival, tier, words, tokens, out_len, inst, out_off, start, done, group, n_groups, t_mid=None,
-                  pct=(50, 99), e2e_out=None, qdelay_out=None, count_out=None, workspace=None):
+                  pct=(50, 99), e2e_out=None, qdelay_out=None, count_out=None, workspace=None, stage=True):
     """ds_latency_stats -> (e2e_out, qdelay_out, count_out), each laid out [4*G, n_pct] / [4*G] with G = n_groups * phases:
     rows [0, 3G) are the (group, tier) segments 3*g+tier, rows [3G, 4G) the per-group overall segments."""
     tr = _traces(trace_off, arrival, tier, words, tokens, out_len)
@@ -191,8 +191,11 @@ def latency_stats(trace_off, arrival, tier, words, tokens, out_len, inst, out_of
         qdelay_out = torch.empty((4 * G, n_pct), dtype=torch.int64, device=dev)
     if count_out is None:
         count_out = torch.empty(4 * G, dtype=torch.int64, device=dev)
-    if workspace is None:
-        workspace = _workspace(_lib.WS_TAIL_STATS, 4 * G, n_pct, dev)
+    if workspace is None:     # histograms + the optional staging area (5 bytes per simulated request)
+        nbytes = workspace_bytes(_lib.WS_TAIL_STATS, 4 * G, n_pct)
+        if stage:
+            nbytes += workspace_bytes(_lib.WS_LATENCY_STAGE, int((start if start is not None else done).numel()), 0)
+        workspace = torch.empty(nbytes, dtype=torch.uint8, device=dev)
     arr = (C.c_int32 * n_pct)(*[int(x) for x in pct])
     check("ds_latency_stats", lib().ds_latency_stats(C.byref(tr), _ptr(inst), n_inst, _ptr(out_off), _ptr(start), _ptr(done),
                                                      _ptr(group), n_groups, _ptr(t_mid), arr, n_pct, _ptr(e2e_out), _ptr(qdelay_out),

@@ -17,6 +17,7 @@ constexpr unsigned long long kSign = 0x8000000000000000ull;
 struct Ws {               // header at the start of the workspace
   unsigned long long and_bits, or_bits;
   unsigned int any;
+  unsigned int nostage;   // ds_latency_stats: the staged keys are unusable (no room, or out_off is not a partition)
 };
 // Digits are aligned to the highest bit on which the keys differ (diff = AND ^ OR of all keys): pass j = 0, 1, ... covers
 // bits [top - 8(j+1), top - 8j) clamped at 0, top = number of low bits that vary. A fixed alignment (bits 56-63, 48-55, ...)
@@ -219,7 +220,16 @@ __global__ void select_kernel(int n_seg, int n_pct, int d, const Ws* hdr, const 
 struct LatArgs {
   const int64_t* trace_off; const int64_t* arrival; const uint8_t* tier; const ds_instance* inst; const int64_t* out_off;
   const int64_t* ticks; const int32_t* group; const int64_t* t_mid; long long n_inst; int n_groups;   // groups after phases
+  // Staging (optional, the part of the workspace beyond the histograms): the count pass leaves the low 32 bits of every key
+  // and its segment code 3*g+tier (255 = not counted) at the request's output index. When every key agrees on bits 32..63
+  // (latencies below 2^32 ticks = 71 minutes) the digit passes stream these 5 bytes per request linearly - mostly out of
+  // L2 - instead of recomputing tick - arrival per instance (16 B per request and three dependent header loads per
+  // instance, which made a pass that matches nothing cost 100 us for 164 MB).
+  unsigned int* skey; unsigned char* scode; long long cap;
 };
+__device__ __forceinline__ bool stage_usable(const LatArgs& a, const Ws* hdr) {
+  return a.skey != nullptr && !hdr->nostage && vary_top(hdr->and_bits ^ hdr->or_bits) <= 32;
+}
 
 // kCount: segment counts + AND/OR of all keys. Otherwise: digit-d histogram of the keys matching each (segment, pct) prefix.
 template <bool kCount>
@@ -242,6 +252,43 @@ __global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pc
   const unsigned dmask = (1u << dp.width) - 1u;
   // one WARP per instance: the dependent header loads (instance -> trace -> offsets) of 16 warps per block overlap
   const int lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
+  bool stage = a.skey != nullptr;      // count pass: this warp may still write staged keys
+  if (!kCount && stage_usable(a, hdr)) {
+    // staged pass: 4 consecutive requests per thread (one 16-byte + one 4-byte load), the grid strides over the requests
+    const long long n = a.out_off[a.n_inst];
+    const unsigned long long khi = hdr->and_bits & 0xffffffff00000000ull;   // bits 32..63 are common to all keys
+    const unsigned segall0 = 3u * (unsigned)a.n_groups;
+    for (long long i4 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 4; i4 < ((n + 127) & ~127ll);   // warp-uniform trips
+         i4 += (long long)gridDim.x * blockDim.x * 4) {
+      unsigned kk[4]; unsigned cc[4];
+      if (i4 + 3 < n) {
+        const uint4 kv = *reinterpret_cast<const uint4*>(a.skey + i4);
+        const uchar4 cv = *reinterpret_cast<const uchar4*>(a.scode + i4);
+        kk[0] = kv.x; kk[1] = kv.y; kk[2] = kv.z; kk[3] = kv.w; cc[0] = cv.x; cc[1] = cv.y; cc[2] = cv.z; cc[3] = cv.w;
+      } else {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { const bool in = i4 + u < n; kk[u] = in ? a.skey[i4 + u] : 0u; cc[u] = in ? a.scode[i4 + u] : 255u; }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const bool ok = cc[u] != 255u;
+        const unsigned long long k = khi | kk[u];
+        const unsigned s_t = ok ? cc[u] : 0u, s_a = segall0 + ((s_t * 171u) >> 9);   // x/3 for x < 256
+        const unsigned long long hi = hshift >= 64 ? 0ull : (k >> hshift);
+        const unsigned dig = (unsigned)(k >> shift) & dmask;
+        unsigned mm = 0;
+        for (int q = 0; q < n_pct; ++q) {
+          mm |= (ok && hi == pfx_s[s_t * n_pct + q]) ? (1u << q) : 0u;
+          mm |= (ok && hi == pfx_s[s_a * n_pct + q]) ? (256u << q) : 0u;
+        }
+        if (!__any_sync(0xffffffffu, mm != 0u)) continue;
+        for (int q = 0; q < n_pct; ++q) {
+          agg_add(sh, (mm >> q) & 1u, (s_t * n_pct + q) * 256 + dig);
+          agg_add(sh, (mm >> (8 + q)) & 1u, (s_a * n_pct + q) * 256 + dig);
+        }
+      }
+    }
+  } else
   for (long long ii = (long long)blockIdx.x * nwarp + (threadIdx.x >> 5); ii < a.n_inst; ii += (long long)gridDim.x * nwarp) {
     const int t = a.inst[ii].trace;
     const long long lo = a.trace_off[t], n = a.trace_off[t + 1] - lo, oo = a.out_off[ii];
@@ -249,6 +296,16 @@ __global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pc
     const bool ph = a.t_mid != nullptr;
     const long long tm = ph ? a.t_mid[t] : 0;
     const bool gok = g0 >= 0 && (ph ? 2 * g0 + 1 : g0) < a.n_groups;
+    if (kCount && stage) {
+      // the staged passes walk [0, out_off[n_inst]) linearly: the instances' ranges must tile it in order; slots that no
+      // request owns (padding between ranges, before the first one) are marked "not counted"
+      const long long oe = a.out_off[ii + 1], gb = ii == 0 ? 0 : oo;
+      if (oo < 0 || oe < oo + n || oe > a.cap) { if (lane == 0) atomicOr(&hdr->nostage, 1u); stage = false; }
+      else {
+        for (long long j = gb + lane; j < oo; j += 32) a.scode[j] = 255;
+        for (long long j = oo + n + lane; j < oe; j += 32) a.scode[j] = 255;
+      }
+    }
     for (long long base = 0; base < n; base += 32 * kUnroll) {   // warp-uniform trip count
       long long av[kUnroll], tv[kUnroll]; int tr[kUnroll];
 #pragma unroll
@@ -267,6 +324,8 @@ __global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pc
           if (ok) { kand &= k; kor |= k; any = true; }
           agg_add(sh, ok, s_t);
           agg_add(sh, ok, s_a);
+          const long long r = base + u * 32 + lane;
+          if (stage && r < n) { a.skey[oo + r] = (unsigned)k; a.scode[oo + r] = ok ? (unsigned char)s_t : (unsigned char)255; }
         } else {
           const unsigned long long hi = hshift >= 64 ? 0ull : (k >> hshift);
           const unsigned dig = (unsigned)(k >> shift) & dmask;
@@ -300,6 +359,8 @@ __global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pc
 }  // namespace k3
 
 size_t ws_tail_stats(int64_t n_seg, int64_t n_pct) { return k3::make_layout(nullptr, n_seg, n_pct).total; }
+// staging area of ds_latency_stats for n_total simulated requests: u32 keys | u8 segment codes
+size_t ws_latency_stage(int64_t n_total) { return n_total > 0 ? align_up(5 * (size_t)n_total, 256) + 1024 : 0; }   // (the callee keeps 512 for alignment)
 
 }  // namespace ds
 
@@ -401,7 +462,16 @@ extern "C" int ds_latency_stats(const ds_traces* tr, const ds_instance* inst, in
       continue;
     }
     k3::LatArgs a{tr->trace_off, tr->arrival_tick, tr->tier, inst, out_off, metric == 0 ? done_tick : start_tick, group, t_mid,
-                  (long long)n_inst, G};
+                  (long long)n_inst, G, nullptr, nullptr, 0};
+    // whatever the caller's workspace holds beyond the histograms is the staging area (5 bytes per simulated request)
+    const size_t extra = workspace_bytes - L.total;
+    if (extra >= 512 + 5) {
+      long long cap = (long long)((extra - 512) / 5);
+      if (cap > 0xffffffffll) cap = 0xffffffffll;
+      a.cap = cap;
+      a.skey = (unsigned int*)((char*)workspace + L.total);
+      a.scode = (unsigned char*)workspace + L.total + align_up(4 * (size_t)cap, 256);
+    }
     k3::lat_pass_kernel<true><<<(unsigned)blocks, 512, sizeof(unsigned) * (size_t)n_seg, s>>>(a, n_pct, 0, L.hdr, L.counts, L.prefix, L.hist);
     k3::init_kernel<<<(nsq + 255) / 256, 256, 0, s>>>(L.counts, n_seg, n_pct, pc, L.hdr, L.prefix, L.rank, count_out);
     note_launch(2);

@@ -48,7 +48,11 @@ class HotPath:
         self.ws_char = ws(_lib.WS_CHARACTERIZE, 0 if self.text is None else self.text.numel(), c.n_traces * c.n_req)
         self.ws_sim = ws(_lib.WS_SIMULATE, n, self.n_inst)
         G = self.n_groups
-        self.ws_tail = ws(_lib.WS_TAIL_STATS, 4 * G, len(self.pct))
+        # histograms, and for the fused call the staging area behind them (5 bytes per simulated request: 32-bit keys + segment codes)
+        nb = api.workspace_bytes(_lib.WS_TAIL_STATS, 4 * G, len(self.pct))
+        if fused:
+            nb += api.workspace_bytes(_lib.WS_LATENCY_STAGE, n, 0)
+        self.ws_tail = torch.empty(nb, dtype=torch.uint8, device=dev)
         # percentiles: rows [0,3G) = (group, tier) segments, rows [3G,4G) = per-group overall (ds_latency_stats layout)
         self.e2e_stats = torch.empty((4 * G, len(self.pct)), dtype=torch.int64, device=dev)
         self.qd_stats = torch.empty((4 * G, len(self.pct)), dtype=torch.int64, device=dev)

@@ -74,15 +74,16 @@ def _fused_vs_oracle(G, c, pct=(50, 99)):
     Gn = c.n_groups * (2 if c.t_mid is not None else 1)
     d = G.upload(c)
     import torch
-    ge, gq, gc = ds.latency_stats(d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"], d["inst"],
-                                  d["out_off"], torch.from_numpy(st).to(G.DEV), torch.from_numpy(dn).to(G.DEV), d["group"],
-                                  c.n_groups, d["t_mid"], pct)
-    ge, gq, gc = ge.cpu().numpy(), gq.cpu().numpy(), gc.cpu().numpy()
-    for vals, got in ((e2e, ge), (qd, gq)):
-        ot, ct = oracle.tail_stats(vals, seg_t, 3 * Gn, pct)
-        oa, ca = oracle.tail_stats(vals, seg_a, Gn, pct)
-        assert np.array_equal(got[:3 * Gn], ot) and np.array_equal(got[3 * Gn:], oa)
-        assert np.array_equal(gc[:3 * Gn], ct) and np.array_equal(gc[3 * Gn:], ca)
+    for stage in (True, False):      # with and without the staging area (32-bit keys + segment codes) behind the histograms
+        ge, gq, gc = ds.latency_stats(d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"], d["inst"],
+                                      d["out_off"], torch.from_numpy(st).to(G.DEV), torch.from_numpy(dn).to(G.DEV), d["group"],
+                                      c.n_groups, d["t_mid"], pct, stage=stage)
+        ge, gq, gc = ge.cpu().numpy(), gq.cpu().numpy(), gc.cpu().numpy()
+        for vals, got in ((e2e, ge), (qd, gq)):
+            ot, ct = oracle.tail_stats(vals, seg_t, 3 * Gn, pct)
+            oa, ca = oracle.tail_stats(vals, seg_a, Gn, pct)
+            assert np.array_equal(got[:3 * Gn], ot) and np.array_equal(got[3 * Gn:], oa)
+            assert np.array_equal(gc[:3 * Gn], ct) and np.array_equal(gc[3 * Gn:], ca)
 
 
 def test_fused_latency_stats(G):
@@ -99,3 +100,57 @@ def test_fused_latency_stats(G):
     c1 = wl._trace_workload("t", 6, 1, 40, sv, [(wl.FIFO, wl.EXACT, 0.0)], oracle.characterize, rho=0.5)
     c1.tier[:] = 1                                                                               # tiers 0 and 2 empty -> -1
     _fused_vs_oracle(G, c1)
+
+
+def test_fused_staging_edge_cases(G):
+    """The staging area of ds_latency_stats: keys that need more than 32 bits, padded and out-of-order out_off, a staging
+    area that is too small - every case must give the oracle's percentiles (the unstaged passes take over)."""
+    import torch
+    import paper_2606_02982_b200 as ds
+    from paper_2606_02982_b200 import workload as wl
+    from paper_2606_02982_b200 import _lib
+    sv = wl.Server(max_batch=8, kv_budget=3000)
+    combos = [(p, wl.SPLIT, 0.1) for p in (wl.FIFO, wl.SJF, wl.AGING)]
+    c = wl._trace_workload("t", 15, 4, 900, sv, combos, oracle.characterize, rho=1.2)
+    st, dn, _ = oracle.simulate(c.trace_off, c.arrival, c.tier, c.words, c.tokens, c.out_len, c.server, c.instances)
+    n_inst, n_req, Gn, pct = len(c.instances), 900, c.n_groups, (50, 95, 99)
+
+    def check(st_h, dn_h, out_off_h, ws_extra, tier_h=None):
+        tier_h = c.tier if tier_h is None else tier_h
+        n_tot = int(max(out_off_h[:-1]) + n_req) if len(out_off_h) > 1 else 0
+        n_tot = max(n_tot, int(out_off_h[-1]))
+        S = np.full(n_tot, -7, np.int64); D = np.full(n_tot, -7, np.int64)
+        for i in range(n_inst):
+            S[out_off_h[i]:out_off_h[i] + n_req] = st_h[i * n_req:(i + 1) * n_req]
+            D[out_off_h[i]:out_off_h[i] + n_req] = dn_h[i * n_req:(i + 1) * n_req]
+        e2e, qd, seg_t, seg_a = oracle.latencies(c.trace_off, c.arrival, tier_h, c.words, c.tokens, c.out_len, c.instances,
+                                                 out_off_h, S, D, c.group, c.t_mid)
+        d = G.upload(c)
+        d["tier"] = torch.from_numpy(tier_h).to(G.DEV)
+        nb = ds.api.workspace_bytes(_lib.WS_TAIL_STATS, 4 * Gn, len(pct)) + ws_extra
+        ws = torch.empty(nb, dtype=torch.uint8, device=G.DEV)
+        ge, gq, gc = ds.latency_stats(d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"], d["inst"],
+                                      torch.from_numpy(out_off_h).to(G.DEV), torch.from_numpy(S).to(G.DEV), torch.from_numpy(D).to(G.DEV),
+                                      d["group"], c.n_groups, d["t_mid"], pct, workspace=ws)
+        sel = np.zeros(n_tot, bool)
+        for i in range(n_inst):
+            sel[out_off_h[i]:out_off_h[i] + n_req] = True
+        for vals, got in ((e2e, ge.cpu().numpy()), (qd, gq.cpu().numpy())):
+            v, a, b = vals[sel], seg_t[sel], seg_a[sel]
+            ot, ct = oracle.tail_stats(v, a, 3 * Gn, pct)
+            oa, ca = oracle.tail_stats(v, b, Gn, pct)
+            assert np.array_equal(got[:3 * Gn], ot) and np.array_equal(got[3 * Gn:], oa)
+            assert np.array_equal(gc.cpu().numpy()[:3 * Gn], ct) and np.array_equal(gc.cpu().numpy()[3 * Gn:], ca)
+
+    full = ds.api.workspace_bytes(_lib.WS_LATENCY_STAGE, 2 * n_inst * n_req + 64, 0)
+    off = c.out_off.copy()
+    check(st, dn, off, full)                                             # staged
+    check(st, dn, off, 5 * 100)                                          # staging area too small -> unstaged passes
+    pad = (np.arange(n_inst + 1, dtype=np.int64) * (n_req + 37)) + 11    # gap before the first range and between ranges
+    check(st, dn, pad, full)
+    perm = c.out_off[:-1][::-1].copy()                                   # ranges not in instance order -> unstaged passes
+    check(st, dn, np.concatenate([perm, c.out_off[-1:]]), full)
+    big = dn.copy(); big[5::7] += 1 << 33                                # keys differ above bit 31 -> unstaged passes
+    check(st, big, off, full)
+    shifted_st, shifted_dn = st + (1 << 40), dn + (1 << 40)              # common high bits, low 32 vary: still staged
+    check(shifted_st, shifted_dn, off, full)
