@@ -7,6 +7,7 @@
 // atomics otherwise) -> select kernel (one thread per (segment, percentile) walks 256 bins, fixes the digit,
 // reduces the rank). Traffic: 12 B per value per non-skipped digit; only keys matching the prefix are counted.
 #include "common.cuh"
+#include <type_traits>
 
 namespace ds {
 namespace k3 {
@@ -231,6 +232,29 @@ __device__ __forceinline__ bool stage_usable(const LatArgs& a, const Ws* hdr) {
   return a.skey != nullptr && !hdr->nostage && vary_top(hdr->and_bits ^ hdr->or_bits) <= 32;
 }
 
+// which of a staged key's (segment, percentile) prefixes it matches: bit q = its (group, tier) segment, bit 8+q = the
+// group's "all" segment. NP = n_pct when it is 1..4 (unrolled, no loop or index arithmetic per percentile), 0 = any.
+template <int NP>
+__device__ __forceinline__ unsigned match32(const unsigned* pfx32, unsigned s_t, unsigned s_a, unsigned hi, int n_pct) {
+  unsigned mm = 0;
+  if (NP == 2) {                               // the report's (50, 99): one 8-byte read per segment
+    const uint2 pt = *reinterpret_cast<const uint2*>(pfx32 + 2 * s_t), pa = *reinterpret_cast<const uint2*>(pfx32 + 2 * s_a);
+    mm = (hi == pt.x ? 1u : 0u) | (hi == pt.y ? 2u : 0u) | (hi == pa.x ? 256u : 0u) | (hi == pa.y ? 512u : 0u);
+  } else if (NP > 0) {
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+      mm |= (hi == pfx32[s_t * NP + q]) ? (1u << q) : 0u;
+      mm |= (hi == pfx32[s_a * NP + q]) ? (256u << q) : 0u;
+    }
+  } else {
+    for (int q = 0; q < n_pct; ++q) {
+      mm |= (hi == pfx32[s_t * n_pct + q]) ? (1u << q) : 0u;
+      mm |= (hi == pfx32[s_a * n_pct + q]) ? (256u << q) : 0u;
+    }
+  }
+  return mm;
+}
+
 // kCount: segment counts + AND/OR of all keys. Otherwise: digit-d histogram of the keys matching each (segment, pct) prefix.
 template <bool kCount>
 __global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pct, int d, Ws* hdr, unsigned long long* counts,
@@ -245,49 +269,71 @@ __global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pc
   }
   for (int i = threadIdx.x; i < nb; i += blockDim.x) sh[i] = 0;
   __shared__ unsigned long long pfx_s[kMaxSegPct];                  // the prefixes, read 2 x n_pct times per key
-  if (!kCount) for (int i = threadIdx.x; i < n_seg * n_pct; i += blockDim.x) pfx_s[i] = prefix[i];
+  __shared__ __align__(8) unsigned int pfx32_s[kMaxSegPct];                      // staged passes: bits [hshift, 32) of the prefixes
+  if (!kCount) {
+    const int hs = dp.lo + dp.width;
+    for (int i = threadIdx.x; i < n_seg * n_pct; i += blockDim.x) {
+      const unsigned long long pf = prefix[i];
+      pfx_s[i] = pf;
+      pfx32_s[i] = hs >= 32 ? 0u : ((unsigned)pf & (0xffffffffu >> hs));
+    }
+  }
   __syncthreads();
   unsigned long long kand = ~0ull, kor = 0ull; bool any = false;
   const int shift = dp.lo, hshift = dp.lo + dp.width;
   const unsigned dmask = (1u << dp.width) - 1u;
+  // First digit pass: every prefix still is the bits common to ALL keys, so each key matches all of its (segment,
+  // percentile) pairs. Only the (group, tier) histogram of percentile 0 is built from the keys; the group's "all"
+  // histogram (the sum over its tiers) and the other percentiles' copies are filled in shared memory afterwards:
+  // one aggregated add per key instead of 2 x n_pct. The count pass does the same with the segment counts.
+  const bool first = !kCount && d == 7;
   // one WARP per instance: the dependent header loads (instance -> trace -> offsets) of 16 warps per block overlap
   const int lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
   bool stage = a.skey != nullptr;      // count pass: this warp may still write staged keys
   if (!kCount && stage_usable(a, hdr)) {
-    // staged pass: 4 consecutive requests per thread (one 16-byte + one 4-byte load), the grid strides over the requests
+    // staged pass, all in 32 bits (measured: the 64-bit form of this loop - variable 64-bit shifts, 8-byte prefix compares -
+    // executed 120 instructions per key and was issue-bound at 80-110 us for 102 MB). Every key agrees with every prefix
+    // on bits 32..63 (they are common to all keys), so only bits [hshift, 32) are compared.
+    // 4 consecutive requests per thread (one 16-byte + one 4-byte load), the grid strides over the requests.
     const long long n = a.out_off[a.n_inst];
-    const unsigned long long khi = hdr->and_bits & 0xffffffff00000000ull;   // bits 32..63 are common to all keys
     const unsigned segall0 = 3u * (unsigned)a.n_groups;
-    for (long long i4 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 4; i4 < ((n + 127) & ~127ll);   // warp-uniform trips
-         i4 += (long long)gridDim.x * blockDim.x * 4) {
-      unsigned kk[4]; unsigned cc[4];
-      if (i4 + 3 < n) {
-        const uint4 kv = *reinterpret_cast<const uint4*>(a.skey + i4);
-        const uchar4 cv = *reinterpret_cast<const uchar4*>(a.scode + i4);
-        kk[0] = kv.x; kk[1] = kv.y; kk[2] = kv.z; kk[3] = kv.w; cc[0] = cv.x; cc[1] = cv.y; cc[2] = cv.z; cc[3] = cv.w;
-      } else {
+    const long long gstride = (long long)gridDim.x * blockDim.x * 4, nr = (n + 127) & ~127ll;   // warp-uniform trips
+    auto run = [&](auto np_tag) {
+      constexpr int NP = decltype(np_tag)::value;
+      for (long long i4 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 4; i4 < nr; i4 += gstride) {
+        unsigned kk[4], cc[4];
+        if (i4 + 3 < n) {
+          const uint4 kv = *reinterpret_cast<const uint4*>(a.skey + i4);
+          const uchar4 cv = *reinterpret_cast<const uchar4*>(a.scode + i4);
+          kk[0] = kv.x; kk[1] = kv.y; kk[2] = kv.z; kk[3] = kv.w; cc[0] = cv.x; cc[1] = cv.y; cc[2] = cv.z; cc[3] = cv.w;
+        } else {
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { const bool in = i4 + u < n; kk[u] = in ? a.skey[i4 + u] : 0u; cc[u] = in ? a.scode[i4 + u] : 255u; }
-      }
+          for (int u = 0; u < 4; ++u) { const bool in = i4 + u < n; kk[u] = in ? a.skey[i4 + u] : 0u; cc[u] = in ? a.scode[i4 + u] : 255u; }
+        }
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const bool ok = cc[u] != 255u;
-        const unsigned long long k = khi | kk[u];
-        const unsigned s_t = ok ? cc[u] : 0u, s_a = segall0 + ((s_t * 171u) >> 9);   // x/3 for x < 256
-        const unsigned long long hi = hshift >= 64 ? 0ull : (k >> hshift);
-        const unsigned dig = (unsigned)(k >> shift) & dmask;
-        unsigned mm = 0;
-        for (int q = 0; q < n_pct; ++q) {
-          mm |= (ok && hi == pfx_s[s_t * n_pct + q]) ? (1u << q) : 0u;
-          mm |= (ok && hi == pfx_s[s_a * n_pct + q]) ? (256u << q) : 0u;
-        }
-        if (!__any_sync(0xffffffffu, mm != 0u)) continue;
-        for (int q = 0; q < n_pct; ++q) {
-          agg_add(sh, (mm >> q) & 1u, (s_t * n_pct + q) * 256 + dig);
-          agg_add(sh, (mm >> (8 + q)) & 1u, (s_a * n_pct + q) * 256 + dig);
+        for (int u = 0; u < 4; ++u) {
+          const bool ok = cc[u] != 255u;
+          const unsigned s_t = ok ? cc[u] : 0u;
+          if (first) {     // every key matches every prefix of its segments: one add, the other histograms follow from it
+            agg_add(sh, ok, (s_t * n_pct) * 256 + ((kk[u] >> shift) & dmask));
+            continue;
+          }
+          const unsigned hi = __funnelshift_r(kk[u], 0u, hshift);                     // kk >> hshift, 0 when hshift = 32
+          const unsigned s_a = segall0 + ((s_t * 171u) >> 9);                          // x/3 for x < 256
+          const unsigned mm = ok ? match32<NP>(pfx32_s, s_t, s_a, hi, n_pct) : 0u;
+          if (!__any_sync(0xffffffffu, mm != 0u)) continue;
+          const unsigned dig = (kk[u] >> shift) & dmask;
+          for (int q = 0; q < n_pct; ++q) {
+            agg_add(sh, (mm >> q) & 1u, (s_t * n_pct + q) * 256 + dig);
+            agg_add(sh, (mm >> (8 + q)) & 1u, (s_a * n_pct + q) * 256 + dig);
+          }
         }
       }
-    }
+    };
+    if (n_pct == 2) run(std::integral_constant<int, 2>{});
+    else if (n_pct == 1) run(std::integral_constant<int, 1>{});
+    else if (n_pct == 3) run(std::integral_constant<int, 3>{});
+    else run(std::integral_constant<int, 0>{});
   } else
   for (long long ii = (long long)blockIdx.x * nwarp + (threadIdx.x >> 5); ii < a.n_inst; ii += (long long)gridDim.x * nwarp) {
     const int t = a.inst[ii].trace;
@@ -322,13 +368,13 @@ __global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pc
         const unsigned s_t = (unsigned)(3 * g + (ok ? tr[u] : 0)), s_a = (unsigned)(3 * a.n_groups + g);
         if (kCount) {
           if (ok) { kand &= k; kor |= k; any = true; }
-          agg_add(sh, ok, s_t);
-          agg_add(sh, ok, s_a);
+          agg_add(sh, ok, s_t);                   // (s_a's count is the sum over the group's tiers: added after the loop)
           const long long r = base + u * 32 + lane;
           if (stage && r < n) { a.skey[oo + r] = (unsigned)k; a.scode[oo + r] = ok ? (unsigned char)s_t : (unsigned char)255; }
         } else {
           const unsigned long long hi = hshift >= 64 ? 0ull : (k >> hshift);
           const unsigned dig = (unsigned)(k >> shift) & dmask;
+          if (first) { agg_add(sh, ok, (s_t * n_pct) * 256 + dig); continue; }
           // which of the key's (segment, percentile) prefixes it matches: bit q = tier segment, bit 8+q = "all" segment.
           // After the first pass almost no key matches anything: one vote rejects the whole warp.
           unsigned mm = 0;
@@ -346,6 +392,22 @@ __global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pc
     }
   }
   __syncthreads();
+  if (kCount) {
+    for (int g = threadIdx.x; g < a.n_groups; g += blockDim.x) sh[3 * a.n_groups + g] = sh[3 * g] + sh[3 * g + 1] + sh[3 * g + 2];
+    __syncthreads();
+  } else if (first) {
+    for (int i = threadIdx.x; i < a.n_groups * 256; i += blockDim.x) {
+      const int g = i >> 8, dg = i & 255;
+      unsigned sum = 0;
+      for (int t = 0; t < 3; ++t) {
+        const unsigned c = sh[((3 * g + t) * n_pct) * 256 + dg];
+        sum += c;
+        for (int q = 1; q < n_pct; ++q) sh[((3 * g + t) * n_pct + q) * 256 + dg] = c;
+      }
+      for (int q = 0; q < n_pct; ++q) sh[((3 * a.n_groups + g) * n_pct + q) * 256 + dg] = sum;
+    }
+    __syncthreads();
+  }
   if (kCount) {
     for (int dd = 16; dd > 0; dd >>= 1) { kand &= __shfl_xor_sync(0xffffffffu, kand, dd); kor |= __shfl_xor_sync(0xffffffffu, kor, dd); }
     const unsigned anym = __ballot_sync(0xffffffffu, any);
