@@ -298,8 +298,9 @@ __global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pc
     const long long n = a.out_off[a.n_inst];
     const unsigned segall0 = 3u * (unsigned)a.n_groups;
     const long long gstride = (long long)gridDim.x * blockDim.x * 4, nr = (n + 127) & ~127ll;   // warp-uniform trips
-    auto run = [&](auto np_tag) {
+    auto run = [&](auto np_tag, auto first_tag) {
       constexpr int NP = decltype(np_tag)::value;
+      constexpr bool kFirst = decltype(first_tag)::value;
       for (long long i4 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 4; i4 < nr; i4 += gstride) {
         unsigned kk[4], cc[4];
         if (i4 + 3 < n) {
@@ -314,14 +315,19 @@ __global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pc
         for (int u = 0; u < 4; ++u) {
           const bool ok = cc[u] != 255u;
           const unsigned s_t = ok ? cc[u] : 0u;
-          if (first) {     // every key matches every prefix of its segments: one add, the other histograms follow from it
+          if (kFirst) {    // every key matches every prefix of its segments: one add, the other histograms follow from it
             agg_add(sh, ok, (s_t * n_pct) * 256 + ((kk[u] >> shift) & dmask));
             continue;
           }
           const unsigned hi = __funnelshift_r(kk[u], 0u, hshift);                     // kk >> hshift, 0 when hshift = 32
           const unsigned s_a = segall0 + ((s_t * 171u) >> 9);                          // x/3 for x < 256
+          if (NP == 2) {   // reject first with one predicate (four chained compares), build the match mask only for survivors
+            const uint2 pt = *reinterpret_cast<const uint2*>(pfx32_s + 2 * s_t), pa = *reinterpret_cast<const uint2*>(pfx32_s + 2 * s_a);
+            const bool hit = ok & ((hi == pt.x) | (hi == pt.y) | (hi == pa.x) | (hi == pa.y));
+            if (!__any_sync(0xffffffffu, hit)) continue;
+          }
           const unsigned mm = ok ? match32<NP>(pfx32_s, s_t, s_a, hi, n_pct) : 0u;
-          if (!__any_sync(0xffffffffu, mm != 0u)) continue;
+          if (NP != 2 && !__any_sync(0xffffffffu, mm != 0u)) continue;
           const unsigned dig = (kk[u] >> shift) & dmask;
           for (int q = 0; q < n_pct; ++q) {
             agg_add(sh, (mm >> q) & 1u, (s_t * n_pct + q) * 256 + dig);
@@ -330,10 +336,11 @@ __global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pc
         }
       }
     };
-    if (n_pct == 2) run(std::integral_constant<int, 2>{});
-    else if (n_pct == 1) run(std::integral_constant<int, 1>{});
-    else if (n_pct == 3) run(std::integral_constant<int, 3>{});
-    else run(std::integral_constant<int, 0>{});
+    if (first) run(std::integral_constant<int, 0>{}, std::true_type{});
+    else if (n_pct == 2) run(std::integral_constant<int, 2>{}, std::false_type{});
+    else if (n_pct == 1) run(std::integral_constant<int, 1>{}, std::false_type{});
+    else if (n_pct == 3) run(std::integral_constant<int, 3>{}, std::false_type{});
+    else run(std::integral_constant<int, 0>{}, std::false_type{});
   } else
   for (long long ii = (long long)blockIdx.x * nwarp + (threadIdx.x >> 5); ii < a.n_inst; ii += (long long)gridDim.x * nwarp) {
     const int t = a.inst[ii].trace;
