@@ -38,6 +38,13 @@ def test_hand_traces(G, golden_dir):
         c = G.tiny_workload(wl, case["req"], sv, [(case["policy"], case["estimator"], case["alpha"])])
         st, dn, ema = G.gpu_simulate(c)
         assert st.tolist() == case["start"] and dn.tolist() == case["done"], case["name"]
+        if "est" in case:                                   # frozen admission-time estimates (H7: R-ORD) through ds_simulate_est
+            import paper_2606_02982_b200 as ds
+            d = G.upload(c)
+            st2, dn2, _, est = ds.simulate_est(d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"],
+                                               c.server, d["inst"], d["out_off"], int(c.out_off[-1]))
+            assert ds.device_status() == 0
+            assert est.cpu().tolist() == case["est"] and st2.cpu().tolist() == case["start"], case["name"]
 
 
 def test_cfg0_full(G):
@@ -87,6 +94,36 @@ def test_equal_ticks_zero_lengths_and_ties(G):
         sv = wl.Server(max_batch=mb, kv_budget=kv, aging_step=7000)
         c = G.tiny_workload(wl, req, sv, [(p, e, 0.3) for p in wl.ALL_POLICIES for e in (wl.SPLIT, wl.EXACT)])
         _assert_same(G.gpu_simulate(c), _oracle(c), c)
+
+
+def test_estimates_above_the_kv_budget(G):
+    # A8 progress guarantee + head-of-line blocking at scale: a budget so small that many estimates alone exceed it (they are
+    # admitted only into an empty server) and nearly every admission is a KV decision
+    for mb, kv, seed in ((4, 150, 3), (32, 120, 4), (128, 180, 5)):
+        sv = wl.Server(max_batch=mb, kv_budget=kv, aging_step=60_000)
+        combos = [(p, e, 0.2) for p in wl.ALL_POLICIES + [wl.AGING_UNCLAMPED] for e in (wl.SPLIT, wl.EXACT)]
+        c = wl._trace_workload("t", seed, 2, 500, sv, combos, oracle.characterize, rho=0.4)
+        assert (c.tokens > kv).mean() > 0.05 and (c.words > kv).any()
+        _assert_same(G.gpu_simulate(c), _oracle(c), c)
+
+
+def test_same_tick_arrivals_and_completions_random(G):
+    # R-ORD at scale (H7 repeated with random sizes): triplets far apart on an idle batch-1 server; a arrives at T, its
+    # completion tick T+S(a) is known in closed form; c arrives one tick before it (old factor), b exactly on it (new factor)
+    from _simutil import service_time
+    rng = np.random.default_rng(12)
+    sv = wl.Server(max_batch=1, kv_budget=0, aging_step=50_000)
+    rows = []
+    for k in range(130):
+        T, tier = k * 100_000, int(rng.integers(0, 3))
+        W, P, O = rng.integers(1, 200, 3), rng.integers(1, 300, 3), rng.integers(1, 8, 3)
+        S = service_time(int(P[0]), int(O[0]), sv)
+        rows += [[T, tier, W[0], P[0], O[0]], [T + S - 1, tier, W[1], P[1], O[1]], [T + S, tier, W[2], P[2], O[2]]]
+    combos = [(p, wl.SPLIT, a) for p in wl.ALL_POLICIES for a in (0.5, 0.9)]
+    c = G.tiny_workload(wl, rows, sv, combos)
+    o = _oracle(c)
+    assert all(np.isin(c.arrival, o[1][i * c.n_req:(i + 1) * c.n_req]).sum() >= 130 for i in range(c.n_inst))
+    _assert_same(G.gpu_simulate(c), o, c)
 
 
 def test_bad_arguments(G):

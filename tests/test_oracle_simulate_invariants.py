@@ -204,3 +204,59 @@ def test_aging_brute_force_against_direct_key():
             assert st[r] == now
             now += service_time(req[r][3], 1, sv)
         assert len(order) == n
+
+
+def check_kv_admission_from_outputs(arrival, P, O, start, done, max_batch, kv_budget, step):
+    """I2 + A8 verified from the outputs alone (FIFO, EXACT estimator, iteration cost == `step` ticks whatever the batch):
+    with a constant iteration cost a running request has decoded g = (t - start)/step tokens at boundary t, so the context
+    held, kv_used(t) = sum over running r of P[r] + g[r], is reconstructed without the simulator. Every admission and every
+    boundary at which the FIFO head stayed queued although a slot was free must agree with SURVEY.md §8(c) C.2 step 4:
+    admit iff server empty or kv_used + est <= kv_budget (est = P); a deferred head blocks everything behind it."""
+    n = len(P)
+    assert (done - start == O * step).all()                       # exactly O iterations in the batch
+    assert (np.diff(start) >= 0).all()                            # FIFO admits in index order
+    def running_before(c, t):                                     # requests holding a slot at boundary t when c is considered:
+        r = np.arange(c)                                          # FIFO: only lower indices can have been admitted before c
+        return r[(start[:c] <= t) & (done[:c] > t)]               # done == t retired in step 2, before step 4
+    def kv_used(rs, t):
+        assert ((t - start[rs]) % step == 0).all()                # boundaries of a busy period lie on its grid
+        return int((P[rs] + (t - start[rs]) // step).sum())
+    n_deferred = n_over = 0
+    for c in range(n):
+        t = int(start[c])
+        rs = running_before(c, t)
+        assert len(rs) < max_batch                                # I2: |R| <= max_batch
+        if len(rs) > 0:
+            assert kv_used(rs, t) + P[c] <= kv_budget, (c, t)     # admitted into a busy server => it fitted
+        elif P[c] > kv_budget:
+            n_over += 1                                           # progress guarantee: admitted although est > budget
+        # boundaries at which c was already the queue head (c-1 admitted) and had arrived, but was not admitted
+        t_head = max(int(arrival[c]), int(start[c - 1]) if c else 0)
+        if t_head < t:
+            busy = running_before(c, t - 1)                       # the busy period c waits in
+            assert len(busy) > 0                                  # I5: an idle server never leaves a queued request waiting
+            g0 = int(start[busy].max())                           # a grid point of that busy period
+            k0 = -(-(t_head - g0) // step)                        # first boundary at or after t_head
+            for tb in range(g0 + k0 * step, t, step):
+                rb = running_before(c, tb)
+                assert len(rb) > 0
+                if len(rb) < max_batch:                           # a slot was free: only the KV budget can have deferred c
+                    assert kv_used(rb, tb) + P[c] > kv_budget, (c, tb)
+                    n_deferred += 1
+    return n_deferred, n_over
+
+
+def test_i2_kv_accounting_and_a8_reconstructed_from_outputs():
+    # direct check of I2 (kv_used = sum(P+g)) and of the three parts of A8 (check on the estimate, head-of-line blocking,
+    # unconditional admission into an empty server), independent of the oracle's own bookkeeping
+    rng = np.random.default_rng(11)
+    n, step = 3000, 1000
+    P = rng.integers(1, 60, n).astype(np.int64)
+    P[rng.integers(0, n, 40)] = rng.integers(130, 200, 40)        # some estimates alone exceed the budget
+    O = rng.integers(1, 30, n).astype(np.int64)
+    arr = np.cumsum(rng.integers(0, 2 * 1900, n)).astype(np.int64)     # utilisation high enough for regular deferrals
+    req = np.stack([arr, rng.integers(0, 3, n), P, P, O], 1)
+    sv = server(max_batch=6, kv_budget=120, c_base=step, c_batch=0, c_ctx=0, c_prefill=0)
+    st, dn, _ = run_oracle(req, sv, wl.FIFO, wl.EXACT)
+    n_deferred, n_over = check_kv_admission_from_outputs(arr, P, O, st, dn, 6, 120, step)
+    assert n_deferred > 200 and n_over > 10                       # the case does exercise deferral and the progress rule

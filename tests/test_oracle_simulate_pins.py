@@ -1,4 +1,6 @@
-"""Pins for oracle.simulate: hand-worked traces H1-H6, EMA bit pattern H3, closed forms."""
+"""Pins for oracle.simulate: hand-worked traces H1-H10, EMA bit pattern H3, closed forms.
+H7-H10 (derivations: DESIGN.md §4.4) pin the readings R-ORD (same-tick order), A8 (KV deferral is head-of-line blocking; an
+empty server admits unconditionally) and the KV release kv_used -= P+g on retirement."""
 import json
 import math
 import os
@@ -18,14 +20,31 @@ def _golden(golden_dir):
 
 def test_hand_traces(golden_dir):
     g = _golden(golden_dir)
-    assert len(g["cases"]) == 12
+    assert len(g["cases"]) == 19
     for c in g["cases"]:
         sv = server(**c["server"])
         if "weight" in c["server"]:
             sv.weight = tuple(c["server"]["weight"])
-        st, dn, ema = run_oracle(c["req"], sv, c["policy"], c["estimator"], c["alpha"])
+        st, dn, ema, est = run_oracle(c["req"], sv, c["policy"], c["estimator"], c["alpha"], want_est=True)
         assert st.tolist() == c["start"], c["name"]
         assert dn.tolist() == c["done"], c["name"]
+        if "est" in c:
+            assert est.tolist() == c["est"], c["name"]
+
+
+def test_h7_factor_after_same_tick_completion():
+    # H7 (R-ORD, SURVEY.md:486): r0 completes at 2162 with m = 2/4 and alpha = 0.5 -> B[Std] = 0.5*1 + 0.5*0.5 = 0.75 exactly;
+    # r1 (arrival 2161 < 2162) was estimated with the old factor 1.0, r2 (arrival 2162) with 0.75: ceil(0.75*8) = 6, not 8
+    req = [[0, 1, 4, 2, 1], [2161, 1, 7, 3, 1], [2162, 1, 8, 5, 1]]
+    sv = server(traj_every=1)
+    st, dn, ema, traj, est = run_oracle(req, sv, wl.SJF, wl.SPLIT, 0.5, want_traj=True, want_est=True)
+    assert traj[0].tolist() == [1.0, 0.75, 1.0]
+    assert est.tolist() == [4, 7, 6]
+    assert st[2] < st[1]                       # SJF serves r2 (est 6) before r1 (est 7)
+    # moving r2 one tick earlier makes it an INGEST-EARLY arrival: old factor, est 8, served after r1
+    req[2][0] = 2161
+    st, dn, ema, est = run_oracle(req, sv, wl.SJF, wl.SPLIT, 0.5, want_est=True)
+    assert est.tolist() == [4, 7, 8] and st[1] < st[2]
 
 
 def test_h3_ema_bit_pattern(golden_dir):
