@@ -52,15 +52,15 @@ def _o():
         p = C.c_void_p
         lib.oracle_characterize.argtypes = [p, C.c_int64, p, C.c_int64, p, p]
         lib.oracle_simulate.argtypes = [p, p, p, C.c_int64, p, p, p, p, p, p, p]
-        lib.oracle_estimation_error.argtypes = [p, p, C.c_int64, p, p, p, p, C.c_int32, p, p]
+        lib.oracle_estimation_error.argtypes = [p, p, C.c_int64, p, p, p, p, p, C.c_int32, p, p]
         lib.oracle_estimation_error.restype = C.c_int
-        lib.oracle_queue_depth.argtypes = [p, p, C.c_int64, p, p, C.c_int64, C.c_int64, C.c_int64, p]
+        lib.oracle_queue_depth.argtypes = [p, p, C.c_int64, p, p, p, C.c_int64, C.c_int64, C.c_int64, p]
         lib.oracle_queue_depth.restype = C.c_int
         lib.oracle_simulate_budget.argtypes = [p, p, p, p, p, C.c_int64, p, p, p, p, p, p, p]
         lib.oracle_simulate_budget.restype = C.c_int
         lib.oracle_simulate_closed.argtypes = [p, p, p, p, C.c_int64, C.c_int64, C.c_int64, p, C.c_int64, p, p, p, p, p, p, p, p]
         lib.oracle_simulate_closed.restype = C.c_int
-        lib.oracle_latencies.argtypes = [p, p, C.c_int64, p, p, p, p, p, p, p, p, p]
+        lib.oracle_latencies.argtypes = [p, p, C.c_int64, p, p, p, p, p, p, p, p, p, p]
         lib.oracle_tail_stats.argtypes = [p, p, C.c_int64, C.c_int32, p, C.c_int32, p, p]
         for f in (lib.oracle_characterize, lib.oracle_simulate, lib.oracle_latencies, lib.oracle_tail_stats):
             f.restype = C.c_int
@@ -135,7 +135,8 @@ def simulate(trace_off, arrival, tier, words, tokens, out_len, server, instances
     return out
 
 
-def latencies(trace_off, arrival, tier, words, tokens, out_len, instances, out_off, start, done, group=None, t_mid=None):
+def latencies(trace_off, arrival, tier, words, tokens, out_len, instances, out_off, start, done, group=None, t_mid=None,
+              arrival_override=None):
     tr, keep = _traces(trace_off, arrival, tier, words, tokens, out_len)
     inst = _c(instances, INSTANCE_DTYPE)
     out_off = _c(out_off, np.int64)
@@ -148,7 +149,8 @@ def latencies(trace_off, arrival, tier, words, tokens, out_len, instances, out_o
     sa = np.zeros(n, np.int32)
     g = None if group is None else _c(group, np.int32)
     tm = None if t_mid is None else _c(t_mid, np.int64)
-    rc = _o().oracle_latencies(C.byref(tr), _p(inst), len(inst), _p(out_off), _p(start), _p(done), _p(g), _p(tm),
+    ao = None if arrival_override is None else _c(arrival_override, np.int64)
+    rc = _o().oracle_latencies(C.byref(tr), _p(inst), len(inst), _p(out_off), _p(ao), _p(start), _p(done), _p(g), _p(tm),
                                _p(e2e), _p(qd), _p(st), _p(sa))
     assert rc == 0
     return e2e, qd, st, sa
@@ -170,7 +172,7 @@ ERR_FIELDS = ("n", "sum_abs_err", "sum_sq_err", "sum_est", "sum_tokens", "n_shor
 
 
 def estimation_error(trace_off, arrival, tier, words, tokens, out_len, instances, out_off, est, start, group, n_groups,
-                     want_class_seg=False):
+                     want_class_seg=False, arrival_override=None):
     """-> sums int64[n_groups, 11] (ERR_FIELDS) and, if asked, class_seg int32 per simulated request."""
     tr, keep = _traces(trace_off, arrival, tier, words, tokens, out_len)
     inst = _c(instances, INSTANCE_DTYPE)
@@ -180,21 +182,24 @@ def estimation_error(trace_off, arrival, tier, words, tokens, out_len, instances
     g = None if group is None else _c(group, np.int32)
     out = np.zeros((n_groups, 11), np.int64)
     seg = np.zeros(est.size, np.int32) if want_class_seg else None
-    rc = _o().oracle_estimation_error(C.byref(tr), _p(inst), len(inst), _p(out_off), _p(est), _p(start), _p(g), n_groups,
+    ao = None if arrival_override is None else _c(arrival_override, np.int64)
+    rc = _o().oracle_estimation_error(C.byref(tr), _p(inst), len(inst), _p(out_off), _p(ao), _p(est), _p(start), _p(g), n_groups,
                                       _p(out), _p(seg))
     if rc:
         raise ValueError("oracle_estimation_error: contract violation")
     return (out, seg) if want_class_seg else out
 
 
-def queue_depth(trace_off, arrival, tier, words, tokens, out_len, instances, out_off, start, t0, dt, n_samples):
+def queue_depth(trace_off, arrival, tier, words, tokens, out_len, instances, out_off, start, t0, dt, n_samples,
+                arrival_override=None):
     """-> depth int32[n_inst, n_samples, 3]: requests of each tier queued (arrival <= t < start) at t = t0 + j*dt."""
     tr, keep = _traces(trace_off, arrival, tier, words, tokens, out_len)
     inst = _c(instances, INSTANCE_DTYPE)
     out_off = _c(out_off, np.int64)
     start = _c(start, np.int64)
     depth = np.zeros((len(inst), int(n_samples), 3), np.int32)
-    rc = _o().oracle_queue_depth(C.byref(tr), _p(inst), len(inst), _p(out_off), _p(start), int(t0), int(dt), int(n_samples),
+    ao = None if arrival_override is None else _c(arrival_override, np.int64)
+    rc = _o().oracle_queue_depth(C.byref(tr), _p(inst), len(inst), _p(out_off), _p(ao), _p(start), int(t0), int(dt), int(n_samples),
                                  _p(depth))
     if rc:
         raise ValueError("oracle_queue_depth: contract violation")

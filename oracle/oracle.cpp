@@ -298,14 +298,16 @@ extern "C" int oracle_simulate_closed(const oracle_traces* tr, const uint8_t* ca
                        ema_final, traj_off, ema_traj, est_out);
 }
 
+// arrival_override (nullable, indexed like start_tick): the per-instance arrival ticks of a closed-loop run
+// (oracle_simulate_closed's arrival_out; "50 concurrent clients"), used instead of tr->arrival_tick.
 extern "C" int oracle_latencies(const oracle_traces* tr, const oracle_instance* inst, int64_t n_inst,
-                                const int64_t* out_off, const int64_t* start_tick, const int64_t* done_tick,
+                                const int64_t* out_off, const int64_t* arrival_override, const int64_t* start_tick, const int64_t* done_tick,
                                 const int32_t* group, const int64_t* t_mid, int64_t* e2e, int64_t* qdelay,
                                 int32_t* seg_tier, int32_t* seg_all) {
   for (int64_t ii = 0; ii < n_inst; ++ii) {
     int64_t t = inst[ii].trace, lo = tr->trace_off[t], n = tr->trace_off[t + 1] - lo;
     for (int64_t r = 0; r < n; ++r) {
-      int64_t o = out_off[ii] + r, a = tr->arrival_tick[lo + r];
+      int64_t o = out_off[ii] + r, a = arrival_override ? arrival_override[o] : tr->arrival_tick[lo + r];
       e2e[o] = done_tick[o] - a;        // end-to-end latency
       qdelay[o] = start_tick[o] - a;    // queue wait
       int32_t gph = group ? group[ii] : 0;
@@ -339,7 +341,7 @@ extern "C" int oracle_tail_stats(const int64_t* values, const int32_t* seg_id, i
 }
 
 extern "C" int oracle_estimation_error(const oracle_traces* tr, const oracle_instance* inst, int64_t n_inst,
-                                       const int64_t* out_off, const int64_t* est, const int64_t* start_tick,
+                                       const int64_t* out_off, const int64_t* arrival_override, const int64_t* est, const int64_t* start_tick,
                                        const int32_t* group, int32_t n_groups, int64_t* out, int32_t* class_seg) {
   for (int64_t k = 0; k < (int64_t)n_groups * 11; ++k) out[k] = 0;
   for (int64_t ii = 0; ii < n_inst; ++ii) {
@@ -354,7 +356,8 @@ extern "C" int oracle_estimation_error(const oracle_traces* tr, const oracle_ins
       int cls = e <= 128 ? 0 : (e <= 512 ? 1 : 2);          // Eq. 4
       o[0] += 1; o[1] += err < 0 ? -err : err; o[2] += err * err; o[3] += e; o[4] += P;
       o[5 + cls] += 1;
-      if (start_tick) o[8 + cls] += start_tick[out_off[ii] + r] - tr->arrival_tick[lo + r];   // queue wait
+      if (start_tick)                                        // queue wait; closed loop: the instance's own arrivals
+        o[8 + cls] += start_tick[out_off[ii] + r] - (arrival_override ? arrival_override[out_off[ii] + r] : tr->arrival_tick[lo + r]);
       if (class_seg) class_seg[out_off[ii] + r] = 3 * g + cls;
     }
   }
@@ -365,13 +368,13 @@ extern "C" int oracle_estimation_error(const oracle_traces* tr, const oracle_ins
 // its arrival tick until the tick it is admitted to the batch. depth[i][j][k] = #{r of tier k : arrival <= t_j < start},
 // t_j = t0 + j*dt. Written as the definition: every request increments the samples it covers.
 extern "C" int oracle_queue_depth(const oracle_traces* tr, const oracle_instance* inst, int64_t n_inst, const int64_t* out_off,
-                                  const int64_t* start_tick, int64_t t0, int64_t dt, int64_t n_samples, int32_t* depth) {
+                                  const int64_t* arrival_override, const int64_t* start_tick, int64_t t0, int64_t dt, int64_t n_samples, int32_t* depth) {
   if (dt < 1 || n_samples < 0) return -1;
   for (int64_t k = 0; k < n_inst * n_samples * 3; ++k) depth[k] = 0;
   for (int64_t ii = 0; ii < n_inst; ++ii) {
     int64_t t = inst[ii].trace, lo = tr->trace_off[t], n = tr->trace_off[t + 1] - lo;
     for (int64_t r = 0; r < n; ++r) {
-      int64_t a = tr->arrival_tick[lo + r], st = start_tick[out_off[ii] + r];
+      int64_t a = arrival_override ? arrival_override[out_off[ii] + r] : tr->arrival_tick[lo + r], st = start_tick[out_off[ii] + r];
       for (int64_t j = 0; j < n_samples; ++j) {
         int64_t tj = t0 + j * dt;
         if (tj >= st) break;

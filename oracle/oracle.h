@@ -81,19 +81,21 @@ int oracle_simulate_closed(const oracle_traces* tr, const uint8_t* category, con
 /* Estimation fidelity (Eq. 3-4 job classes; Tables IV, IX, X): per reporting group, exact integer sums
  * over its simulated requests: out[g*11 + ..] = { n, sum|est-P|, sum(est-P)^2, sum est, sum P, n_short, n_medium, n_long,
  * sum qdelay_short, sum qdelay_medium, sum qdelay_long } with class short: est<=128, medium: est<=512, long: else.
- * start_tick nullable (qdelay sums 0). class_seg nullable: 3*group+class per simulated request. */
+ * start_tick nullable (qdelay sums 0). class_seg nullable: 3*group+class per simulated request.
+ * arrival_override (nullable, here and below; indexed like start_tick): per-instance arrival ticks of a closed-loop run
+ * (oracle_simulate_closed's arrival_out), used instead of tr->arrival_tick. */
 int oracle_estimation_error(const oracle_traces* tr, const oracle_instance* inst, int64_t n_inst, const int64_t* out_off,
-                            const int64_t* est, const int64_t* start_tick, const int32_t* group, int32_t n_groups,
+                            const int64_t* arrival_override, const int64_t* est, const int64_t* start_tick, const int32_t* group, int32_t n_groups,
                             int64_t* out, int32_t* class_seg);
 
 /* Queue depth per tenant tier over time (Fig. 8): depth[(i*n_samples + j)*3 + k] =
  * #{requests r of instance i with tier k : arrival <= t0 + j*dt < start_tick}. dt >= 1. */
 int oracle_queue_depth(const oracle_traces* tr, const oracle_instance* inst, int64_t n_inst, const int64_t* out_off,
-                       const int64_t* start_tick, int64_t t0, int64_t dt, int64_t n_samples, int32_t* depth);
+                       const int64_t* arrival_override, const int64_t* start_tick, int64_t t0, int64_t dt, int64_t n_samples, int32_t* depth);
 
 /* PAPER.md:270 (queue wait vs end-to-end latency). seg outputs nullable. */
 int oracle_latencies(const oracle_traces* tr, const oracle_instance* inst, int64_t n_inst, const int64_t* out_off,
-                     const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, const int64_t* t_mid,
+                     const int64_t* arrival_override, const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, const int64_t* t_mid,
                      int64_t* e2e, int64_t* qdelay, int32_t* seg_tier, int32_t* seg_all);
 
 /* PAPER.md:436 (P50/P95/P99 tables), reading A13 (nearest rank). */
