@@ -22,6 +22,9 @@
  *  - Scratch memory comes from a caller-supplied workspace; query its size with ds_workspace_bytes().
  *    Workspace contents are undefined on entry and exit; two calls in flight need two workspaces.
  *  - There is no CPU fallback: every function fails with DS_ECUDA if no CUDA device is usable.
+ *  - Devices: every call works on the calling thread's current CUDA device (cudaSetDevice); pointers, stream and workspace
+ *    must belong to it. The status word, the SM count used to size grids and the kernels' shared-memory attributes are
+ *    kept per device, so one process may drive several devices (bench.py uses one process per GPU all the same).
  */
 #ifndef DRIFTSCHED_H
 #define DRIFTSCHED_H
@@ -43,6 +46,7 @@ extern "C" {
 #define DS_DEV_BAD_TRACE 2u    /* ds_simulate: tier > 2, out_len < 1, words/tokens < 0 or arrivals decreasing */
 #define DS_DEV_KEY_RANGE 4u    /* ds_simulate: SJF key overflow (est >= 2^39 or trace longer than 2^24) */
 #define DS_DEV_BAD_INSTANCE 8u /* ds_simulate: instance field out of range; ds_estimation_error: group out of range */
+#define DS_DEV_BAD_OUT_OFF 16u /* ds_simulate: out_off[i] < 0 or out_off[i] + trace length > n_total (instance skipped) */
 
 /* ---------------------------------------------------------------------------------------------- (a)
  * Workload characterization ("whitespace-delimited word counts" vs
@@ -54,7 +58,11 @@ extern "C" {
  *   words_out[i]  = number of maximal runs of non-WS bytes                      (the split() proxy)
  *   tokens_out[i] = sum over maximal LETTER runs of ceil(len/4) + number of PUNCT bytes
  *                   (BASELINE.json:configs[0] pseudo-token rule standing in for the model tokenizer)
- * bytes   [n_bytes]      device, any alignment (16-byte alignment is fastest)
+ * bytes   [n_bytes]      device, any alignment (16-byte alignment is fastest). The kernel reads whole 16-byte-aligned
+ *                        pieces: up to 15 bytes before bytes and after bytes + n_bytes are loaded (and ignored) when the
+ *                        ends are not 16-byte aligned. Such a piece never leaves the 256-byte allocation granule that holds
+ *                        a byte of the buffer, so any cudaMalloc / torch (sub-)allocation is safe; a buffer carved out of
+ *                        a foreign mapping at finer granularity must be padded to 16-byte boundaries.
  * offsets [n_prompts+1]  device, 0 <= offsets[0], non-decreasing, offsets[n_prompts] <= n_bytes
  * words_out, tokens_out [n_prompts] device, overwritten.
  * workspace: ds_workspace_bytes(DS_WS_CHARACTERIZE, n_bytes, n_prompts).
@@ -107,22 +115,28 @@ typedef struct {
  *   EMA on completion: m=P/base; B = (1-a)*B + a*m in fp64, four separately rounded operations.
  * inst        [n_inst]            device
  * out_off     [n_inst+1]          device; instance i writes start/done at out_off[i] + local request index
- * start_tick, done_tick           device, int64, sized out_off[n_inst]; done_tick is also used as scratch
+ * n_total                         HOST value: out_off[n_inst] = number of simulated requests = length of every per-request
+ *                                 output array; an instance whose range leaves [0, n_total) is skipped (DS_DEV_BAD_OUT_OFF)
+ * start_tick, done_tick           device, int64, sized n_total; done_tick is also used as scratch
  *                                 for the frozen estimates while a request is queued
  * ema_final   [n_inst*3]          device, fp64 B[tier] at the end of the run
  * traj_off    [n_inst+1] nullable device; instance i owns trajectory samples [traj_off[i], traj_off[i+1]),
  *                                 floor(n_req_i / traj_every) of them
  * ema_traj    [traj_off[n_inst]*3] nullable device fp64
- * workspace: ds_workspace_bytes(DS_WS_SIMULATE, total_requests_over_instances, n_inst).
+ * workspace: ds_workspace_bytes(DS_WS_SIMULATE, n_total, n_inst) bytes are REQUIRED (DS_ENOMEM otherwise): header,
+ *   instance permutation and one 8-byte SJF heap slot per simulated request (touched only by SJF instances with more
+ *   than 256 requests queued, but always validated).
+ * Contract checked on the device (DS_DEV_BAD_TRACE, outputs of that instance unspecified): tier <= 2, words/tokens >= 0,
+ *   out_len >= 1, arrival_tick >= 0 and non-decreasing over every pair of neighbouring requests of a trace.
  * Launches: 1 memset (work counter) + 2 kernels (policy-major ordering of the instances, simulation). */
 int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
-                const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
+                const int64_t* out_off, int64_t n_total, int64_t* start_tick, int64_t* done_tick, double* ema_final,
                 const int64_t* traj_off, double* ema_traj, void* workspace, size_t workspace_bytes, void* stream);
 
 /* ds_simulate that also returns the frozen admission-time estimate of every simulated request (reading A5):
  * est_out [out_off[n_inst]] int64 device, same indexing as start_tick. Everything else as ds_simulate. */
 int ds_simulate_est(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
-                    const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
+                    const int64_t* out_off, int64_t n_total, int64_t* start_tick, int64_t* done_tick, double* ema_final,
                     const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace, size_t workspace_bytes,
                     void* stream);
 
@@ -145,9 +159,9 @@ typedef struct {
   double f_max;
 } ds_budget;
 int ds_simulate_budget(const ds_traces* tr, const uint8_t* category, const ds_budget* bp, const ds_server* sv,
-                       const ds_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t* start_tick, int64_t* done_tick,
-                       double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace,
-                       size_t workspace_bytes, void* stream);
+                       const ds_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t n_total, int64_t* start_tick,
+                       int64_t* done_tick, double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out,
+                       void* workspace, size_t workspace_bytes, void* stream);
 
 /* ds_simulate_budget with CLOSED-LOOP arrivals ("50 concurrent clients",
  * 3000 requests per run): only the first n_clients requests of a trace arrive at their tr->arrival_tick; every completion
@@ -155,8 +169,10 @@ int ds_simulate_budget(const ds_traces* tr, const uint8_t* category, const ds_bu
  * think_ticks. Same-tick order as everywhere (R-ORD): completions, then same-tick arrivals, which therefore see the updated
  * factors. n_clients >= 1, think_ticks >= 0 (host values; DS_EINVAL otherwise); n_clients >= trace length = the open loop.
  * Contract: the arrival sequence the loop produces must be non-decreasing in request index like every trace's, i.e. the
- * first n_clients arrival ticks must not lie after the first release (they are all 0 when the paper's clients start
- * together); a later one sets DS_DEV_BAD_TRACE and the instance's outputs are unspecified.
+ * first n_clients arrival ticks (non-decreasing, like every trace) must not lie after the first release: staggered client
+ * starts are fine as long as the last client starts no later than the first completion + think_ticks (they are all 0 when
+ * the paper's clients start together). Every release is compared with the arrival before it; a violation sets
+ * DS_DEV_BAD_TRACE and the instance's outputs are unspecified.
  * arrival_out [out_off[n_inst]] int64 device (written): the arrival tick of every simulated request - per instance,
  * because arrivals now depend on the policy; latencies are done_tick - arrival_out / start_tick - arrival_out.
  * batch_wait_ticks >= 0 ("batch wait interval of 0.01 seconds before dispatching"; 0 = none; reading B6): an
@@ -164,7 +180,8 @@ int ds_simulate_budget(const ds_traces* tr, const uint8_t* category, const ds_bu
  * a + batch_wait_ticks, whichever is first; a busy server admits at every iteration boundary as before.
  * Everything else as ds_simulate_budget. */
 int ds_simulate_closed(const ds_traces* tr, const uint8_t* category, const ds_budget* bp, const ds_server* sv, int32_t n_clients,
-                       int64_t think_ticks, int64_t batch_wait_ticks, const ds_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t* arrival_out,
+                       int64_t think_ticks, int64_t batch_wait_ticks, const ds_instance* inst, int64_t n_inst, const int64_t* out_off,
+                       int64_t n_total, int64_t* arrival_out,
                        int64_t* start_tick, int64_t* done_tick, double* ema_final, const int64_t* traj_off, double* ema_traj,
                        int64_t* est_out, void* workspace, size_t workspace_bytes, void* stream);
 
@@ -177,9 +194,13 @@ int ds_simulate_closed(const ds_traces* tr, const uint8_t* category, const ds_bu
  *   input + output tokens, Eq. 1) and qdelay = start_tick - arrival (0 if start_tick is NULL).
  *   MAE = out[1]/out[0], RMSE = sqrt(out[2]/out[0]), mean bias = out[4]/out[3] are left to the caller (fp64).
  * class_seg (nullable) [out_off[n_inst]] int32 device: 3*g + class, usable as seg_id for ds_tail_stats.
- * A group outside [0, n_groups) sets DS_DEV_BAD_INSTANCE. Launches: 1 memset + 1 kernel. */
+ * A group outside [0, n_groups) sets DS_DEV_BAD_INSTANCE. Launches: 1 memset + 1 kernel.
+ * arrival_override (nullable; here and in ds_queue_depth, ds_latencies, ds_latency_stats): int64 device array indexed like
+ *   start_tick (out_off[i] + local request index) holding the arrival tick of every simulated request; when given it is
+ *   used instead of tr->arrival_tick. It is the arrival_out of ds_simulate_closed: in a closed loop (the
+ *   setup behind Tables VI-IX and Fig. 8) arrivals depend on the instance's policy, so the trace's array does not hold them. */
 int ds_estimation_error(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, const int64_t* out_off,
-                        const int64_t* est, const int64_t* start_tick, const int32_t* group, int32_t n_groups,
+                        const int64_t* arrival_override, const int64_t* est, const int64_t* start_tick, const int32_t* group, int32_t n_groups,
                         int64_t* out, int32_t* class_seg, void* stream);
 
 /* Queue depth per tenant tier over time (Fig. 8: "per-tenant queue depth"):
@@ -188,17 +209,18 @@ int ds_estimation_error(const ds_traces* tr, const ds_instance* inst, int64_t n_
  * depth [n_inst*n_samples*3] int32 device (written); t0 any tick, dt >= 1, n_samples >= 0 (host values).
  * Launches: 1 memset + 2 kernels. */
 int ds_queue_depth(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, const int64_t* out_off,
-                   const int64_t* start_tick, int64_t t0, int64_t dt, int64_t n_samples, int32_t* depth, void* stream);
+                   const int64_t* arrival_override, const int64_t* start_tick, int64_t t0, int64_t dt, int64_t n_samples, int32_t* depth, void* stream);
 
 /* ---------------------------------------------------------------------------------------------- (c)
  * Latency derivation (worker timestamps separate queueing from inference):
- *   e2e = done - arrival, qdelay = start - arrival, per simulated request (same indexing as start/done).
+ *   e2e = done - arrival, qdelay = start - arrival, per simulated request (same indexing as start/done);
+ *   arrival = tr->arrival_tick, or arrival_override (see ds_estimation_error) for closed-loop runs.
  * Segment ids for ds_tail_stats, with g = group[i] (nullable -> 0) and, if t_mid != NULL,
  *   g = 2*g + (arrival >= t_mid[trace]) (pre/post-drift phase, BASELINE.json:configs[4]):
  *   seg_tier = 3*g + tier (per-tier statistics), seg_all = g (overall). Either seg output may be NULL.
  * n_total = out_off[n_inst] must be passed by the caller (host value). Launches: 1 kernel. */
 int ds_latencies(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t n_total,
-                 const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, const int64_t* t_mid,
+                 const int64_t* arrival_override, const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, const int64_t* t_mid,
                  int64_t* e2e, int64_t* qdelay, int32_t* seg_tier, int32_t* seg_all, void* stream);
 
 /* Segmented percentiles by MSB-first radix select (PAPER.md:436 P50/P95/P99; Tables VI-VIII).
@@ -224,7 +246,7 @@ int ds_tail_stats(const int64_t* values, const int32_t* seg_id, int64_t n, int32
  *   32-bit keys + segment codes and the digit passes stream those instead of recomputing tick - arrival (same results,
  *   bit-exact; any other case silently takes the unstaged passes). Launches per wanted metric: 2 memsets + 2 + up to 8 x 2 kernels. */
 int ds_latency_stats(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, const int64_t* out_off,
-                     const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, int32_t n_groups,
+                     const int64_t* arrival_override, const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, int32_t n_groups,
                      const int64_t* t_mid, const int32_t* pct, int32_t n_pct, int64_t* e2e_out, int64_t* qdelay_out,
                      int64_t* count_out, void* workspace, size_t workspace_bytes, void* stream);
 

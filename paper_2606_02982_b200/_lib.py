@@ -50,15 +50,15 @@ def lib():
         L = C.CDLL(LIB_PATH)
         p, i64, i32, sz = C.c_void_p, C.c_int64, C.c_int32, C.c_size_t
         L.ds_characterize.argtypes = [p, i64, p, i64, p, p, p, sz, p]
-        L.ds_simulate.argtypes = [C.POINTER(DsTraces), C.POINTER(DsServer), p, i64, p, p, p, p, p, p, p, sz, p]
-        L.ds_simulate_est.argtypes = [C.POINTER(DsTraces), C.POINTER(DsServer), p, i64, p, p, p, p, p, p, p, p, sz, p]
-        L.ds_simulate_budget.argtypes = [C.POINTER(DsTraces), p, C.POINTER(DsBudget), C.POINTER(DsServer), p, i64, p, p, p, p, p, p, p, p, sz, p]
-        L.ds_simulate_closed.argtypes = [C.POINTER(DsTraces), p, C.POINTER(DsBudget), C.POINTER(DsServer), i32, i64, i64, p, i64, p, p, p, p, p, p, p, p, p, sz, p]
-        L.ds_estimation_error.argtypes = [C.POINTER(DsTraces), p, i64, p, p, p, p, i32, p, p, p]
-        L.ds_queue_depth.argtypes = [C.POINTER(DsTraces), p, i64, p, p, i64, i64, i64, p, p]
-        L.ds_latencies.argtypes = [C.POINTER(DsTraces), p, i64, p, i64, p, p, p, p, p, p, p, p, p]
+        L.ds_simulate.argtypes = [C.POINTER(DsTraces), C.POINTER(DsServer), p, i64, p, i64, p, p, p, p, p, p, sz, p]
+        L.ds_simulate_est.argtypes = [C.POINTER(DsTraces), C.POINTER(DsServer), p, i64, p, i64, p, p, p, p, p, p, p, sz, p]
+        L.ds_simulate_budget.argtypes = [C.POINTER(DsTraces), p, C.POINTER(DsBudget), C.POINTER(DsServer), p, i64, p, i64, p, p, p, p, p, p, p, sz, p]
+        L.ds_simulate_closed.argtypes = [C.POINTER(DsTraces), p, C.POINTER(DsBudget), C.POINTER(DsServer), i32, i64, i64, p, i64, p, i64, p, p, p, p, p, p, p, p, sz, p]
+        L.ds_estimation_error.argtypes = [C.POINTER(DsTraces), p, i64, p, p, p, p, p, i32, p, p, p]
+        L.ds_queue_depth.argtypes = [C.POINTER(DsTraces), p, i64, p, p, p, i64, i64, i64, p, p]
+        L.ds_latencies.argtypes = [C.POINTER(DsTraces), p, i64, p, i64, p, p, p, p, p, p, p, p, p, p]
         L.ds_tail_stats.argtypes = [p, p, i64, i32, C.POINTER(i32), i32, p, p, p, sz, p]
-        L.ds_latency_stats.argtypes = [C.POINTER(DsTraces), p, i64, p, p, p, p, i32, p, C.POINTER(i32), i32, p, p, p, p, sz, p]
+        L.ds_latency_stats.argtypes = [C.POINTER(DsTraces), p, i64, p, p, p, p, p, i32, p, C.POINTER(i32), i32, p, p, p, p, sz, p]
         L.ds_workspace_bytes.argtypes = [C.c_int, i64, i64]
         L.ds_workspace_bytes.restype = sz
         L.ds_device_status.argtypes = [p]

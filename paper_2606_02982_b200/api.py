@@ -100,11 +100,11 @@ def simulate(trace_off, arrival, tier, words, tokens, out_len, server, inst, out
     if est_out is not None:                     # ds_simulate_est: same call, also writes the frozen estimates
         _need_cuda(est_out)
         assert est_out.dtype == torch.int64 and est_out.numel() >= n_total
-        check("ds_simulate_est", lib().ds_simulate_est(C.byref(tr), C.byref(sv), _ptr(inst), n_inst, _ptr(out_off), _ptr(start),
+        check("ds_simulate_est", lib().ds_simulate_est(C.byref(tr), C.byref(sv), _ptr(inst), n_inst, _ptr(out_off), int(n_total), _ptr(start),
                                                        _ptr(done), _ptr(ema_final), _ptr(traj_off), _ptr(ema_traj), _ptr(est_out),
                                                        _ptr(workspace), workspace.numel(), _stream()))
         return start, done, ema_final
-    check("ds_simulate", lib().ds_simulate(C.byref(tr), C.byref(sv), _ptr(inst), n_inst, _ptr(out_off), _ptr(start), _ptr(done),
+    check("ds_simulate", lib().ds_simulate(C.byref(tr), C.byref(sv), _ptr(inst), n_inst, _ptr(out_off), int(n_total), _ptr(start), _ptr(done),
                                            _ptr(ema_final), _ptr(traj_off), _ptr(ema_traj), _ptr(workspace), workspace.numel(),
                                            _stream()))
     return start, done, ema_final
@@ -123,25 +123,25 @@ ERR_FIELDS = 11
 
 
 def estimation_error(trace_off, arrival, tier, words, tokens, out_len, inst, out_off, n_total, est, start=None, group=None,
-                     n_groups=1, want_class_seg=False, out=None):
+                     n_groups=1, want_class_seg=False, out=None, arrival_override=None):
     """ds_estimation_error -> sums int64[n_groups, 11] (and class_seg int32[n_total] if asked)."""
     tr = _traces(trace_off, arrival, tier, words, tokens, out_len)
-    _need_cuda(inst, out_off, est, start, group, out)
+    _need_cuda(inst, out_off, est, start, group, out, arrival_override)
     n_inst = inst.numel() // INSTANCE_BYTES
     dev = est.device
     if out is None:
         out = torch.empty((n_groups, ERR_FIELDS), dtype=torch.int64, device=dev)
     seg = torch.empty(n_total, dtype=torch.int32, device=dev) if want_class_seg else None
-    check("ds_estimation_error", lib().ds_estimation_error(C.byref(tr), _ptr(inst), n_inst, _ptr(out_off), _ptr(est), _ptr(start),
+    check("ds_estimation_error", lib().ds_estimation_error(C.byref(tr), _ptr(inst), n_inst, _ptr(out_off), _ptr(arrival_override), _ptr(est), _ptr(start),
                                                            _ptr(group), n_groups, _ptr(out), _ptr(seg), _stream()))
     return (out, seg) if want_class_seg else out
 
 
 def latencies(trace_off, arrival, tier, words, tokens, out_len, inst, out_off, n_total, start, done, group=None, t_mid=None,
-              want_seg_tier=True, want_seg_all=True, out=None):
+              want_seg_tier=True, want_seg_all=True, out=None, arrival_override=None):
     """ds_latencies -> (e2e, qdelay, seg_tier, seg_all)."""
     tr = _traces(trace_off, arrival, tier, words, tokens, out_len)
-    _need_cuda(inst, out_off, start, done, group, t_mid)
+    _need_cuda(inst, out_off, start, done, group, t_mid, arrival_override)
     n_inst = inst.numel() // INSTANCE_BYTES
     dev = start.device
     if out is not None:
@@ -152,7 +152,7 @@ def latencies(trace_off, arrival, tier, words, tokens, out_len, inst, out_off, n
         qd = torch.empty(n_total, dtype=torch.int64, device=dev)
         st = torch.empty(n_total, dtype=torch.int32, device=dev) if want_seg_tier else None
         sa = torch.empty(n_total, dtype=torch.int32, device=dev) if want_seg_all else None
-    check("ds_latencies", lib().ds_latencies(C.byref(tr), _ptr(inst), n_inst, _ptr(out_off), n_total, _ptr(start), _ptr(done),
+    check("ds_latencies", lib().ds_latencies(C.byref(tr), _ptr(inst), n_inst, _ptr(out_off), n_total, _ptr(arrival_override), _ptr(start), _ptr(done),
                                              _ptr(group), _ptr(t_mid), _ptr(e2e), _ptr(qd), _ptr(st), _ptr(sa), _stream()))
     return e2e, qd, st, sa
 
@@ -176,11 +176,11 @@ def tail_stats(values, seg_id, n_segments, pct=(50, 99), out=None, count_out=Non
 
 
 def latency_stats(trace_off, arrival, tier, words, tokens, out_len, inst, out_off, start, done, group, n_groups, t_mid=None,
-                  pct=(50, 99), e2e_out=None, qdelay_out=None, count_out=None, workspace=None, stage=True):
+                  pct=(50, 99), e2e_out=None, qdelay_out=None, count_out=None, workspace=None, stage=True, arrival_override=None):
     """ds_latency_stats -> (e2e_out, qdelay_out, count_out), each laid out [4*G, n_pct] / [4*G] with G = n_groups * phases:
     rows [0, 3G) are the (group, tier) segments 3*g+tier, rows [3G, 4G) the per-group overall segments."""
     tr = _traces(trace_off, arrival, tier, words, tokens, out_len)
-    _need_cuda(inst, out_off, start, done, group, t_mid, e2e_out, qdelay_out, count_out)
+    _need_cuda(inst, out_off, start, done, group, t_mid, e2e_out, qdelay_out, count_out, arrival_override)
     n_inst = inst.numel() // INSTANCE_BYTES
     dev = start.device
     G = n_groups * (2 if t_mid is not None else 1)
@@ -197,20 +197,21 @@ def latency_stats(trace_off, arrival, tier, words, tokens, out_len, inst, out_of
             nbytes += workspace_bytes(_lib.WS_LATENCY_STAGE, int((start if start is not None else done).numel()), 0)
         workspace = torch.empty(nbytes, dtype=torch.uint8, device=dev)
     arr = (C.c_int32 * n_pct)(*[int(x) for x in pct])
-    check("ds_latency_stats", lib().ds_latency_stats(C.byref(tr), _ptr(inst), n_inst, _ptr(out_off), _ptr(start), _ptr(done),
+    check("ds_latency_stats", lib().ds_latency_stats(C.byref(tr), _ptr(inst), n_inst, _ptr(out_off), _ptr(arrival_override), _ptr(start), _ptr(done),
                                                      _ptr(group), n_groups, _ptr(t_mid), arr, n_pct, _ptr(e2e_out), _ptr(qdelay_out),
                                                      _ptr(count_out), _ptr(workspace), workspace.numel(), _stream()))
     return e2e_out, qdelay_out, count_out
 
 
-def queue_depth(trace_off, arrival, tier, words, tokens, out_len, inst, out_off, start, t0, dt, n_samples, out=None):
+def queue_depth(trace_off, arrival, tier, words, tokens, out_len, inst, out_off, start, t0, dt, n_samples, out=None,
+                arrival_override=None):
     """ds_queue_depth -> depth int32[n_inst, n_samples, 3]."""
     tr = _traces(trace_off, arrival, tier, words, tokens, out_len)
-    _need_cuda(inst, out_off, start, out)
+    _need_cuda(inst, out_off, start, out, arrival_override)
     n_inst = inst.numel() // INSTANCE_BYTES
     if out is None:
         out = torch.empty((n_inst, int(n_samples), 3), dtype=torch.int32, device=start.device)
-    check("ds_queue_depth", lib().ds_queue_depth(C.byref(tr), _ptr(inst), n_inst, _ptr(out_off), _ptr(start), int(t0), int(dt),
+    check("ds_queue_depth", lib().ds_queue_depth(C.byref(tr), _ptr(inst), n_inst, _ptr(out_off), _ptr(arrival_override), _ptr(start), int(t0), int(dt),
                                                  int(n_samples), _ptr(out), _stream()))
     return out
 
@@ -240,12 +241,12 @@ def simulate_budget(trace_off, arrival, tier, words, tokens, out_len, category, 
             arrival_out = torch.empty(n_total, dtype=torch.int64, device=dev)
         _need_cuda(arrival_out)
         check("ds_simulate_closed", lib().ds_simulate_closed(C.byref(tr), _ptr(category), C.byref(bp), C.byref(sv), int(n_clients),
-                                                             int(think_ticks), int(batch_wait), _ptr(inst), n_inst, _ptr(out_off), _ptr(arrival_out),
+                                                             int(think_ticks), int(batch_wait), _ptr(inst), n_inst, _ptr(out_off), int(n_total), _ptr(arrival_out),
                                                              _ptr(start), _ptr(done), _ptr(ema_final), _ptr(traj_off), _ptr(ema_traj),
                                                              _ptr(est_out), _ptr(workspace), workspace.numel(), _stream()))
         return start, done, ema_final, arrival_out
     check("ds_simulate_budget", lib().ds_simulate_budget(C.byref(tr), _ptr(category), C.byref(bp), C.byref(sv), _ptr(inst), n_inst,
-                                                         _ptr(out_off), _ptr(start), _ptr(done), _ptr(ema_final), _ptr(traj_off),
+                                                         _ptr(out_off), int(n_total), _ptr(start), _ptr(done), _ptr(ema_final), _ptr(traj_off),
                                                          _ptr(ema_traj), _ptr(est_out), _ptr(workspace), workspace.numel(), _stream()))
     return start, done, ema_final
 

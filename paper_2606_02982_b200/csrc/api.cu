@@ -2,6 +2,7 @@
 #include <atomic>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 
 #include "common.cuh"
 
@@ -12,14 +13,38 @@ __device__ unsigned int g_status_word = 0;
 static thread_local char t_cuda_err[256] = "";
 static std::atomic<long long> g_launches{0};
 
-unsigned int* status_ptr() {
-  static unsigned int* p = nullptr;
-  if (!p) {
+// Per-DEVICE state (a process may drive several devices, one after the other or from several threads): the status word's
+// address, the SM count and which kernels already have their dynamic-shared-memory attribute set on that device.
+namespace {
+struct DeviceState { unsigned int* status = nullptr; int num_sms = 0; unsigned attr_mask = 0; bool init = false; };
+constexpr int kMaxDevices = 64;
+DeviceState g_dev[kMaxDevices];
+std::mutex g_dev_mu;
+DeviceState* device_state() {   // state of the calling thread's current device, nullptr on a CUDA error
+  int d = -1;
+  if (cudaGetDevice(&d) != cudaSuccess || d < 0 || d >= kMaxDevices) return nullptr;
+  std::lock_guard<std::mutex> lk(g_dev_mu);
+  DeviceState& st = g_dev[d];
+  if (!st.init) {
     void* q = nullptr;
     if (cudaGetSymbolAddress(&q, g_status_word) != cudaSuccess) return nullptr;
-    p = (unsigned int*)q;
+    int n = 0;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, d) != cudaSuccess || n < 1) return nullptr;
+    st.status = (unsigned int*)q; st.num_sms = n; st.init = true;
   }
-  return p;
+  return &st;
+}
+}  // namespace
+
+unsigned int* status_ptr() { DeviceState* st = device_state(); return st ? st->status : nullptr; }
+int num_sms() { DeviceState* st = device_state(); return st ? st->num_sms : 0; }
+bool attr_needed(int which) {
+  DeviceState* st = device_state();
+  if (!st) return true;
+  std::lock_guard<std::mutex> lk(g_dev_mu);
+  const bool need = !(st->attr_mask & (1u << which));
+  st->attr_mask |= 1u << which;
+  return need;
 }
 
 void note_launch(int n) { g_launches += n; }

@@ -592,12 +592,9 @@ extern "C" int ds_characterize(const uint8_t* bytes, int64_t n_bytes, const int6
             CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return cuda_fail(cudaErrorInvalidValue);
   }
-  static bool attr_set = false;
-  if (!attr_set) {
+  if (attr_needed(DS_ATTR_K1))
     DS_CUDA(cudaFuncSetAttribute(k1::characterize_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(k1::Smem)));
-    attr_set = true;
-  }
-  long long grid = (long long)kNumSMs * k1::kCtasPerSM;
+  long long grid = (long long)num_sms() * k1::kCtasPerSM;
   const long long need = (n_chunks + k1::kWarps - 1) / k1::kWarps;
   if (grid > need) grid = need;
   const k1::Mul mu = {2u, 4u, 16u, 1u << 31, 1u << 30, 1u << 28, 1u << 16, 0u - (1u << 16)};

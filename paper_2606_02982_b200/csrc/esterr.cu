@@ -13,7 +13,7 @@ __global__ void __launch_bounds__(256) esterr_kernel(const int64_t* __restrict__
                                                      const int32_t* __restrict__ tokens, const int32_t* __restrict__ out_len,
                                                      const ds_instance* __restrict__ inst,
                                                      long long n_inst, const int64_t* __restrict__ out_off,
-                                                     const int64_t* __restrict__ est, const int64_t* __restrict__ start,
+                                                     const int64_t* __restrict__ arr_ov, const int64_t* __restrict__ est, const int64_t* __restrict__ start,
                                                      const int32_t* __restrict__ group, int n_groups, unsigned long long* out,
                                                      int32_t* __restrict__ class_seg, unsigned int* status) {
   const int lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
@@ -24,13 +24,14 @@ __global__ void __launch_bounds__(256) esterr_kernel(const int64_t* __restrict__
     const int g = group ? group[ii] : 0;
     if (g < 0 || g >= n_groups) { if (lane == 0) atomicOr(status, DS_DEV_BAD_INSTANCE); continue; }
     const bool with_out = inst[ii].estimator >= DS_BUDGET_SPLIT;     // budget estimators predict input + output tokens (Eq. 1)
+    const int64_t* __restrict__ ap = arr_ov ? arr_ov + oo : arrival + lo;   // closed loop: the instance's own arrival ticks
     unsigned long long acc[kFields];
 #pragma unroll
     for (int k = 0; k < kFields; ++k) acc[k] = 0ull;
     for (long long r = lane; r < n; r += 32) {
       const long long e = est[oo + r], P = (long long)tokens[lo + r] + (with_out ? (long long)out_len[lo + r] : 0ll), err = e - P;
       const int cls = e <= 128 ? 0 : (e <= 512 ? 1 : 2);                     // Eq. 4
-      const unsigned long long qd = start ? (unsigned long long)(start[oo + r] - arrival[lo + r]) : 0ull;
+      const unsigned long long qd = start ? (unsigned long long)(start[oo + r] - ap[r]) : 0ull;
       acc[0] += 1ull; acc[1] += (unsigned long long)(err < 0 ? -err : err); acc[2] += (unsigned long long)(err * err);
       acc[3] += (unsigned long long)e; acc[4] += (unsigned long long)P;
 #pragma unroll
@@ -55,19 +56,19 @@ __global__ void __launch_bounds__(256) esterr_kernel(const int64_t* __restrict__
 }  // namespace ds
 
 extern "C" int ds_estimation_error(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, const int64_t* out_off,
-                                   const int64_t* est, const int64_t* start_tick, const int32_t* group, int32_t n_groups,
+                                   const int64_t* arrival_override, const int64_t* est, const int64_t* start_tick, const int32_t* group, int32_t n_groups,
                                    int64_t* out, int32_t* class_seg, void* stream) {
   using namespace ds;
   if (!tr || n_inst < 0 || n_groups < 1 || !out) return DS_EINVAL;
-  if (n_inst > 0 && (!inst || !out_off || !est || !tr->trace_off || !tr->tokens || !tr->out_len || (start_tick && !tr->arrival_tick))) return DS_EINVAL;
+  if (n_inst > 0 && (!inst || !out_off || !est || !tr->trace_off || !tr->tokens || !tr->out_len || (start_tick && !arrival_override && !tr->arrival_tick))) return DS_EINVAL;
   cudaStream_t s = (cudaStream_t)stream;
   unsigned int* status = status_ptr();
   if (!status) return cuda_fail(cudaGetLastError());
   DS_CUDA(cudaMemsetAsync(out, 0, sizeof(int64_t) * k4::kFields * (size_t)n_groups, s));
   if (n_inst == 0) return DS_OK;
   long long blocks = (n_inst + 7) / 8;
-  if (blocks > kNumSMs * 8) blocks = kNumSMs * 8;
-  k4::esterr_kernel<<<(unsigned)blocks, 256, 0, s>>>(tr->trace_off, tr->arrival_tick, tr->tokens, tr->out_len, inst, n_inst, out_off, est, start_tick,
+  if (blocks > num_sms() * 8) blocks = num_sms() * 8;
+  k4::esterr_kernel<<<(unsigned)blocks, 256, 0, s>>>(tr->trace_off, tr->arrival_tick, tr->tokens, tr->out_len, inst, n_inst, out_off, arrival_override, est, start_tick,
                                                     group, n_groups, (unsigned long long*)out, class_seg, status);
   note_launch();
   DS_CUDA(cudaGetLastError());

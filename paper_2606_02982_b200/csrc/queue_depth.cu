@@ -20,17 +20,18 @@ __device__ __forceinline__ long long first_sample(long long x, long long t0, lon
 __global__ void __launch_bounds__(256) diff_kernel(const int64_t* __restrict__ trace_off, const int64_t* __restrict__ arrival,
                                                    const uint8_t* __restrict__ tier, const ds_instance* __restrict__ inst,
                                                    long long n_inst, const int64_t* __restrict__ out_off,
-                                                   const int64_t* __restrict__ start, long long t0, long long dt,
+                                                   const int64_t* __restrict__ arr_ov, const int64_t* __restrict__ start, long long t0, long long dt,
                                                    long long n_samples, int* __restrict__ depth) {
   const int lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
   for (long long ii = (long long)blockIdx.x * nwarp + (threadIdx.x >> 5); ii < n_inst; ii += (long long)gridDim.x * nwarp) {
     const int t = inst[ii].trace;
     const long long lo = trace_off[t], n = trace_off[t + 1] - lo, oo = out_off[ii];
     int* row = depth + ii * n_samples * 3;
+    const int64_t* __restrict__ ap = arr_ov ? arr_ov + oo : arrival + lo;   // closed loop: the instance's own arrival ticks
     for (long long r = lane; r < n; r += 32) {
       const int k = tier[lo + r];
       if (k > 2) continue;                                  // (ds_simulate reports bad tiers)
-      const long long ja = first_sample(arrival[lo + r], t0, dt, n_samples);
+      const long long ja = first_sample(ap[r], t0, dt, n_samples);
       const long long js = first_sample(start[oo + r], t0, dt, n_samples);
       if (ja < js) {
         atomicAdd(row + ja * 3 + k, 1);
@@ -65,16 +66,16 @@ __global__ void __launch_bounds__(256) scan_kernel(long long n_inst, long long n
 }  // namespace ds
 
 extern "C" int ds_queue_depth(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, const int64_t* out_off,
-                              const int64_t* start_tick, int64_t t0, int64_t dt, int64_t n_samples, int32_t* depth, void* stream) {
+                              const int64_t* arrival_override, const int64_t* start_tick, int64_t t0, int64_t dt, int64_t n_samples, int32_t* depth, void* stream) {
   using namespace ds;
   if (!tr || n_inst < 0 || dt < 1 || n_samples < 0) return DS_EINVAL;
   if (n_inst == 0 || n_samples == 0) return DS_OK;
-  if (!inst || !out_off || !start_tick || !depth || !tr->trace_off || !tr->arrival_tick || !tr->tier) return DS_EINVAL;
+  if (!inst || !out_off || !start_tick || !depth || !tr->trace_off || (!arrival_override && !tr->arrival_tick) || !tr->tier) return DS_EINVAL;
   cudaStream_t s = (cudaStream_t)stream;
   DS_CUDA(cudaMemsetAsync(depth, 0, sizeof(int32_t) * 3 * (size_t)n_samples * (size_t)n_inst, s));
   long long blocks = (n_inst + 7) / 8;
-  if (blocks > kNumSMs * 8) blocks = kNumSMs * 8;
-  k5::diff_kernel<<<(unsigned)blocks, 256, 0, s>>>(tr->trace_off, tr->arrival_tick, tr->tier, inst, n_inst, out_off, start_tick, t0, dt,
+  if (blocks > num_sms() * 8) blocks = num_sms() * 8;
+  k5::diff_kernel<<<(unsigned)blocks, 256, 0, s>>>(tr->trace_off, tr->arrival_tick, tr->tier, inst, n_inst, out_off, arrival_override, start_tick, t0, dt,
                                                   n_samples, depth);
   k5::scan_kernel<<<(unsigned)blocks, 256, 0, s>>>(n_inst, n_samples, depth);
   note_launch(2);

@@ -51,6 +51,8 @@ struct Params {
   int32_t n_clients; int64_t think; int64_t* arrival_out;   // closed-loop arrivals (ds_simulate_closed), n_clients = 0: open loop
   int64_t batch_wait;                                        // ds_simulate_closed: dispatch gate of an idle server (0 = none)
   unsigned long long* heap_ws; unsigned int* counter; unsigned int* status; const unsigned int* perm;
+  int64_t n_total;                                           // out_off[n_inst] as stated by the caller: size of every per-request output and of the heap region
+  unsigned n_sms;
 };
 
 // 64-bit warp min (keys are unique, so the min identifies its lane)
@@ -138,6 +140,10 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   const int32_t* __restrict__ P = p.tokens + lo;
   const int32_t* __restrict__ O = p.out_len + lo;
   const long long oo = p.out_off[inst_id];
+  if (oo < 0 || oo + n64 > p.n_total) {                     // this instance's outputs (and SJF heap region) would leave the caller's arrays
+    if (lane == 0) atomicOr(p.status, DS_DEV_BAD_OUT_OFF);
+    return;
+  }
   int64_t* __restrict__ st = p.start_tick + oo;
   int64_t* dn = p.done_tick + oo;
   const int32_t* __restrict__ BASE = split ? W : P;
@@ -174,8 +180,10 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   const bool closed = kBudget && p.n_clients > 0;
   int64_t* arr_d = closed ? p.arrival_out + oo : nullptr;
   int released = n;
+  long long last_rel = 0;                // closed loop: arrival tick of the most recently submitted request (contract: non-decreasing)
   if (closed) {
     released = p.n_clients < n ? p.n_clients : n;
+    last_rel = released > 0 ? (long long)arr[released - 1] : 0;
     for (int i = lane; i < n; i += 32) __stcg(arr_d + i, i < released ? arr[i] : kInf);
     __syncwarp();
   }
@@ -184,14 +192,16 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   // arrival window: lane holds request wb+lane
   int wb = 0; long long w_arr = kInf; int w_tier = 0, w_base = 0, w_cat = 0;
   auto load_window = [&]() {
+    const long long w_prev_last = wb > 0 ? shfl_i64(w_arr, 31) : 0;   // last arrival of the window being replaced (lane 0's predecessor)
     const int i = wb + lane;
     if (i < n) { w_arr = arr_at(i); w_tier = tier[i]; w_base = BASE[i]; } else { w_arr = kInf; w_tier = 0; w_base = 0; }
     if (kBudget) {
       w_cat = i < n ? (int)cat[i] : 0;
       if (w_cat > 3) { atomicOr(p.status, DS_DEV_BAD_TRACE); w_cat = 3; }
     }
-    const long long prev = __shfl_up_sync(kFull, w_arr, 1);
-    const bool bad = (i < n) && (w_tier > 2 || w_base < 0 || w_arr < 0 || (lane > 0 && w_arr < prev) || O[i] < 1);   // (out_len checked here, 32 at a time)
+    long long prev = __shfl_up_sync(kFull, w_arr, 1);
+    if (lane == 0) prev = w_prev_last;
+    const bool bad = (i < n) && (w_tier > 2 || w_base < 0 || w_arr < 0 || w_arr < prev || O[i] < 1);   // (out_len checked here, 32 at a time)
     if (bad) atomicOr(p.status, DS_DEV_BAD_TRACE);
     if (w_tier > 2) w_tier = 2;
     if (w_base < 0) w_base = 0;
@@ -319,6 +329,8 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       ++done;
       if (kBudget && closed && released < n) {                // the client whose request completed submits the next one
         const long long t_new = now + p.think;
+        if (t_new < last_rel && lane == 0) atomicOr(p.status, DS_DEV_BAD_TRACE);   // a client's start tick lies after this release
+        last_rel = t_new;
         if (lane == 0) __stcg(arr_d + released, t_new);
         if (lane == released - wb) w_arr = t_new;             // (unsigned compare not needed: released >= next >= wb)
         if (released == next) an = t_new;
@@ -574,7 +586,7 @@ __global__ void __launch_bounds__(k2::kWarpsPerBlock * 32, DS_K2_MIN_BLOCKS) sim
   // instance per policy on configs[1]); the split only sets the starting point, stealing evens out the rest.
   unsigned smid;
   asm("mov.u32 %0, %%smid;" : "=r"(smid));
-  const unsigned sm148 = smid % 148u;
+  const unsigned sm148 = (smid % p.n_sms) * 148u / p.n_sms;      // position of this SM on the 148-SM scale the split was measured on
   int bucket = sm148 < 26 ? 0 : sm148 < 57 ? 1 : sm148 < 92 ? 2 : sm148 < 122 ? 3 : 4;
   for (;;) {
     unsigned k = 0;
@@ -632,11 +644,11 @@ size_t ws_simulate(int64_t total_requests, int64_t n_inst) {
 }  // namespace ds
 static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_budget* bp, int32_t n_clients, int64_t think_ticks,
                          int64_t batch_wait, int64_t* arrival_out, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
-                         const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
+                         const int64_t* out_off, int64_t n_total, int64_t* start_tick, int64_t* done_tick, double* ema_final,
                          const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace, size_t workspace_bytes,
                          void* stream) {
   using namespace ds;
-  if (!tr || !sv || n_inst < 0) return DS_EINVAL;
+  if (!tr || !sv || n_inst < 0 || n_total < 0) return DS_EINVAL;
   if (n_inst == 0) return DS_OK;
   if (!inst || !out_off || !start_tick || !done_tick || !ema_final || !workspace) return DS_EINVAL;
   if (tr->n_traces < 1 || !tr->trace_off || !tr->arrival_tick || !tr->tier || !tr->words || !tr->tokens || !tr->out_len) return DS_EINVAL;
@@ -651,7 +663,12 @@ static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_
     for (int t = 0; t < 3; ++t) if (!(bp->s_tenant[t] > 0.0)) return DS_EINVAL;
     if (!(bp->f_slope >= 0.0) || !(bp->f_max >= 1.0)) return DS_EINVAL;
   }
-  if (workspace_bytes < 256 + perm_bytes(n_inst)) return DS_ENOMEM;
+  // the whole documented workspace is required: header + permutation + one SJF heap slot per simulated request (the heap
+  // region is only touched by SJF instances with more than kHeapSmem requests queued, but which launch will need it is
+  // not known on the host)
+  if (workspace_bytes < ws_simulate(n_total, n_inst)) return DS_ENOMEM;
+  const int n_sms = num_sms();
+  if (n_sms < 1) return cuda_fail(cudaGetLastError());
   cudaStream_t s = (cudaStream_t)stream;
   k2::Params p;
   p.trace_off = tr->trace_off; p.arrival = tr->arrival_tick; p.tier = tr->tier; p.words = tr->words; p.tokens = tr->tokens;
@@ -670,8 +687,7 @@ static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_
   p.heap_ws = (unsigned long long*)((char*)workspace + 256 + perm_bytes(n_inst));
   p.status = status_ptr();
   if (!p.status) return cuda_fail(cudaGetLastError());
-  // the heap region is only touched by SJF instances beyond kHeapSmem queued requests; its size is checked here
-  // against the documented formula only when it can be needed at all (caller passes total requests to the query)
+  p.n_total = n_total; p.n_sms = (unsigned)n_sms;
   DS_CUDA(cudaMemsetAsync(workspace, 0, 256, s));
   k2::order_kernel<<<1, 1024, 0, s>>>(inst, n_inst, perm, (unsigned int*)workspace);
   note_launch();
@@ -680,7 +696,7 @@ static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_
   auto launch = [&](auto kern) -> int {
     DS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, 0));
     if (per_sm < 1) per_sm = 1;
-    long long blocks = (long long)kNumSMs * per_sm;
+    long long blocks = (long long)n_sms * per_sm;
     const long long need = (n_inst + k2::kWarpsPerBlock - 1) / k2::kWarpsPerBlock;
     if (blocks > need) blocks = need;
     kern<<<(unsigned)blocks, threads, 0, s>>>(p);
@@ -701,37 +717,37 @@ static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_
 }
 
 extern "C" int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
-                           const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
+                           const int64_t* out_off, int64_t n_total, int64_t* start_tick, int64_t* done_tick, double* ema_final,
                            const int64_t* traj_off, double* ema_traj, void* workspace, size_t workspace_bytes, void* stream) {
-  return simulate_impl(tr, nullptr, nullptr, 0, 0, 0, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, nullptr, workspace,
+  return simulate_impl(tr, nullptr, nullptr, 0, 0, 0, nullptr, sv, inst, n_inst, out_off, n_total, start_tick, done_tick, ema_final, traj_off, ema_traj, nullptr, workspace,
                        workspace_bytes, stream);
 }
 
 extern "C" int ds_simulate_est(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
-                               const int64_t* out_off, int64_t* start_tick, int64_t* done_tick, double* ema_final,
+                               const int64_t* out_off, int64_t n_total, int64_t* start_tick, int64_t* done_tick, double* ema_final,
                                const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace,
                                size_t workspace_bytes, void* stream) {
   if (n_inst > 0 && !est_out) return DS_EINVAL;
-  return simulate_impl(tr, nullptr, nullptr, 0, 0, 0, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out, workspace,
+  return simulate_impl(tr, nullptr, nullptr, 0, 0, 0, nullptr, sv, inst, n_inst, out_off, n_total, start_tick, done_tick, ema_final, traj_off, ema_traj, est_out, workspace,
                        workspace_bytes, stream);
 }
 
 extern "C" int ds_simulate_budget(const ds_traces* tr, const uint8_t* category, const ds_budget* bp, const ds_server* sv,
-                                  const ds_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t* start_tick,
+                                  const ds_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t n_total, int64_t* start_tick,
                                   int64_t* done_tick, double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out,
                                   void* workspace, size_t workspace_bytes, void* stream) {
   if (!bp) return DS_EINVAL;
-  return simulate_impl(tr, category, bp, 0, 0, 0, nullptr, sv, inst, n_inst, out_off, start_tick, done_tick, ema_final, traj_off, ema_traj,
+  return simulate_impl(tr, category, bp, 0, 0, 0, nullptr, sv, inst, n_inst, out_off, n_total, start_tick, done_tick, ema_final, traj_off, ema_traj,
                        est_out, workspace, workspace_bytes, stream);
 }
 
 extern "C" int ds_simulate_closed(const ds_traces* tr, const uint8_t* category, const ds_budget* bp, const ds_server* sv,
                                   int32_t n_clients, int64_t think_ticks, int64_t batch_wait_ticks, const ds_instance* inst,
                                   int64_t n_inst,
-                                  const int64_t* out_off, int64_t* arrival_out, int64_t* start_tick, int64_t* done_tick,
+                                  const int64_t* out_off, int64_t n_total, int64_t* arrival_out, int64_t* start_tick, int64_t* done_tick,
                                   double* ema_final, const int64_t* traj_off, double* ema_traj, int64_t* est_out, void* workspace,
                                   size_t workspace_bytes, void* stream) {
   if (!bp || n_clients < 1) return DS_EINVAL;
-  return simulate_impl(tr, category, bp, n_clients, think_ticks, batch_wait_ticks, arrival_out, sv, inst, n_inst, out_off, start_tick, done_tick,
+  return simulate_impl(tr, category, bp, n_clients, think_ticks, batch_wait_ticks, arrival_out, sv, inst, n_inst, out_off, n_total, start_tick, done_tick,
                        ema_final, traj_off, ema_traj, est_out, workspace, workspace_bytes, stream);
 }

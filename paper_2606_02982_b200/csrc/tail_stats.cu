@@ -51,7 +51,8 @@ inline Layout make_layout(void* base, int64_t n_seg, int64_t n_pct) {
 
 __global__ void latencies_kernel(const int64_t* __restrict__ trace_off, const int64_t* __restrict__ arrival,
                                  const uint8_t* __restrict__ tier, const ds_instance* __restrict__ inst,
-                                 const int64_t* __restrict__ out_off, const int64_t* __restrict__ start,
+                                 const int64_t* __restrict__ out_off, const int64_t* __restrict__ arr_ov,
+                                 const int64_t* __restrict__ start,
                                  const int64_t* __restrict__ done, const int32_t* __restrict__ group,
                                  const int64_t* __restrict__ t_mid, int64_t* __restrict__ e2e, int64_t* __restrict__ qd,
                                  int32_t* __restrict__ seg_tier, int32_t* __restrict__ seg_all) {
@@ -61,8 +62,9 @@ __global__ void latencies_kernel(const int64_t* __restrict__ trace_off, const in
   const int g0 = group ? group[ii] : 0;
   const bool ph = t_mid != nullptr;
   const long long tm = ph ? t_mid[t] : 0;
+  const int64_t* __restrict__ ap = arr_ov ? arr_ov + oo : arrival + lo;   // closed loop: the instance's own arrival ticks
   for (long long r = threadIdx.x; r < n; r += blockDim.x) {
-    const long long a = arrival[lo + r];
+    const long long a = ap[r];
     e2e[oo + r] = done[oo + r] - a;
     qd[oo + r] = start[oo + r] - a;
     const int g = ph ? g0 * 2 + (a >= tm ? 1 : 0) : g0;
@@ -220,6 +222,7 @@ __global__ void select_kernel(int n_seg, int n_pct, int d, const Ws* hdr, const 
 // counted in two segments: 3*g+tier ("tier" block, 3*G segments) and 3*G+g ("all" block, G segments).
 struct LatArgs {
   const int64_t* trace_off; const int64_t* arrival; const uint8_t* tier; const ds_instance* inst; const int64_t* out_off;
+  const int64_t* arr_ov;   // nullable: per-instance arrival ticks (closed loop), indexed like ticks
   const int64_t* ticks; const int32_t* group; const int64_t* t_mid; long long n_inst; int n_groups;   // groups after phases
   // Staging (optional, the part of the workspace beyond the histograms): the count pass leaves the low 32 bits of every key
   // and its segment code 3*g+tier (255 = not counted) at the request's output index. When every key agrees on bits 32..63
@@ -359,13 +362,14 @@ __global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pc
         for (long long j = oo + n + lane; j < oe; j += 32) a.scode[j] = 255;
       }
     }
+    const int64_t* __restrict__ ap = a.arr_ov ? a.arr_ov + oo : a.arrival + lo;
     for (long long base = 0; base < n; base += 32 * kUnroll) {   // warp-uniform trip count
       long long av[kUnroll], tv[kUnroll]; int tr[kUnroll];
 #pragma unroll
       for (int u = 0; u < kUnroll; ++u) {
         const long long r = base + u * 32 + lane;
         const bool in = r < n;
-        av[u] = in ? a.arrival[lo + r] : 0; tv[u] = in ? a.ticks[oo + r] : 0; tr[u] = in ? (int)a.tier[lo + r] : -1;
+        av[u] = in ? ap[r] : 0; tv[u] = in ? a.ticks[oo + r] : 0; tr[u] = in ? (int)a.tier[lo + r] : -1;
       }
 #pragma unroll
       for (int u = 0; u < kUnroll; ++u) {
@@ -434,14 +438,14 @@ size_t ws_latency_stage(int64_t n_total) { return n_total > 0 ? align_up(5 * (si
 }  // namespace ds
 
 extern "C" int ds_latencies(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, const int64_t* out_off, int64_t n_total,
-                            const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, const int64_t* t_mid,
+                            const int64_t* arrival_override, const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, const int64_t* t_mid,
                             int64_t* e2e, int64_t* qdelay, int32_t* seg_tier, int32_t* seg_all, void* stream) {
   using namespace ds;
   if (!tr || n_inst < 0 || n_total < 0) return DS_EINVAL;
   if (n_inst == 0 || n_total == 0) return DS_OK;
   if (!inst || !out_off || !start_tick || !done_tick || !e2e || !qdelay || n_inst > 0x7fffffff) return DS_EINVAL;
   k3::latencies_kernel<<<(unsigned)n_inst, 256, 0, (cudaStream_t)stream>>>(tr->trace_off, tr->arrival_tick, tr->tier, inst, out_off,
-                                                                        start_tick, done_tick, group, t_mid, e2e, qdelay, seg_tier, seg_all);
+                                                                        arrival_override, start_tick, done_tick, group, t_mid, e2e, qdelay, seg_tier, seg_all);
   note_launch();
   DS_CUDA(cudaGetLastError());
   return DS_OK;
@@ -463,7 +467,7 @@ extern "C" int ds_tail_stats(const int64_t* values, const int32_t* seg_id, int64
   const int nsq = n_segments * n_pct;
   const int threads = 512;
   long long blocks = (n + threads * k3::kUnroll - 1) / (threads * k3::kUnroll);
-  if (blocks > kNumSMs * 4) blocks = kNumSMs * 4;
+  if (blocks > num_sms() * 4) blocks = num_sms() * 4;
   if (blocks < 1) blocks = 1;
   const size_t csm = n_segments <= 4096 ? sizeof(unsigned) * (size_t)n_segments : 0;
   k3::count_kernel<<<(unsigned)blocks, threads, csm, s>>>(values, seg_id, n, n_segments, L.hdr, L.counts);
@@ -471,15 +475,12 @@ extern "C" int ds_tail_stats(const int64_t* values, const int32_t* seg_id, int64
   note_launch(2);
   const size_t hsm = sizeof(unsigned) * 256 * (size_t)nsq;
   const bool priv = hsm <= 160 * 1024;
-  static bool attr_set = false;
-  if (priv && !attr_set) {
+  if (priv && attr_needed(DS_ATTR_K3_HIST))
     DS_CUDA(cudaFuncSetAttribute(k3::hist_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
-    attr_set = true;
-  }
   long long per_sm = priv ? (long long)(200 * 1024) / (long long)(hsm + 1024) : 4;   // resident blocks by shared memory
   if (per_sm > 4) per_sm = 4;
   if (per_sm < 1) per_sm = 1;
-  long long hblocks = priv ? (long long)kNumSMs * per_sm : blocks;
+  long long hblocks = priv ? (long long)num_sms() * per_sm : blocks;
   if (hblocks > blocks) hblocks = blocks;
   for (int d = 7; d >= 0; --d) {
     if (priv) k3::hist_kernel<true><<<(unsigned)hblocks, threads, hsm, s>>>(values, seg_id, n, n_segments, n_pct, d, L.hdr, L.prefix, L.hist);
@@ -492,13 +493,13 @@ extern "C" int ds_tail_stats(const int64_t* values, const int32_t* seg_id, int64
 }
 
 extern "C" int ds_latency_stats(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, const int64_t* out_off,
-                                const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, int32_t n_groups,
+                                const int64_t* arrival_override, const int64_t* start_tick, const int64_t* done_tick, const int32_t* group, int32_t n_groups,
                                 const int64_t* t_mid, const int32_t* pct, int32_t n_pct, int64_t* e2e_out, int64_t* qdelay_out,
                                 int64_t* count_out, void* workspace, size_t workspace_bytes, void* stream) {
   using namespace ds;
   if (!tr || n_inst < 0 || n_groups < 1 || n_pct < 1 || n_pct > k3::kMaxPct || !pct || !workspace) return DS_EINVAL;
   if (!e2e_out && !qdelay_out) return DS_EINVAL;
-  if (n_inst > 0 && (!inst || !out_off || !tr->trace_off || !tr->arrival_tick || !tr->tier)) return DS_EINVAL;
+  if (n_inst > 0 && (!inst || !out_off || !tr->trace_off || (!arrival_override && !tr->arrival_tick) || !tr->tier)) return DS_EINVAL;
   if ((e2e_out && !done_tick) || (qdelay_out && !start_tick)) { if (n_inst > 0) return DS_EINVAL; }
   const int G = n_groups * (t_mid ? 2 : 1), n_seg = 4 * G, nsq = n_seg * n_pct;
   const size_t hsm = sizeof(unsigned) * 256 * (size_t)nsq;
@@ -508,15 +509,12 @@ extern "C" int ds_latency_stats(const ds_traces* tr, const ds_instance* inst, in
   k3::Layout L = k3::make_layout(workspace, n_seg, n_pct);
   if (workspace_bytes < L.total) return DS_ENOMEM;
   cudaStream_t s = (cudaStream_t)stream;
-  static bool attr_set = false;
-  if (!attr_set) {
+  if (attr_needed(DS_ATTR_K3_LAT))
     DS_CUDA(cudaFuncSetAttribute(k3::lat_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-    attr_set = true;
-  }
   long long per_sm = (long long)(200 * 1024) / (long long)(hsm + 1024);
   if (per_sm > 3) per_sm = 3;
   if (per_sm < 1) per_sm = 1;
-  long long blocks = (long long)kNumSMs * per_sm;
+  long long blocks = (long long)num_sms() * per_sm;
   if (blocks > (n_inst + 15) / 16) blocks = (n_inst + 15) / 16;
   if (blocks < 1) blocks = 1;
   for (int metric = 0; metric < 2; ++metric) {
@@ -530,7 +528,7 @@ extern "C" int ds_latency_stats(const ds_traces* tr, const ds_instance* inst, in
       note_launch(2);
       continue;
     }
-    k3::LatArgs a{tr->trace_off, tr->arrival_tick, tr->tier, inst, out_off, metric == 0 ? done_tick : start_tick, group, t_mid,
+    k3::LatArgs a{tr->trace_off, tr->arrival_tick, tr->tier, inst, out_off, arrival_override, metric == 0 ? done_tick : start_tick, group, t_mid,
                   (long long)n_inst, G, nullptr, nullptr, 0};
     // whatever the caller's workspace holds beyond the histograms is the staging area (5 bytes per simulated request)
     const size_t extra = workspace_bytes - L.total;

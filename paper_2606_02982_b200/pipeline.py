@@ -12,7 +12,9 @@ from . import _lib, api
 class HotPath:
     """Device-resident buffers for one workload (see workload.Workload) and the step that runs the path."""
 
-    def __init__(self, wl_obj, device="cuda:0", pct=(50, 99), fused=True):
+    def __init__(self, wl_obj, device="cuda:0", pct=(50, 99), fused=True, share=None):
+        """share: another HotPath of the same workload whose OUTPUT buffers and workspaces this one reuses (only the
+        inputs are private): the slots of a HostPipeline whose outputs do not fit twice (configs[3]: 98 GB)."""
         c = wl_obj
         self.c = c
         self.dev = torch.device(device)
@@ -35,6 +37,12 @@ class HotPath:
         self.n_inst = c.n_inst
         self.n_groups = c.n_groups * (2 if c.t_mid is not None else 1)
         n, dev = self.n_total, self.dev
+        self.n_text_prompts = 0 if self.offsets is None else self.offsets.numel() - 1   # (a text sample may cover fewer prompts)
+        if share is not None:
+            for k in ("start", "done", "ema_final", "traj_off", "ema_traj", "ws_char", "ws_sim", "ws_tail", "e2e_stats", "qd_stats",
+                      "counts4", "stats", "counts", "e2e", "qdelay", "seg_tier", "seg_all"):
+                setattr(self, k, getattr(share, k))
+            return
         self.start = torch.empty(n, dtype=torch.int64, device=dev)
         self.done = torch.empty(n, dtype=torch.int64, device=dev)
         self.ema_final = torch.empty((self.n_inst, 3), dtype=torch.float64, device=dev)
@@ -45,7 +53,7 @@ class HotPath:
             self.traj_off = up(toff)
             self.ema_traj = torch.zeros((int(toff[-1]), 3), dtype=torch.float64, device=dev)
         ws = lambda which, a, b: torch.empty(api.workspace_bytes(which, a, b), dtype=torch.uint8, device=dev)
-        self.ws_char = ws(_lib.WS_CHARACTERIZE, 0 if self.text is None else self.text.numel(), c.n_traces * c.n_req)
+        self.ws_char = ws(_lib.WS_CHARACTERIZE, 0 if self.text is None else self.text.numel(), self.n_text_prompts)
         self.ws_sim = ws(_lib.WS_SIMULATE, n, self.n_inst)
         G = self.n_groups
         # histograms, and for the fused call the staging area behind them (5 bytes per simulated request: 32-bit keys + segment codes)
@@ -76,7 +84,8 @@ class HotPath:
         mark = (lambda: ev.append(self._rec())) if timed_events else (lambda: None)
         mark()
         if self.text is not None:
-            api.characterize(self.text, self.offsets, self.words, self.tokens, self.ws_char)
+            k = self.n_text_prompts       # the prompts that exist as text (all of them, or the materialised sample)
+            api.characterize(self.text, self.offsets, self.words[:k], self.tokens[:k], self.ws_char)
         mark()
         api.simulate(self.trace_off, self.arrival, self.tier, self.words, self.tokens, self.out_len, self.c.server, self.inst,
                      self.out_off, self.n_total, self.start, self.done, self.ema_final, self.traj_off, self.ema_traj, self.ws_sim)
@@ -105,25 +114,36 @@ class HotPath:
 class HostPipeline:
     """End-to-end path for HOST inputs and outputs: `depth` HotPath slots and three CUDA streams, so the host-to-device
     copy of step i+1, the kernels of step i and the device-to-host copy of step i-1 overlap (PCIe is the slowest of the
-    three on configs[1]). Orchestration only: every computation still happens inside libdriftsched.so."""
+    three on configs[1]). Orchestration only: every computation still happens inside libdriftsched.so.
 
-    IN_FIELDS = ("text", "offsets", "arrival", "tier", "out_len")
+    result="ticks": every step returns start/done ticks of every simulated request, the EMA factors and the percentile
+    tables; result="stats": only the factors, percentile tables and segment counts come back (the per-request ticks stay in
+    device memory: 52 GB on configs[3]). share_outputs: the slots have private inputs but share one set of output
+    buffers and workspaces (for workloads whose outputs do not fit twice); a step then starts only after the previous
+    step's results have left the device."""
 
-    def __init__(self, wl_obj, device="cuda:0", depth=2):
+    def __init__(self, wl_obj, device="cuda:0", depth=2, share_outputs=False, result="ticks"):
         self.dev = torch.device(device)
-        self.slots = [HotPath(wl_obj, device) for _ in range(depth)]
+        first = HotPath(wl_obj, device)
+        self.slots = [first] + [HotPath(wl_obj, device, share=first if share_outputs else None) for _ in range(depth - 1)]
+        self.share = share_outputs
         self.s_in, self.s_run, self.s_out = (torch.cuda.Stream(self.dev) for _ in range(3))
         mk = lambda: [torch.cuda.Event() for _ in range(depth)]
         self.ev_in, self.ev_run, self.ev_out = mk(), mk(), mk()
-        self.out_dev = [[hp.start, hp.done, hp.ema_final] + list(hp.stats.values()) for hp in self.slots]
+        ticks = (lambda hp: [hp.start, hp.done]) if result == "ticks" else (lambda hp: [])
+        self.out_dev = [ticks(hp) + [hp.ema_final, hp.e2e_stats, hp.qd_stats, hp.counts4] for hp in self.slots]
         self.out_host = [[torch.empty(t.shape, dtype=t.dtype).pin_memory() for t in outs] for outs in self.out_dev]
         self.h2d_bytes = 0
         self.d2h_bytes = sum(t.numel() * t.element_size() for t in self.out_host[0])
+        # per-step inputs: the text and the trace records; (words, tokens) too when the text does not cover every prompt
+        self.in_fields = ("text", "offsets", "arrival", "tier", "out_len")
+        if first.text is None or first.n_text_prompts < first.words.numel():
+            self.in_fields += ("words", "tokens")
 
     def pin_inputs(self, wl_obj):
         """Pinned host copies of the per-step inputs (what a caller would hand over)."""
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-        h = {f: pin(getattr(wl_obj, f)) for f in self.IN_FIELDS if getattr(wl_obj, f) is not None}
+        h = {f: pin(getattr(wl_obj, f)) for f in self.in_fields if getattr(wl_obj, f) is not None}
         self.h2d_bytes = sum(t.numel() * t.element_size() for t in h.values())
         return h
 
@@ -142,6 +162,8 @@ class HostPipeline:
             if i >= depth:
                 self.s_in.wait_event(self.ev_run[k])      # the kernels that last read this slot's inputs are done
                 self.s_run.wait_event(self.ev_out[k])     # and its outputs have left the device
+            if self.share and i >= 1:
+                self.s_run.wait_event(self.ev_out[(i - 1) % depth])   # shared outputs: the previous step's results are out
             with torch.cuda.stream(self.s_in):
                 for f, h in host_inputs.items():
                     getattr(hp, f).copy_(h, non_blocking=True)

@@ -232,7 +232,7 @@ def make_instances(n_traces, combos):
 
 
 def _trace_workload(name, seed, n_traces, n_req, sv, combos, characterize, *, rho=None, mean_ticks=None,
-                    out_dist=0, drift=False, materialise=True):
+                    out_dist=0, drift=False, materialise=True, text_traces=0):
     tier, out_len, expo = make_requests(seed, n_traces, n_req, out_dist)
     post = None
     if drift:
@@ -246,6 +246,14 @@ def _trace_workload(name, seed, n_traces, n_req, sv, combos, characterize, *, rh
         tokens = np.asarray(tokens, np.int32)
     else:
         words, tokens = make_counts(seed, n_traces, n_req, post)
+        if text_traces > 0:
+            # text-free configuration with a materialised sample: the prompts of the first text_traces traces exist as text
+            # and their (W, P) come from `characterize`; the remaining traces keep the numeric draw of the same word law
+            nt = min(text_traces, n_traces)
+            text, offsets = make_text(seed, nt, n_req, None if post is None else post[:nt * n_req])
+            w, t = characterize(text, offsets)
+            words[:nt * n_req] = np.asarray(w, np.int32)
+            tokens[:nt * n_req] = np.asarray(t, np.int32)
     if mean_ticks is None:
         mean_ticks = np.array([
             mean_interarrival_ticks(rho, tokens[t * n_req:(t + 1) * n_req], out_len[t * n_req:(t + 1) * n_req], sv)
@@ -306,12 +314,14 @@ def config1(characterize, n_traces=1024, n_req=2000, seed=1):
     return _trace_workload("cfg1", seed, n_traces, n_req, sv, combos, characterize, rho=0.85)
 
 
-def config3(characterize=None, n_traces=16384, n_req=10000, seed=3, materialise=False):
-    """configs[3]: heavy contention, Pareto outputs, batch 128, KV 65536, aging 250 ms, 4 alphas."""
+def config3(characterize=None, n_traces=16384, n_req=10000, seed=3, materialise=False, text_traces=0):
+    """configs[3]: heavy contention, Pareto outputs, batch 128, KV 65536, aging 250 ms, 4 alphas. text_traces > 0: the
+    prompts of the first text_traces traces are materialised as text (Workload.text / .offsets cover those prompts only)
+    and characterised by `characterize`; SURVEY.md §8(d) draws the other traces' (W, P) numerically."""
     sv = Server(max_batch=128, kv_budget=65536, aging_step=250_000)
     combos = [(p, SPLIT, a) for p in ALL_POLICIES for a in (0.05, 0.1, 0.2, 0.5)]
     return _trace_workload("cfg3", seed, n_traces, n_req, sv, combos, characterize, rho=0.95, out_dist=1,
-                           materialise=materialise)
+                           materialise=materialise, text_traces=text_traces)
 
 
 def config4(characterize=None, n_traces=4096, n_req=50000, seed=4, materialise=False, traj_every=1000):

@@ -140,6 +140,45 @@ def test_bad_arguments(G):
     assert ds.device_status() & 8
 
 
+def test_workspace_and_output_ranges_are_validated(G):
+    # the whole documented workspace is required (header + permutation + SJF heap slots): one byte short => DS_ENOMEM, no launch
+    import torch
+    import paper_2606_02982_b200 as ds
+    from paper_2606_02982_b200 import _lib
+    sv = wl.Server(max_batch=4, kv_budget=0)
+    c = wl._trace_workload("t", 41, 1, 2000, sv, [(wl.SJF, wl.SPLIT, 0.1)], None, rho=3.0, materialise=False)   # overload: queue > 256
+    d = G.upload(c)
+    n_total = int(c.out_off[-1])
+    need = ds.workspace_bytes(_lib.WS_SIMULATE, n_total, c.n_inst)
+    args = (d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"], c.server, d["inst"], d["out_off"], n_total)
+    with pytest.raises(ds.DsError) as e:
+        ds.simulate(*args, workspace=torch.empty(need - 1, dtype=torch.uint8, device=G.DEV))
+    assert e.value.code == _lib.DS_ENOMEM
+    st, dn, ema = ds.simulate(*args, workspace=torch.empty(need, dtype=torch.uint8, device=G.DEV))
+    assert ds.device_status() == 0
+    o = _oracle(c)
+    assert np.array_equal(st.cpu().numpy(), o[0]) and np.array_equal(dn.cpu().numpy(), o[1])
+    # an instance whose output range leaves [0, n_total) is skipped and reported, nothing is written outside the arrays
+    canary = torch.full((n_total + 64,), -7, dtype=torch.int64, device=G.DEV)
+    st2, dn2, _ = ds.simulate(d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"], c.server, d["inst"],
+                              d["out_off"], n_total - 1, start=canary[:n_total - 1], done=torch.empty(n_total, dtype=torch.int64, device=G.DEV)[:n_total - 1])
+    assert ds.device_status() & 16
+    assert bool((canary == -7).all())
+
+
+def test_decreasing_arrivals_are_reported(G):
+    # the monotone-arrival contract is checked on every pair of neighbouring requests, also across the 32-request windows
+    import paper_2606_02982_b200 as ds
+    sv = wl.Server(max_batch=4, kv_budget=0)
+    for bad_at in (5, 32, 64, 96):            # inside a window, and on lane 0 of a window (pair (31, 32) etc.)
+        c = wl._trace_workload("t", 43, 1, 200, sv, [(p, wl.EXACT, 0.0) for p in wl.ALL_POLICIES], None, rho=0.8, materialise=False)
+        c.arrival[bad_at] = c.arrival[bad_at - 1] - 1
+        d = G.upload(c)
+        ds.simulate(d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"], c.server, d["inst"], d["out_off"],
+                    int(c.out_off[-1]))
+        assert ds.device_status() & 2, bad_at
+
+
 def test_large_costs_take_the_64bit_path(G):
     # cost constants near 2^31 and one huge out_len: the per-trace bound fails, so the kernel must use its 64-bit state
     sv = wl.Server(max_batch=6, kv_budget=9000, aging_step=3_000_000_000, c_base=2_000_000_000, c_batch=150_000_000,

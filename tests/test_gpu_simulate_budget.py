@@ -148,7 +148,7 @@ def test_closed_loop(G, n_clients, think, max_batch, kv):
     cat, out_len = wl.assign_categories(51 + n_clients, c.out_len)
     arrival = c.arrival.copy().reshape(3, 700)
     arrival[:, n_clients:] = 0                       # ignored by the closed loop; must not matter
-    arrival[:, :n_clients] = np.minimum(arrival[:, :n_clients], 50_000)
+    arrival[:, :n_clients] = np.minimum(arrival[:, :n_clients], 2_000)   # staggered starts, all before the first release (>= 2150 ticks)
     arrival = arrival.reshape(-1)
     bp = wl.Budget(s_tenant=(1.25, 1.0, 0.8), f_slope=0.001, f_max=1.3)
     tr = (c.trace_off, arrival, c.tier, c.words, c.tokens, out_len)
@@ -188,6 +188,44 @@ def test_closed_loop_hand_trace_and_contract(G):
     assert arr.tolist() == [0, 0, 0, 2168] and st.tolist() == [6504, 4324, 0, 2168] and dn.tolist() == [8708, 6504, 2168, 4324]
     with pytest.raises(ds.DsError):
         ds.api.simulate_budget(*targs, cat, bp, c.server, d["inst"], d["out_off"], 4, n_clients=3, think_ticks=-5)
+
+
+def test_closed_loop_staggered_client_starts(G):
+    # clients that do not start together: fine while the last start is not after the first release (header contract) ...
+    import paper_2606_02982_b200 as ds
+    sv = wl.Server(max_batch=8, kv_budget=3000, aging_step=40_000)
+    combos = [(p, wl.BUDGET_SPLIT, 0.1) for p in wl.ALL_POLICIES + [wl.AGING_UNCLAMPED]]
+    c = wl._trace_workload("t", 71, 2, 500, sv, combos, oracle.characterize, rho=1.0)
+    cat, out_len = wl.assign_categories(71, c.out_len)
+    n_clients = 40
+    arrival = np.zeros((2, 500), np.int64)
+    arrival[:, :n_clients] = np.arange(n_clients) * 37             # staggered: last start 1443 ticks, first completion >= 2150
+    arrival = arrival.reshape(-1)
+    tr = (c.trace_off, arrival, c.tier, c.words, c.tokens, out_len)
+    ost, odn, oema, oarr = oracle.simulate_budget(*tr, cat, wl.Budget(), sv, c.instances, out_off=c.out_off, n_clients=n_clients, think_ticks=5)
+    assert (np.diff(oarr.reshape(-1, 500), axis=1) >= 0).all()     # the contract holds on this input
+    d = G.upload(c)
+    d["out_len"] = torch.from_numpy(out_len).to(G.DEV)
+    d["arrival"] = torch.from_numpy(arrival).to(G.DEV)
+    targs = (d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"])
+    n_total = int(c.out_off[-1])
+    dcat = torch.from_numpy(cat).to(G.DEV)
+    st, dn, ema, arr = ds.simulate_closed(*targs, dcat, wl.Budget(), sv, n_clients, 5, 0, d["inst"], d["out_off"], n_total)
+    assert ds.device_status() == 0
+    assert np.array_equal(arr.cpu().numpy(), oarr) and np.array_equal(st.cpu().numpy(), ost) and np.array_equal(dn.cpu().numpy(), odn)
+    assert np.array_equal(ema.cpu().numpy().view(np.uint64), oema.view(np.uint64))
+    # ... and reported when violated: a client that starts long after the first release makes the arrivals non-monotone
+    for pos in (n_clients - 1, 31):                                # the last client; a client whose successor opens the next window
+        bad = arrival.copy().reshape(2, 500)
+        bad[:, pos:n_clients] = 10_000_000
+        d["arrival"] = torch.from_numpy(bad.reshape(-1)).to(G.DEV)
+        targs = (d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"])
+        for pol in (wl.FIFO, wl.AGING_UNCLAMPED):
+            inst, _ = wl.make_instances(2, [(pol, wl.BUDGET_SPLIT, 0.1)])
+            from paper_2606_02982_b200.api import instances_to_device
+            off = torch.from_numpy(np.arange(3, dtype=np.int64) * 500).to(G.DEV)
+            ds.simulate_closed(*targs, dcat, wl.Budget(), sv, n_clients, 5, 0, instances_to_device(inst, G.DEV), off, 1000)
+            assert ds.device_status() & 2, (pos, pol)
 
 
 @pytest.mark.parametrize("rho,n_clients,W,max_batch", [(0.3, 600, 10_000, 4), (0.6, 600, 10_000, 32), (0.3, 600, 3_000, 1),
@@ -256,14 +294,34 @@ def test_paper_setup_closed_loop_tables(G):
     assert ds.device_status() == 0
     assert np.array_equal(arr.cpu().numpy(), oarr) and np.array_equal(st.cpu().numpy(), ost) and np.array_equal(dn.cpu().numpy(), odn)
     assert np.array_equal(ema.cpu().numpy().view(np.uint64), oema.view(np.uint64))
-    seg_h = np.repeat(c.group, c.n_req).astype(np.int32)                # one segment per (policy, mode), runs pooled
+    # reporting, all inside the library, with the closed loop's own arrivals (arrival_override = arrival_out):
+    # (1) fused percentiles: Tables VI-VIII (P50/P95/P99 of end-to-end latency and queue wait per (policy, mode) x tier and overall)
     pct = (50, 95, 99)
-    want, wcnt = oracle.tail_stats(odn - oarr, seg_h, c.n_groups, pct)
-    got, gcnt = ds.tail_stats(dn - arr, torch.from_numpy(seg_h).to(G.DEV), c.n_groups, pct)
-    assert np.array_equal(got.cpu().numpy(), want) and np.array_equal(gcnt.cpu().numpy(), wcnt)
-    osum = oracle.estimation_error(*tr, c.instances, c.out_off, oest, ost, c.group, c.n_groups)
-    gsum = ds.api.estimation_error(*targs, d["inst"], d["out_off"], n_total, est, st, d["group"], c.n_groups)
-    assert np.array_equal(gsum.cpu().numpy()[:, :8], osum[:, :8])       # (queue-wait sums use tr.arrival: not the closed-loop ones)
+    oe2e, oqd, oseg_t, oseg_a = oracle.latencies(*tr, c.instances, c.out_off, ost, odn, c.group, arrival_override=oarr)
+    ge, gq, gc = ds.latency_stats(*targs, d["inst"], d["out_off"], st, dn, d["group"], c.n_groups, pct=pct, arrival_override=arr)
+    G3 = 3 * c.n_groups
+    for vals, got_stats in ((oe2e, ge), (oqd, gq)):
+        wt, ct = oracle.tail_stats(vals, oseg_t, G3, pct)
+        wa, ca = oracle.tail_stats(vals, oseg_a, c.n_groups, pct)
+        assert np.array_equal(got_stats.cpu().numpy(), np.concatenate([wt, wa]))
+    assert np.array_equal(gc.cpu().numpy(), np.concatenate([ct, ca]))
+    want = wa_e2e = oracle.tail_stats(oe2e, oseg_a, c.n_groups, pct)[0]
+    # (2) the unfused pair gives the same latencies and percentiles
+    e2e, qd, seg_t, seg_a = ds.latencies(*targs, d["inst"], d["out_off"], n_total, st, dn, d["group"], arrival_override=arr)
+    assert np.array_equal(e2e.cpu().numpy(), oe2e) and np.array_equal(qd.cpu().numpy(), oqd)
+    got, gcnt = ds.tail_stats(e2e, seg_a, c.n_groups, pct)
+    assert np.array_equal(got.cpu().numpy(), want)
+    # (3) Table IX / Tables IV, X: all eleven sums, the queue wait by job class now being the closed loop's
+    osum = oracle.estimation_error(*tr, c.instances, c.out_off, oest, ost, c.group, c.n_groups, arrival_override=oarr)
+    gsum = ds.estimation_error(*targs, d["inst"], d["out_off"], n_total, est, st, d["group"], c.n_groups, arrival_override=arr)
+    assert np.array_equal(gsum.cpu().numpy(), osum)
+    assert (osum[:, 8:].sum(axis=1) > 0).all()
+    # (4) Fig. 8: per-tenant queue depth over time of the closed loop
+    t_end = int(odn.max())
+    odepth = oracle.queue_depth(*tr, c.instances, c.out_off, ost, 0, t_end // 300 + 1, 300, arrival_override=oarr)
+    gdepth = ds.queue_depth(*targs, d["inst"], d["out_off"], st, 0, t_end // 300 + 1, 300, arrival_override=arr)
+    assert np.array_equal(gdepth.cpu().numpy(), odepth)
+    assert odepth.sum(axis=2).max() <= 50                               # never more than the 50 clients' requests queued
     # the paper's headline on its own setup: SJF lowers the median end-to-end latency against FIFO
     g = {c.extra["combos"][k]: k for k in range(c.n_groups)}
     fifo, sjf = g[(wl.FIFO, wl.BUDGET_SPLIT, 0.1)], g[(wl.SJF, wl.BUDGET_SPLIT, 0.1)]
