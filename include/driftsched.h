@@ -79,6 +79,7 @@ typedef struct {              /* SoA request records, traces concatenated; HOST 
   const int32_t* words;        /* split() count, >= 0 */
   const int32_t* tokens;       /* pseudo-token count = true prompt length, >= 0 */
   const int32_t* out_len;      /* decode length, >= 1 */
+  int64_t n_requests;          /* HOST copy of trace_off[n_traces]: requests over all traces = length of the five arrays above */
 } ds_traces;
 
 typedef struct {              /* continuous-batching server model, BASELINE.json:configs[0] */
@@ -123,12 +124,13 @@ typedef struct {
  * traj_off    [n_inst+1] nullable device; instance i owns trajectory samples [traj_off[i], traj_off[i+1]),
  *                                 floor(n_req_i / traj_every) of them
  * ema_traj    [traj_off[n_inst]*3] nullable device fp64
- * workspace: ds_workspace_bytes(DS_WS_SIMULATE, n_total, n_inst) bytes are REQUIRED (DS_ENOMEM otherwise): header,
- *   instance permutation and one 8-byte SJF heap slot per simulated request (touched only by SJF instances with more
- *   than 256 requests queued, but always validated).
+ * workspace: ds_workspace_bytes(DS_WS_SIMULATE, n_total, n_inst) + ds_workspace_bytes(DS_WS_SIMULATE_TRACES, tr->n_requests, 0)
+ *   bytes are REQUIRED (DS_ENOMEM otherwise): header, instance permutation, one 8-byte SJF heap slot per simulated request
+ *   (touched only by SJF instances with more than 256 requests queued, but always validated), then one packed 16-byte
+ *   record per trace request (tokens/words ratio, tokens, out_len; written by a pre-pass of every call).
  * Contract checked on the device (DS_DEV_BAD_TRACE, outputs of that instance unspecified): tier <= 2, words/tokens >= 0,
  *   out_len >= 1, arrival_tick >= 0 and non-decreasing over every pair of neighbouring requests of a trace.
- * Launches: 1 memset (work counter) + 2 kernels (policy-major ordering of the instances, simulation). */
+ * Launches: 1 memset (work counter) + 3 kernels (policy-major ordering of the instances, request records, simulation). */
 int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
                 const int64_t* out_off, int64_t n_total, int64_t* start_tick, int64_t* done_tick, double* ema_final,
                 const int64_t* traj_off, double* ema_traj, void* workspace, size_t workspace_bytes, void* stream);
@@ -254,6 +256,7 @@ int ds_latency_stats(const ds_traces* tr, const ds_instance* inst, int64_t n_ins
 #define DS_WS_SIMULATE 1
 #define DS_WS_TAIL_STATS 2
 #define DS_WS_LATENCY_STAGE 3 /* n = simulated requests over all instances; m unused: optional staging area of ds_latency_stats */
+#define DS_WS_SIMULATE_TRACES 4 /* n = tr->n_requests; m unused: second, mandatory part of the ds_simulate* workspace */
 /* Workspace size in bytes for call `which` with the two size arguments named at that call. Never 0. */
 size_t ds_workspace_bytes(int which, int64_t n, int64_t m);
 

@@ -10,6 +10,7 @@ LIB_PATH = os.path.join(_HERE, "libdriftsched.so")
 DS_OK, DS_EINVAL, DS_ECUDA, DS_ENOMEM = 0, -1, -2, -3
 WS_CHARACTERIZE, WS_SIMULATE, WS_TAIL_STATS = 0, 1, 2
 WS_LATENCY_STAGE = 3
+WS_SIMULATE_TRACES = 4
 
 EXPORTS = ["ds_characterize", "ds_simulate", "ds_simulate_est", "ds_simulate_budget", "ds_simulate_closed", "ds_estimation_error", "ds_queue_depth", "ds_latencies", "ds_tail_stats",
            "ds_latency_stats", "ds_workspace_bytes", "ds_device_status",
@@ -18,7 +19,7 @@ EXPORTS = ["ds_characterize", "ds_simulate", "ds_simulate_est", "ds_simulate_bud
 
 class DsTraces(C.Structure):
     _fields_ = [("n_traces", C.c_int64), ("trace_off", C.c_void_p), ("arrival_tick", C.c_void_p), ("tier", C.c_void_p),
-                ("words", C.c_void_p), ("tokens", C.c_void_p), ("out_len", C.c_void_p)]
+                ("words", C.c_void_p), ("tokens", C.c_void_p), ("out_len", C.c_void_p), ("n_requests", C.c_int64)]
 
 
 class DsServer(C.Structure):

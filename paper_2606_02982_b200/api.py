@@ -34,6 +34,11 @@ def _workspace(which, n, m, device):
     return torch.empty(workspace_bytes(which, n, m), dtype=torch.uint8, device=device)
 
 
+def simulate_workspace_bytes(n_total, n_inst, n_requests):
+    """Both mandatory parts of the ds_simulate* workspace: per simulated request / instance, and per trace request."""
+    return workspace_bytes(_lib.WS_SIMULATE, n_total, n_inst) + workspace_bytes(_lib.WS_SIMULATE_TRACES, n_requests, 0)
+
+
 def launch_count():
     return int(lib().ds_launch_count())
 
@@ -66,7 +71,7 @@ def _traces(trace_off, arrival, tier, words, tokens, out_len):
     assert trace_off.dtype == torch.int64 and arrival.dtype == torch.int64 and tier.dtype == torch.uint8
     assert words.dtype == torch.int32 and tokens.dtype == torch.int32 and out_len.dtype == torch.int32
     return DsTraces(trace_off.numel() - 1, trace_off.data_ptr(), arrival.data_ptr(), tier.data_ptr(), words.data_ptr(),
-                    tokens.data_ptr(), out_len.data_ptr())
+                    tokens.data_ptr(), out_len.data_ptr(), arrival.numel())
 
 
 def _server(sv):
@@ -96,7 +101,7 @@ def simulate(trace_off, arrival, tier, words, tokens, out_len, server, inst, out
     if ema_final is None:
         ema_final = torch.empty((n_inst, 3), dtype=torch.float64, device=dev)
     if workspace is None:
-        workspace = _workspace(_lib.WS_SIMULATE, n_total, n_inst, dev)
+        workspace = torch.empty(simulate_workspace_bytes(n_total, n_inst, arrival.numel()), dtype=torch.uint8, device=dev)
     if est_out is not None:                     # ds_simulate_est: same call, also writes the frozen estimates
         _need_cuda(est_out)
         assert est_out.dtype == torch.int64 and est_out.numel() >= n_total
@@ -235,7 +240,7 @@ def simulate_budget(trace_off, arrival, tier, words, tokens, out_len, category, 
     if ema_final is None:
         ema_final = torch.empty((n_inst, 4), dtype=torch.float64, device=dev)
     if workspace is None:
-        workspace = _workspace(_lib.WS_SIMULATE, n_total, n_inst, dev)
+        workspace = torch.empty(simulate_workspace_bytes(n_total, n_inst, arrival.numel()), dtype=torch.uint8, device=dev)
     if n_clients > 0:   # ds_simulate_closed: closed-loop arrivals, returns arrival_out as a 4th element
         if arrival_out is None:
             arrival_out = torch.empty(n_total, dtype=torch.int64, device=dev)

@@ -60,6 +60,7 @@ size_t ws_characterize(int64_t n_bytes, int64_t n_prompts);
 size_t ws_simulate(int64_t total_requests, int64_t n_inst);
 size_t ws_tail_stats(int64_t n_segments, int64_t n_pct);
 size_t ws_latency_stage(int64_t n_total);
+size_t ws_simulate_traces(int64_t n_requests);
 
 }  // namespace ds
 
@@ -74,6 +75,7 @@ size_t ds_workspace_bytes(int which, int64_t n, int64_t m) {
     case DS_WS_SIMULATE: b = ds::ws_simulate(n, m); break;
     case DS_WS_TAIL_STATS: b = ds::ws_tail_stats(n, m); break;
     case DS_WS_LATENCY_STAGE: b = ds::ws_latency_stage(n); break;
+    case DS_WS_SIMULATE_TRACES: b = ds::ws_simulate_traces(n); break;
     default: b = 0;
   }
   return b < 256 ? 256 : b;

@@ -9,8 +9,15 @@
 // body is compiled once per (slots, policy) so that each policy's queue logic is straight-line code:
 //  - warp-uniform scalars: clock `now`, cursor `next`, next arrival tick `an`, batch size b, kv_used, B[3] (held by
 //    lanes 0..2);
-//  - running set: kSlots slots per lane (max_batch <= 32*kSlots), each {request index, finishing iteration};
-//    completions are found with one REDUX min over (fin - iter);
+//  - running set: 32*kSlots slots {request index, finishing iteration} in shared memory (max_batch <= 32*kSlots) with a
+//    free-slot stack beside them: an admission is one pop + two stores by uniform address (placing a request into one
+//    lane's register slots cost 35 instructions of divergent, predicated code per request). At a completion boundary
+//    lane L loads slots [kSlots*L, kSlots*(L+1)) into registers once (LDS.128), the completions of that boundary are
+//    retired from those registers in ascending request index (one REDUX min each) and the distance to the next
+//    completion is one more REDUX min over (fin - iter);
+//  - per-request records: pack_kernel first writes {m = tokens/words (the feedback ratio of Eq. 6, one fp64 division per
+//    TRACE request instead of one per simulated request), tokens, out_len} as one 16-byte record, so a completion or an
+//    admission is one LDG.128 instead of two to four 4-byte loads with their 64-bit address arithmetic;
 //  - between events the batch is constant, so j iterations cost exactly j*dt + c_ctx*b*j(j-1)/2 ticks (§8(c) step 6
 //    with a constant running set): the kernel jumps to the next event (completion, or arrival when an arrival can
 //    matter) with that closed form; a float estimate gives a provably safe lower bound on j, exact integer arithmetic
@@ -40,6 +47,10 @@ constexpr int kHeapSmem = 256;  // heap entries cached in shared memory per warp
 constexpr long long kInf = 0x7fffffffffffffffLL;
 constexpr unsigned kFull = 0xffffffffu;
 
+// per trace request, written by pack_kernel: m = tokens/words as fp64 (correctly rounded division, the B_measured of Eq. 6
+// under reading A3; -1.0 when words <= 0: no feedback from that request), P = tokens, O = out_len
+struct __align__(16) Rec { double m; int P; int O; };
+
 struct Params {
   const int64_t* trace_off; const int64_t* arrival; const uint8_t* tier; const int32_t* words; const int32_t* tokens;
   const int32_t* out_len; int64_t n_traces;
@@ -51,6 +62,8 @@ struct Params {
   int32_t n_clients; int64_t think; int64_t* arrival_out;   // closed-loop arrivals (ds_simulate_closed), n_clients = 0: open loop
   int64_t batch_wait;                                        // ds_simulate_closed: dispatch gate of an idle server (0 = none)
   unsigned long long* heap_ws; unsigned int* counter; unsigned int* status; const unsigned int* perm;
+  const struct Rec* rec;                                     // [n_requests] packed per-request records (pack_kernel)
+  int32_t use_kv, want_est, want_traj;                       // 32-bit copies of kv_budget > 0, est_out != NULL, trajectory sampling on
   int64_t n_total;                                           // out_off[n_inst] as stated by the caller: size of every per-request output and of the heap region
   unsigned n_sms;
 };
@@ -66,6 +79,15 @@ __device__ __forceinline__ unsigned long long warp_min_u64(unsigned long long v)
 }
 __device__ __forceinline__ long long shfl_i64(long long v, int src) { return __shfl_sync(kFull, v, src); }
 __device__ __forceinline__ double shfl_f64(double v, int src) { return __shfl_sync(kFull, v, src); }
+
+// ---- running set: per warp, 32*kSlots slots in shared memory; lane L scans slots [kSlots*L, kSlots*(L+1)) ----
+constexpr int kFreeIdx = 0x7fffffff;          // idx of a free slot (also "no request" in the min reductions)
+template <int kSlots>
+struct __align__(16) Slots {
+  int idx[32 * kSlots];                       // request index, kFreeIdx = free
+  unsigned fin[32 * kSlots];                  // iteration at whose boundary the request completes
+  unsigned short stack[32 * kSlots];          // free slot numbers, [0, nfree) valid
+};
 
 // ---- SJF heap: implicit 32-ary min-heap, node i has children 32i+1 .. 32i+32 ----
 struct Heap {
@@ -124,7 +146,7 @@ struct TierCursor {
 // the reduced per-tier one (lanes 0..2); a separate instantiation so that the benchmarked path is not touched.
 template <int kSlots, int kPolicy, bool kSmall, bool kBudget>
 __device__ __forceinline__ void run_instance(const Params& p, const unsigned inst_id, const int trace, const bool split, const double alpha,
-                                          unsigned long long* heap_sm, const int lane) {
+                                          unsigned long long* heap_sm, Slots<kSlots>& sl, const int lane) {
   constexpr bool kAging = kPolicy == DS_AGING || kPolicy == DS_AGING_UNCLAMPED;   // both read the heads' arrival ticks
   constexpr bool kCursor = kPolicy == DS_PRIORITY || kPolicy == DS_WEIGHTED || kAging;
   const long long lo = p.trace_off[trace];
@@ -147,15 +169,16 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   int64_t* __restrict__ st = p.start_tick + oo;
   int64_t* dn = p.done_tick + oo;
   const int32_t* __restrict__ BASE = split ? W : P;
-  const bool use_kv = p.kv_budget > 0;
-  int64_t* est_o = p.est_out ? p.est_out + oo : nullptr;
+  const Rec* __restrict__ rec = p.rec + lo;
+  const bool use_kv = p.use_kv != 0;
+  int64_t* est_o = p.want_est ? p.est_out + oo : nullptr;
   const bool need_est = use_kv || kPolicy == DS_SJF || est_o != nullptr;
   // EXACT estimator: m = P/P = 1.0, and (1-a)*1 + a*1 rounds to exactly 1.0 for every a in [0,1] (DESIGN.md §4 A4),
   // so B stays 1.0 and est = base: no fp64 work at all on that path.
   const bool ema_on = (kBudget || split) && alpha > 0.0;
   constexpr int kFac = kBudget ? 4 : 3;           // feedback factors per instance
   const uint8_t* __restrict__ cat = kBudget ? p.category + lo : nullptr;
-  double* traj = (p.ema_traj && p.traj_off && p.traj_every > 0) ? p.ema_traj + kFac * p.traj_off[inst_id] : nullptr;
+  double* traj = p.want_traj ? p.ema_traj + kFac * p.traj_off[inst_id] : nullptr;
   const int max_batch = p.max_batch;
 
   // ---- state (warp-uniform unless noted) ----
@@ -168,9 +191,11 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   bool blocked = false;
   long long collect = -1;                // batch-wait: tick at which the idle dispatcher started collecting (-1: not collecting)
   double Bl = 1.0;                       // lane t < 3 holds B[t]
-  int s_idx[kSlots]; unsigned s_fin[kSlots];   // per lane: running requests
+  // running set: all slots free, the free stack holds every slot number
+  int nfree = 32 * kSlots;
 #pragma unroll
-  for (int s = 0; s < kSlots; ++s) { s_idx[s] = -1; s_fin[s] = 0; }
+  for (int s = 0; s < kSlots; ++s) { sl.idx[s * 32 + lane] = kFreeIdx; sl.fin[s * 32 + lane] = 0u; sl.stack[s * 32 + lane] = (unsigned short)(s * 32 + lane); }
+  __syncwarp();
   Heap heap; heap.sm = heap_sm; heap.gm = p.heap_ws + oo; heap.size = 0;
   TierCursor tc[3];
   const int wtot = p.w0 + p.w1 + p.w2;
@@ -288,17 +313,52 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
     an = next < n ? shfl_i64(w_arr, next - wb) : kInf;
   };
 
-  // 2. RETIRE: completions at `now`, ascending request index (R-ORD); then the distance to the next completion
+  // 2. RETIRE: completions at `now`, ascending request index (R-ORD); then the distance to the next completion.
+  // The lane's slots are loaded into registers once; every completion of this boundary is found and cleared there.
+  const double t1 = __dsub_rn(1.0, alpha);                    // Eq. 5: (1 - alpha), the same rounding every time
   auto retire = [&]() {
-    for (;;) {
-      int lm = 0x7fffffff;
+    __syncwarp();                                             // the slot stores of earlier admissions are visible
+    int ri[kSlots]; unsigned rf[kSlots];
+    if constexpr (kSlots % 4 == 0) {
 #pragma unroll
-      for (int s = 0; s < kSlots; ++s) if (s_idx[s] >= 0 && s_fin[s] == iter) lm = min(lm, s_idx[s]);
-      const int r = __reduce_min_sync(kFull, lm);             // called with dist == 0: at least one request completes now
-      if (r == 0x7fffffff) { dist = 0xffffffffu; break; }     // (defensive: cannot happen; never spin or index with it)
+      for (int q = 0; q < kSlots / 4; ++q) {
+        const int4 vi = *reinterpret_cast<const int4*>(&sl.idx[lane * kSlots + 4 * q]);
+        const uint4 vf = *reinterpret_cast<const uint4*>(&sl.fin[lane * kSlots + 4 * q]);
+        ri[4 * q] = vi.x; ri[4 * q + 1] = vi.y; ri[4 * q + 2] = vi.z; ri[4 * q + 3] = vi.w;
+        rf[4 * q] = vf.x; rf[4 * q + 1] = vf.y; rf[4 * q + 2] = vf.z; rf[4 * q + 3] = vf.w;
+      }
+    } else if constexpr (kSlots == 2) {
+      const int2 vi = *reinterpret_cast<const int2*>(&sl.idx[lane * 2]);
+      const uint2 vf = *reinterpret_cast<const uint2*>(&sl.fin[lane * 2]);
+      ri[0] = vi.x; ri[1] = vi.y; rf[0] = vf.x; rf[1] = vf.y;
+    } else {
 #pragma unroll
-      for (int s = 0; s < kSlots; ++s) if (s_idx[s] == r) s_idx[s] = -1;
-      const int Pr = P[r], Or = max(O[r], 1);
+      for (int s = 0; s < kSlots; ++s) { ri[s] = sl.idx[lane * kSlots + s]; rf[s] = sl.fin[lane * kSlots + s]; }
+    }
+    // completions at this boundary (a free slot has idx = kFreeIdx, so its stale fin cannot match)
+    int lm = kFreeIdx, cnt = 0;
+#pragma unroll
+    for (int s = 0; s < kSlots; ++s) {
+      const bool hit = rf[s] == iter && ri[s] != kFreeIdx;
+      cnt += hit ? 1 : 0;
+      lm = hit ? min(lm, ri[s]) : lm;
+    }
+    int left = __reduce_add_sync(kFull, cnt);                 // called with dist == 0: at least one
+    bool freed_any = false;
+    while (left > 0) {
+      const int r = __reduce_min_sync(kFull, lm);
+      if (r == kFreeIdx) break;                               // (defensive: cannot happen; never index with it)
+      --left;
+      // owner: clear the slot in registers, push its number on the free stack; then the lane's next candidate
+      lm = kFreeIdx;
+#pragma unroll
+      for (int s = 0; s < kSlots; ++s) {
+        if (ri[s] == r) { ri[s] = kFreeIdx; sl.stack[nfree] = (unsigned short)(lane * kSlots + s); freed_any = true; }
+        if (left > 0) lm = (rf[s] == iter && ri[s] != kFreeIdx) ? min(lm, ri[s]) : lm;
+      }
+      ++nfree;
+      const Rec rr = rec[r];                                   // one 16-byte load: m, tokens, out_len
+      const int Pr = rr.P, Or = max(rr.O, 1);
       dn[r] = now;                                            // every lane, same address and value: one store, no branch
       kv_used -= (acc_t)Pr + (acc_t)Or;
       --b;
@@ -308,20 +368,17 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
           const double tb = cr == 0 ? p.bp.t_base[0] : cr == 1 ? p.bp.t_base[1] : cr == 2 ? p.bp.t_base[2] : p.bp.t_base[3];
           if (tb > 0.0) {
             const double m = __ddiv_rn((double)Or, tb);
-            const double t1 = __dsub_rn(1.0, alpha);
             const double t2 = __dmul_rn(t1, shfl_f64(Bl, cr));
             const double t3 = __dmul_rn(alpha, m);
             const double Bn = __dadd_rn(t2, t3);
             if (lane == cr) Bl = Bn;
           }
         }
-      } else if (ema_on) {                                    // Eq. 5-6 (A3): four separately rounded operations
-        const int br = W[r], tr = min((int)tier[r], 2);
-        if (br > 0) {
-          const double m = __ddiv_rn((double)Pr, (double)br);
-          const double t1 = __dsub_rn(1.0, alpha);
+      } else if (ema_on) {                                    // Eq. 5-6 (A3): four separately rounded operations; m = P/W came
+        const int tr = min((int)tier[r], 2);                  // rounded from pack_kernel (the same correctly rounded division)
+        if (rr.m >= 0.0) {                                    // words > 0
           const double t2 = __dmul_rn(t1, shfl_f64(Bl, tr));
-          const double t3 = __dmul_rn(alpha, m);
+          const double t3 = __dmul_rn(alpha, rr.m);
           const double Bn = __dadd_rn(t2, t3);
           if (lane == tr) Bl = Bn;
         }
@@ -338,14 +395,23 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
         __syncwarp();
       }
       if (traj && done % p.traj_every == 0 && lane < kFac) traj[kFac * (done / p.traj_every - 1) + lane] = Bl;
-      // distance to the next completion; 0 = another request completes at this same boundary (one reduction serves as
-      // both the loop test and the result)
-      unsigned d = 0xffffffffu;
-#pragma unroll
-      for (int s = 0; s < kSlots; ++s) if (s_idx[s] >= 0) d = min(d, s_fin[s] - iter);
-      dist = __reduce_min_sync(kFull, d);
-      if (dist != 0) break;
     }
+    // write the cleared slots back (lanes that freed nothing store what they loaded) and take the distance to the next completion
+    unsigned d = 0xffffffffu;
+#pragma unroll
+    for (int s = 0; s < kSlots; ++s) d = ri[s] != kFreeIdx ? min(d, rf[s] - iter) : d;
+    if constexpr (kSlots % 4 == 0) {
+#pragma unroll
+      for (int q = 0; q < kSlots / 4; ++q)
+        *reinterpret_cast<int4*>(&sl.idx[lane * kSlots + 4 * q]) = make_int4(ri[4 * q], ri[4 * q + 1], ri[4 * q + 2], ri[4 * q + 3]);
+    } else if constexpr (kSlots == 2) {
+      *reinterpret_cast<int2*>(&sl.idx[lane * 2]) = make_int2(ri[0], ri[1]);
+    } else {
+#pragma unroll
+      for (int s = 0; s < kSlots; ++s) sl.idx[lane * kSlots + s] = ri[s];
+    }
+    (void)freed_any;
+    dist = __reduce_min_sync(kFull, d);
     blocked = false;
     __syncwarp();
   };
@@ -422,18 +488,12 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
         for (int t = 0; t < 3; ++t) if (t == ct) advance_cursor(tc[t], t, false);
         if (kPolicy == DS_WEIGHTED) { cur = wpos + 1; if (cur >= wtot) cur = 0; }
       }
-      const int Pc = P[c];
-      const int Oc = max(O[c], 1);                             // (a bad out_len was reported when its window was loaded)
+      const Rec rc = rec[c];                                   // one 16-byte load: tokens, out_len (m unused here)
+      const int Pc = rc.P;
+      const int Oc = max(rc.O, 1);                             // (a bad out_len was reported when its window was loaded)
       st[c] = now;                                             // every lane, same address and value
-      bool has_free = false;                                   // first lane with a free slot takes the request
-#pragma unroll
-      for (int s = 0; s < kSlots; ++s) has_free |= s_idx[s] < 0;
-      const unsigned fm = __ballot_sync(kFull, has_free);
-      if (lane == __ffs(fm) - 1) {
-        bool placed = false;
-#pragma unroll
-        for (int s = 0; s < kSlots; ++s) if (!placed && s_idx[s] < 0) { s_idx[s] = c; s_fin[s] = iter + (unsigned)Oc; placed = true; }
-      }
+      const int slot = sl.stack[--nfree];                      // b < max_batch <= 32*kSlots: a free slot exists
+      sl.idx[slot] = c; sl.fin[slot] = iter + (unsigned)Oc;    // (uniform address and value)
       kv_used += (acc_t)Pc; prefill_new += (acc_t)Pc; ++b;
       dist = min(dist, (unsigned)Oc);
     }
@@ -515,6 +575,20 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   __syncwarp();
 }
 
+// One 16-byte record per TRACE request (shared by all instances of the trace): the feedback ratio m = tokens/words of Eq. 6
+// (reading A3) as a correctly rounded fp64 division - bit-identical to dividing at every completion - and the two lengths.
+__global__ void __launch_bounds__(256) pack_kernel(const int32_t* __restrict__ W, const int32_t* __restrict__ P, const int32_t* __restrict__ O,
+                                                   long long n, Rec* __restrict__ rec) {
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const int w = W[i], pt = P[i];
+    Rec r;
+    r.m = w > 0 ? __ddiv_rn((double)pt, (double)w) : -1.0;
+    r.P = pt; r.O = O[i];
+    rec[i] = r;
+  }
+}
+
 // true iff kv_used, the iteration cost (with prefill) and c_ctx*b of every reachable state of this trace stay below
 // 2^31 and every out_len is <= 65535: kv_used <= max_batch*(maxP+maxO) since a running request holds P+g <= P+O tokens.
 __device__ __forceinline__ bool trace_is_small(const Params& p, const int trace, const int lane) {
@@ -579,6 +653,7 @@ template <int kSlots, bool kBudget = false>
 __global__ void __launch_bounds__(k2::kWarpsPerBlock * 32, DS_K2_MIN_BLOCKS) simulate_kernel(const __grid_constant__ Params p) {
   constexpr int kFac = kBudget ? 4 : 3;
   __shared__ unsigned long long heap_sm[kWarpsPerBlock][kHeapSmem];
+  __shared__ Slots<kSlots> slots_sm[kWarpsPerBlock];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   // Policy affinity per SM: every warp of an SM starts on the same bucket and, when it is empty, moves to the bucket
   // with the most instances left, so that an SM executes one policy's code at a time (instruction-cache locality).
@@ -620,8 +695,8 @@ __global__ void __launch_bounds__(k2::kWarpsPerBlock * 32, DS_K2_MIN_BLOCKS) sim
     if (lane < kFac) p.ema_final[kFac * (size_t)inst_id + lane] = 1.0;   // overwritten unless the trace is rejected
     const bool small = trace_is_small(p, in.trace, lane);
 #define DS_RUN(POL)                                                                                             \
-  if (small) run_instance<kSlots, POL, true, kBudget>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane);    \
-  else run_instance<kSlots, POL, false, kBudget>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], lane)
+  if (small) run_instance<kSlots, POL, true, kBudget>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], slots_sm[wib], lane);    \
+  else run_instance<kSlots, POL, false, kBudget>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], slots_sm[wib], lane)
     switch (in.policy) {
       case DS_FIFO: DS_RUN(DS_FIFO); break;
       case DS_PRIORITY: DS_RUN(DS_PRIORITY); break;
@@ -638,8 +713,9 @@ __global__ void __launch_bounds__(k2::kWarpsPerBlock * 32, DS_K2_MIN_BLOCKS) sim
 
 static size_t perm_bytes(int64_t n_inst) { return align_up(sizeof(unsigned int) * (size_t)(n_inst > 0 ? n_inst : 1), 256); }
 size_t ws_simulate(int64_t total_requests, int64_t n_inst) {
-  return 256 + perm_bytes(n_inst) + sizeof(unsigned long long) * (size_t)total_requests;
+  return align_up(256 + perm_bytes(n_inst) + sizeof(unsigned long long) * (size_t)total_requests, 256);
 }
+size_t ws_simulate_traces(int64_t n_requests) { return align_up(sizeof(k2::Rec) * (size_t)(n_requests > 0 ? n_requests : 1), 256); }
 
 }  // namespace ds
 static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_budget* bp, int32_t n_clients, int64_t think_ticks,
@@ -666,7 +742,8 @@ static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_
   // the whole documented workspace is required: header + permutation + one SJF heap slot per simulated request (the heap
   // region is only touched by SJF instances with more than kHeapSmem requests queued, but which launch will need it is
   // not known on the host)
-  if (workspace_bytes < ws_simulate(n_total, n_inst)) return DS_ENOMEM;
+  if (tr->n_requests < 0) return DS_EINVAL;
+  if (workspace_bytes < ws_simulate(n_total, n_inst) + ws_simulate_traces(tr->n_requests)) return DS_ENOMEM;
   const int n_sms = num_sms();
   if (n_sms < 1) return cuda_fail(cudaGetLastError());
   cudaStream_t s = (cudaStream_t)stream;
@@ -688,8 +765,17 @@ static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_
   p.status = status_ptr();
   if (!p.status) return cuda_fail(cudaGetLastError());
   p.n_total = n_total; p.n_sms = (unsigned)n_sms;
+  k2::Rec* recs = (k2::Rec*)((char*)workspace + ws_simulate(n_total, n_inst));
+  p.rec = recs;
+  p.use_kv = sv->kv_budget > 0; p.want_est = est_out != nullptr; p.want_traj = ema_traj && traj_off && sv->traj_every > 0;
   DS_CUDA(cudaMemsetAsync(workspace, 0, 256, s));
   k2::order_kernel<<<1, 1024, 0, s>>>(inst, n_inst, perm, (unsigned int*)workspace);
+  if (tr->n_requests > 0) {
+    long long pb = (tr->n_requests + 255) / 256;
+    if (pb > (long long)n_sms * 16) pb = (long long)n_sms * 16;
+    k2::pack_kernel<<<(unsigned)pb, 256, 0, s>>>(tr->words, tr->tokens, tr->out_len, tr->n_requests, recs);
+    note_launch();
+  }
   note_launch();
   const int threads = k2::kWarpsPerBlock * 32;
   int per_sm = 0;

@@ -54,7 +54,7 @@ class HotPath:
             self.ema_traj = torch.zeros((int(toff[-1]), 3), dtype=torch.float64, device=dev)
         ws = lambda which, a, b: torch.empty(api.workspace_bytes(which, a, b), dtype=torch.uint8, device=dev)
         self.ws_char = ws(_lib.WS_CHARACTERIZE, 0 if self.text is None else self.text.numel(), self.n_text_prompts)
-        self.ws_sim = ws(_lib.WS_SIMULATE, n, self.n_inst)
+        self.ws_sim = torch.empty(api.simulate_workspace_bytes(n, self.n_inst, self.arrival.numel()), dtype=torch.uint8, device=dev)
         G = self.n_groups
         # histograms, and for the fused call the staging area behind them (5 bytes per simulated request: 32-bit keys + segment codes)
         nb = api.workspace_bytes(_lib.WS_TAIL_STATS, 4 * G, len(self.pct))

@@ -24,6 +24,7 @@ def test_host_only_entry_points():
     assert L.ds_strerror(0) == b"ok" and L.ds_strerror(-3) == b"workspace too small"
     assert L.ds_workspace_bytes(_lib.WS_TAIL_STATS, 4, 2) >= 4 * 2 * 256 * 4
     assert L.ds_workspace_bytes(_lib.WS_SIMULATE, 1000, 10) >= 8000
+    assert 16 * 1000 <= L.ds_workspace_bytes(_lib.WS_SIMULATE_TRACES, 1000, 0) <= 16 * 1000 + 256     # one 16-byte record per trace request
     # staging area of ds_latency_stats: 5 bytes per simulated request (+ alignment room); 0 requests -> the 256-byte floor
     assert 5 * 10**6 <= L.ds_workspace_bytes(_lib.WS_LATENCY_STAGE, 10**6, 0) <= 5 * 10**6 + 2048
     assert L.ds_workspace_bytes(_lib.WS_LATENCY_STAGE, 0, 0) == 256
@@ -32,12 +33,13 @@ def test_host_only_entry_points():
 
 
 def test_struct_layouts_match_header():
-    assert ctypes.sizeof(_lib.DsTraces) == 56 and ctypes.sizeof(_lib.DsServer) == 80
+    assert ctypes.sizeof(_lib.DsTraces) == 64 and ctypes.sizeof(_lib.DsServer) == 80
     from paper_2606_02982_b200 import workload as wl
     assert wl.INSTANCE_DTYPE.itemsize == 24
     hdr = open(os.path.join(ROOT, "include", "driftsched.h")).read()
     assert "#define DS_AGING_UNCLAMPED 5" in hdr and wl.AGING_UNCLAMPED == 5 and wl.POLICY_NAMES[5] == "AGING_UNCLAMPED"
     assert "#define DS_WS_LATENCY_STAGE 3" in hdr and _lib.WS_LATENCY_STAGE == 3
+    assert "#define DS_WS_SIMULATE_TRACES 4" in hdr and _lib.WS_SIMULATE_TRACES == 4
 
 
 def test_no_oracle_in_product_path():

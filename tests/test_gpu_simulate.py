@@ -149,7 +149,7 @@ def test_workspace_and_output_ranges_are_validated(G):
     c = wl._trace_workload("t", 41, 1, 2000, sv, [(wl.SJF, wl.SPLIT, 0.1)], None, rho=3.0, materialise=False)   # overload: queue > 256
     d = G.upload(c)
     n_total = int(c.out_off[-1])
-    need = ds.workspace_bytes(_lib.WS_SIMULATE, n_total, c.n_inst)
+    need = ds.simulate_workspace_bytes(n_total, c.n_inst, c.n_traces * c.n_req)      # both mandatory parts
     args = (d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"], c.server, d["inst"], d["out_off"], n_total)
     with pytest.raises(ds.DsError) as e:
         ds.simulate(*args, workspace=torch.empty(need - 1, dtype=torch.uint8, device=G.DEV))
