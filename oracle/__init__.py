@@ -35,7 +35,7 @@ class _Traces(C.Structure):
 class _Server(C.Structure):
     _fields_ = [("max_batch", C.c_int32), ("kv_budget", C.c_int64), ("c_base", C.c_int64), ("c_batch", C.c_int64),
                 ("c_ctx", C.c_int64), ("c_prefill", C.c_int64), ("weight", C.c_int32 * 3), ("aging_step", C.c_int64),
-                ("traj_every", C.c_int32)]
+                ("traj_every", C.c_int32), ("reestimate", C.c_int32)]
 
 
 class _Budget(C.Structure):
@@ -98,7 +98,7 @@ def _traces(trace_off, arrival, tier, words, tokens, out_len):
 
 def _server(sv):
     return _Server(sv.max_batch, sv.kv_budget, sv.c_base, sv.c_batch, sv.c_ctx, sv.c_prefill,
-                   (C.c_int32 * 3)(*sv.weight), sv.aging_step, sv.traj_every)
+                   (C.c_int32 * 3)(*sv.weight), sv.aging_step, sv.traj_every, int(getattr(sv, "reestimate", 0)))
 
 
 def traj_offsets(trace_off, instances, traj_every):

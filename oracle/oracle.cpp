@@ -76,6 +76,26 @@ struct Sim {
   bool budget() const { return estimator >= BUDGET_SPLIT; }
   int64_t base(int64_t r) const { return (estimator == SPLIT || estimator == BUDGET_SPLIT) ? (int64_t)W[r] : (int64_t)P[r]; }
 
+  // Online re-estimation ("adaptive queue reordering, online workload
+  // reclassification"; reading A16 in DESIGN.md §4): with sv->reestimate the estimate of a QUEUED request is not frozen at
+  // arrival (A5) but recomputed from the factors current at every scheduling decision; est[r] ends as the value in force
+  // when r was admitted to the batch.
+  bool reest() const { return sv->reestimate != 0; }
+  int64_t estimate_now(int64_t r) const {
+    int64_t b = base(r);
+    if (budget()) {
+      int c = cat[r];
+      double F = 1.0 + bp->f_slope * (double)b;
+      if (F > bp->f_max) F = bp->f_max;
+      double x = bp->t_base[c] * B[c];
+      x = x * bp->s_tenant[tier[r]];
+      x = x * F;
+      return b + (int64_t)std::ceil(x);
+    }
+    return b > 0 ? (int64_t)std::ceil(B[tier[r]] * (double)b) : 0;
+  }
+  int64_t queued_est(int64_t r) const { return reest() ? estimate_now(r) : est[r]; }
+
   // admit_to_queue(r): estimate frozen at arrival (A5), Eq. 1-2 reduced form (A1).
   void admit_to_queue(int64_t r) {
     int64_t b = base(r);
@@ -137,7 +157,7 @@ struct Sim {
       switch (policy) {
         case FIFO: k0 = 0; break;                                   // key = seq
         case PRIORITY: k0 = tier[r]; break;                         // (tier, seq)
-        case SJF: k0 = est[r]; break;                               // (est, seq)
+        case SJF: k0 = queued_est(r); break;                        // (est, seq)   PAPER.md:231; A16: with the current factors
         default: {                                                  // AGING (A10)
           // PAPER.md:242 "waiting time progressively reduces the effective scheduling score". AGING clamps the score
           // at Premium's level (A10); AGING_UNCLAMPED (reading A15) lets it fall below 0, so
@@ -171,6 +191,7 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
   if (sv->max_batch < 1) return -1;
   if (sv->weight[0] < 1 || sv->weight[1] < 1 || sv->weight[2] < 1) return -1;
   if (sv->aging_step < 1) return -1;
+  if (sv->reestimate != 0 && sv->reestimate != 1) return -1;
   for (int64_t ii = 0; ii < n_inst; ++ii) {
     const oracle_instance& in = inst[ii];
     if (in.trace < 0 || in.trace >= tr->n_traces || in.policy < 0 || in.policy > AGING_UNCLAMPED || !(in.ema_alpha >= 0.0 && in.ema_alpha <= 1.0))
@@ -235,7 +256,9 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
         int wpos = 0;
         size_t qi = s.peek(&wpos);
         int64_t c = s.queued[qi];
-        if (!s.R.empty() && sv->kv_budget > 0 && s.kv_used + s.est[c] > sv->kv_budget) break;  // deferred (A8)
+        int64_t est_c = s.queued_est(c);                     // frozen at arrival (A5), or re-estimated now (A16)
+        if (!s.R.empty() && sv->kv_budget > 0 && s.kv_used + est_c > sv->kv_budget) break;  // deferred (A8)
+        s.est[c] = est_c;                                     // (A16: the estimate in force at admission to the batch)
         s.queued.erase(s.queued.begin() + qi);
         if (s.policy == WEIGHTED) s.cur = (wpos + 1) % (sv->weight[0] + sv->weight[1] + sv->weight[2]);
         st[c] = s.now; s.g[c] = 0;

@@ -34,6 +34,7 @@ typedef struct {
   int32_t weight[3];
   int64_t aging_step;
   int32_t traj_every;
+  int32_t reestimate;          /* 0: estimates frozen at arrival (A5); 1: online re-estimation of queued requests (A16) */
 } oracle_server;
 
 /* policy: 0 FIFO, 1 PRIORITY, 2 WEIGHTED, 3 SJF, 4 AGING (score clamped at Premium's level, A10),

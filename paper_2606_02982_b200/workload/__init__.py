@@ -140,6 +140,7 @@ class Server:
     weight: tuple = (4, 2, 1)
     aging_step: int = 500_000
     traj_every: int = 0
+    reestimate: int = 0      # 1: online re-estimation of queued requests (NEXT-4; A16)
 
 
 @dataclass
