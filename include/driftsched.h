@@ -89,6 +89,12 @@ typedef struct {              /* continuous-batching server model, BASELINE.json
   int32_t weight[3];           /* Weighted policy slots per tier, each >= 1: {4,2,1} configs, {5,3,2} PAPER.md:234 */
   int64_t aging_step;          /* ticks waited per promoted tier level, >= 1 */
   int32_t traj_every;          /* 0 = no EMA trajectory; k = sample B[0..2] every k completions */
+  int32_t reestimate;          /* 0 = estimates frozen at arrival (reading A5, the measured path). 1 = online re-estimation of queued
+                                  requests ("adaptive queue reordering, online workload
+                                  reclassification"; A16): SJF's key and the KV admission check use ceil(B[tier]*base) with the
+                                  factors current at the scheduling decision, est_out is the estimate in force when the request was
+                                  admitted to the batch. ds_simulate / ds_simulate_est only (DS_EINVAL with the budget estimators); a
+                                  variant that scans the queue at every pick, not tuned for throughput. */
 } ds_server;
 
 #define DS_FIFO 0

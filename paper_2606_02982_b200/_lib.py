@@ -25,7 +25,7 @@ class DsTraces(C.Structure):
 class DsServer(C.Structure):
     _fields_ = [("max_batch", C.c_int32), ("kv_budget", C.c_int64), ("c_base", C.c_int64), ("c_batch", C.c_int64),
                 ("c_ctx", C.c_int64), ("c_prefill", C.c_int64), ("weight", C.c_int32 * 3), ("aging_step", C.c_int64),
-                ("traj_every", C.c_int32)]
+                ("traj_every", C.c_int32), ("reestimate", C.c_int32)]
 
 
 class DsBudget(C.Structure):

@@ -76,7 +76,7 @@ def _traces(trace_off, arrival, tier, words, tokens, out_len):
 
 def _server(sv):
     return DsServer(sv.max_batch, sv.kv_budget, sv.c_base, sv.c_batch, sv.c_ctx, sv.c_prefill, (C.c_int32 * 3)(*sv.weight),
-                    sv.aging_step, sv.traj_every)
+                    sv.aging_step, sv.traj_every, int(getattr(sv, "reestimate", 0)))
 
 
 def instances_to_device(instances: np.ndarray, device):

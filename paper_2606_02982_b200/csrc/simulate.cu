@@ -144,14 +144,18 @@ struct TierCursor {
 // trace_is_small(), so they are kept in 32-bit registers and the closed-form jump is two IMAD.WIDE; `now` stays 64-bit.
 // kBudget: the paper's full estimator (Eq. 1-2) with one feedback factor per semantic category (lanes 0..3) instead of
 // the reduced per-tier one (lanes 0..2); a separate instantiation so that the benchmarked path is not touched.
-template <int kSlots, int kPolicy, bool kSmall, bool kBudget>
+// kReest: online re-estimation of queued requests (ds_server.reestimate; reading A16): estimates follow the factors, so
+// neither the SJF heap (keys frozen at insertion) nor the per-tier cursors' cached estimates apply. The queue is a plain
+// array of request indices in the workspace; every pick scans it, 32 entries per step, with the policy's key evaluated on
+// the spot - the oracle's linear peek run by a warp. A variant, not the benchmarked path: O(queue/32) per admission.
+template <int kSlots, int kPolicy, bool kSmall, bool kBudget, bool kReest = false>
 __device__ __forceinline__ void run_instance(const Params& p, const unsigned inst_id, const int trace, const bool split, const double alpha,
                                           unsigned long long* heap_sm, Slots<kSlots>& sl, const int lane) {
   constexpr bool kAging = kPolicy == DS_AGING || kPolicy == DS_AGING_UNCLAMPED;   // both read the heads' arrival ticks
-  constexpr bool kCursor = kPolicy == DS_PRIORITY || kPolicy == DS_WEIGHTED || kAging;
+  constexpr bool kCursor = !kReest && (kPolicy == DS_PRIORITY || kPolicy == DS_WEIGHTED || kAging);
   const long long lo = p.trace_off[trace];
   const long long n64 = p.trace_off[trace + 1] - lo;
-  if (n64 < 0 || n64 > 0x7ffffff0ll || (kPolicy == DS_SJF && n64 > (1 << 24))) {   // local indices are 32-bit (SJF keys: 24-bit)
+  if (n64 < 0 || n64 > 0x7ffffff0ll || (!kReest && kPolicy == DS_SJF && n64 > (1 << 24))) {   // local indices are 32-bit (SJF keys: 24-bit)
     if (lane == 0) atomicOr(p.status, n64 > (1 << 24) ? DS_DEV_KEY_RANGE : DS_DEV_BAD_TRACE);
     return;
   }
@@ -197,6 +201,8 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   for (int s = 0; s < kSlots; ++s) { sl.idx[s * 32 + lane] = kFreeIdx; sl.fin[s * 32 + lane] = 0u; sl.stack[s * 32 + lane] = (unsigned short)(s * 32 + lane); }
   __syncwarp();
   Heap heap; heap.sm = heap_sm; heap.gm = p.heap_ws + oo; heap.size = 0;
+  int* const q = reinterpret_cast<int*>(p.heap_ws + oo);     // kReest: the queued request indices, unordered (n entries fit twice)
+  int qn = 0;
   TierCursor tc[3];
   const int wtot = p.w0 + p.w1 + p.w2;
 
@@ -263,6 +269,11 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       if (m == 0) break;
       const int c = __popc(m);
       long long est = 0;
+      if constexpr (kReest) {                                 // A16: no estimate is taken at arrival; the request joins the array
+        if (pred) __stcg(q + qn + (i - next), i);             // (the ingested lanes are contiguous from request `next`)
+        qn += c;
+        __syncwarp();
+      } else
       if (kBudget) {
         if (need_est) {                                       // Eq. 1-2 in full, frozen at arrival (A5)
           const double tb = w_cat == 0 ? p.bp.t_base[0] : w_cat == 1 ? p.bp.t_base[1] : w_cat == 2 ? p.bp.t_base[2] : p.bp.t_base[3];
@@ -280,8 +291,9 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
           if (w_base > 0) est = (long long)ceil(__dmul_rn(Bt, (double)w_base));
         } else est = w_base;                                  // B == 1.0 exactly
       }
-      if (est_o && pred) est_o[i] = est;                      // frozen admission-time estimate (ds_simulate_est)
-      if (kPolicy == DS_SJF) {
+      if (!kReest && est_o && pred) est_o[i] = est;           // frozen admission-time estimate (ds_simulate_est)
+      if constexpr (kReest) {
+      } else if (kPolicy == DS_SJF) {
         if (pred && est >= (1ll << 39)) atomicOr(p.status, DS_DEV_KEY_RANGE);
         unsigned mm = m;
         while (mm) {
@@ -417,6 +429,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   };
 
   auto queue_nonempty = [&]() -> bool {
+    if (kReest) return qn > 0;
     if (kPolicy == DS_FIFO) return fifo_head < next;
     if (kPolicy == DS_SJF) return heap.size > 0;
     return tc[0].head < next || tc[1].head < next || tc[2].head < next;
@@ -434,6 +447,65 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
     }
     while (b < max_batch) {
       int c = -1, ct = 0, wpos = 0; long long est_c = 0;
+      int qpos = 0;
+      if constexpr (kReest) {
+        if (qn > 0) {
+          // the factors as they are now, in every lane (Bl lives in lanes 0..2)
+          const double B0 = shfl_f64(Bl, 0), B1 = shfl_f64(Bl, 1), B2 = shfl_f64(Bl, 2);
+          auto est_now = [&](const int r, const int tr) -> long long {   // Eq. 1-2 reduced (A1) with the current factor (A16)
+            const int base = max((int)BASE[r], 0);
+            if (!ema_on) return base;                           // B == 1.0 exactly
+            const double Bt = tr == 0 ? B0 : tr == 1 ? B1 : B2;
+            return base > 0 ? (long long)ceil(__dmul_rn(Bt, (double)base)) : 0ll;
+          };
+          long long bk = kInf; int br = kFreeIdx, bp = 0;       // lane-best key (k0, request index) and its position in q
+          int tmin[3] = {kFreeIdx, kFreeIdx, kFreeIdx}, tpos[3] = {0, 0, 0};   // WEIGHTED: oldest queued request per tier
+          for (int j0 = 0; j0 < qn; j0 += 32) {
+            const int j = j0 + lane;
+            if (j < qn) {
+              const int r = __ldcg(q + j);
+              const int tr = min((int)tier[r], 2);
+              if (kPolicy == DS_WEIGHTED) {
+#pragma unroll
+                for (int t = 0; t < 3; ++t) if (tr == t && r < tmin[t]) { tmin[t] = r; tpos[t] = j; }
+              } else {
+                long long k0 = 0;                               // FIFO: key = seq
+                if (kPolicy == DS_PRIORITY) k0 = tr;
+                else if (kPolicy == DS_SJF) k0 = est_now(r, tr);
+                else if (kAging) {
+                  const long long lv = (now - arr_at(r)) / p.aging_step;
+                  k0 = (long long)tr - lv;
+                  if (kPolicy == DS_AGING && k0 < 0) k0 = 0;    // A10: clamped at Premium's level
+                }
+                if (k0 < bk || (k0 == bk && r < br)) { bk = k0; br = r; bp = j; }
+              }
+            }
+          }
+          if (kPolicy == DS_WEIGHTED) {                         // slot pattern (A9): first non-empty tier in block order from cur's block
+            const int m0 = __reduce_min_sync(kFull, tmin[0]), m1 = __reduce_min_sync(kFull, tmin[1]), m2 = __reduce_min_sync(kFull, tmin[2]);
+            const int t0 = cur < p.w0 ? 0 : (cur < p.w0 + p.w1 ? 1 : 2);
+            const unsigned nem = (m0 != kFreeIdx ? 1u : 0u) | (m1 != kFreeIdx ? 2u : 0u) | (m2 != kFreeIdx ? 4u : 0u);
+            ct = -1;
+#pragma unroll
+            for (int k = 2; k >= 0; --k) {
+              int t = t0 + k; if (t >= 3) t -= 3;
+              if ((nem >> t) & 1u) { ct = t; wpos = k == 0 ? cur : (t == 0 ? 0 : (t == 1 ? p.w0 : p.w0 + p.w1)); }
+            }
+            c = ct == 0 ? m0 : ct == 1 ? m1 : m2;
+            const int mine = ct == 0 ? tmin[0] : ct == 1 ? tmin[1] : tmin[2], mp = ct == 0 ? tpos[0] : ct == 1 ? tpos[1] : tpos[2];
+            const unsigned own = __ballot_sync(kFull, mine == c);
+            qpos = __shfl_sync(kFull, mp, __ffs(own) - 1);
+          } else {
+            const unsigned long long kb = warp_min_u64((unsigned long long)bk ^ 0x8000000000000000ull);   // signed order
+            const int cand = ((unsigned long long)bk ^ 0x8000000000000000ull) == kb ? br : kFreeIdx;
+            c = __reduce_min_sync(kFull, cand);
+            const unsigned own = __ballot_sync(kFull, cand == c);
+            qpos = __shfl_sync(kFull, bp, __ffs(own) - 1);
+          }
+          ct = min((int)tier[c], 2);
+          est_c = est_now(c, ct);
+        }
+      } else
       if (kPolicy == DS_FIFO) {
         if (fifo_head < next) { c = fifo_head; est_c = fifo_est; }
       } else if (kPolicy == DS_SJF) {
@@ -479,6 +551,13 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       if (c < 0) break;
       if (b > 0 && use_kv && (long long)kv_used + est_c > p.kv_budget) { blocked = !kAging; break; }   // deferred (A8)
       // pop
+      if constexpr (kReest) {
+        if (lane == 0) { const int lastv = __ldcg(q + qn - 1); __stcg(q + qpos, lastv); }   // order in q is irrelevant: every pick scans all of it
+        --qn;
+        __syncwarp();
+        if (kPolicy == DS_WEIGHTED) { cur = wpos + 1; if (cur >= wtot) cur = 0; }
+        if (est_o) est_o[c] = est_c;                           // the estimate in force at admission to the batch (A16)
+      } else
       if (kPolicy == DS_FIFO) {
         ++fifo_head;
         if (use_kv && fifo_head < next) fifo_est = (long long)__ldcg(dn + fifo_head);
@@ -649,7 +728,7 @@ __global__ void __launch_bounds__(1024) order_kernel(const ds_instance* __restri
   }
 }
 
-template <int kSlots, bool kBudget = false>
+template <int kSlots, bool kBudget = false, bool kReest = false>
 __global__ void __launch_bounds__(k2::kWarpsPerBlock * 32, DS_K2_MIN_BLOCKS) simulate_kernel(const __grid_constant__ Params p) {
   constexpr int kFac = kBudget ? 4 : 3;
   __shared__ unsigned long long heap_sm[kWarpsPerBlock][kHeapSmem];
@@ -695,8 +774,8 @@ __global__ void __launch_bounds__(k2::kWarpsPerBlock * 32, DS_K2_MIN_BLOCKS) sim
     if (lane < kFac) p.ema_final[kFac * (size_t)inst_id + lane] = 1.0;   // overwritten unless the trace is rejected
     const bool small = trace_is_small(p, in.trace, lane);
 #define DS_RUN(POL)                                                                                             \
-  if (small) run_instance<kSlots, POL, true, kBudget>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], slots_sm[wib], lane);    \
-  else run_instance<kSlots, POL, false, kBudget>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], slots_sm[wib], lane)
+  if (small && !kReest) run_instance<kSlots, POL, true, kBudget, false>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], slots_sm[wib], lane);    \
+  else run_instance<kSlots, POL, false, kBudget, kReest>(p, inst_id, in.trace, split, in.ema_alpha, heap_sm[wib], slots_sm[wib], lane)
     switch (in.policy) {
       case DS_FIFO: DS_RUN(DS_FIFO); break;
       case DS_PRIORITY: DS_RUN(DS_PRIORITY); break;
@@ -731,6 +810,7 @@ static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_
   if (sv->max_batch < 1 || sv->max_batch > 256) return DS_EINVAL;
   if (sv->weight[0] < 1 || sv->weight[1] < 1 || sv->weight[2] < 1 || sv->aging_step < 1 || sv->traj_every < 0) return DS_EINVAL;
   if (sv->c_base < 0 || sv->c_batch < 0 || sv->c_ctx < 0 || sv->c_prefill < 0) return DS_EINVAL;
+  if ((sv->reestimate != 0 && sv->reestimate != 1) || (sv->reestimate && bp)) return DS_EINVAL;   // A16 is built for ds_simulate / ds_simulate_est
   if (sv->c_base > 0x7fffffff || sv->c_batch > 0x7fffffff || sv->c_ctx > 0x7fffffff || sv->c_prefill > 0x7fffffff) return DS_EINVAL;
   if (n_inst > 0x7fffffff) return DS_EINVAL;
   if (bp) {
@@ -790,6 +870,7 @@ static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_
     DS_CUDA(cudaGetLastError());
     return DS_OK;
   };
+  if (sv->reestimate) return launch(k2::simulate_kernel<8, false, true>);   // the variant's one instantiation serves every max_batch <= 256
   if (bp) {
     if (sv->max_batch <= 32) return launch(k2::simulate_kernel<1, true>);
     if (sv->max_batch <= 64) return launch(k2::simulate_kernel<2, true>);
