@@ -254,7 +254,9 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
 
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  // the warp index through a warp reduction: its result lives in a uniform register, so everything derived from it (the
+  // span, the TMA row and barrier operands) is uniform for the compiler and the TMA issue needs no operand-broadcast loop
+  const int lane = threadIdx.x & 31, warp = (int)__reduce_max_sync(kFull, threadIdx.x >> 5);
   const long long gw = (long long)blockIdx.x * kWarps + warp, nw = (long long)gridDim.x * kWarps;
   const long long c_begin = gw * n_chunks / nw, c_end = (gw + 1) * n_chunks / nw;   // this warp's span of chunks
   if (c_begin >= c_end) return;                                                     // (no block-wide barrier below)
@@ -487,7 +489,8 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
 #pragma unroll
     for (int g = 0; g < NW; ++g) { att[(h * 32 + lane) * NW + g] = make_uint4(fw[g], ft[g], run, 0u); run += cpk[g]; }
     total += __reduce_add_sync(kFull, own);                           // <= 8192 per field: no carry between the halves
-    if (++s == kStages) { s = 0; parity ^= 1u; }
+    if (kStages == 2) { parity ^= (unsigned)s; s ^= 1; }             // the phase flips when the ring wraps from stage 1 to 0
+    else if (++s == kStages) { s = 0; parity ^= 1u; }
   }
   __syncwarp();
 
