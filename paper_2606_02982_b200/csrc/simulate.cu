@@ -40,8 +40,8 @@ namespace k2 {
 
 constexpr int kWarpsPerBlock = 4;
 #ifndef DS_K2_MIN_BLOCKS
-#define DS_K2_MIN_BLOCKS 6   // resident 128-thread blocks per SM the register allocation is bounded for (measured: 7 and 8
-                             // spill and gain nothing: 13.27 / 13.62 ms against 13.26 ms; 5, 4, 3 blocks: 14.9 / 17.2 / 20.7 ms)
+#define DS_K2_MIN_BLOCKS 7   // resident 128-thread blocks per SM the register allocation is bounded for (r02, with the running set in
+                             // shared memory: 6 / 7 / 8 blocks = configs[3] at 4096 traces 384.0 / 381.3 / 396.8 ms, configs[1] 12.92 / 12.47 / 13.29 ms)
 #endif
 constexpr int kHeapSmem = 256;  // heap entries cached in shared memory per warp
 constexpr long long kInf = 0x7fffffffffffffffLL;
@@ -580,12 +580,13 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
 
   // ---- main loop: one pass per iteration boundary that has an event; event-free boundaries are jumped over ----
   for (;;) {
-#pragma unroll 1
-    for (int ph = 0; ph < 2; ++ph) {                                      // one copy of the ingest code for both phases
-      const long long limit = now - 1 + ph;                               // ticks are integers: "< now" is "<= now-1"
-      if (an <= limit) ingest(limit);                                     // 1. INGEST-EARLY / 3. INGEST-NOW
-      if (ph == 0 && dist == 0) retire();                                 // 2. RETIRE
+    // 1.-3. Two inlined copies of ingest() instead of one in a two-trip loop: the loop's carried state cost ~35 instructions
+    // per request in register moves (measured: configs[3] -4.8 %, configs[1] -6.7 % simulate time).
+    if (dist == 0) {
+      if (an < now) ingest(now - 1);                                      // 1. INGEST-EARLY: arrivals before this tick's completions
+      retire();                                                           // 2. RETIRE
     }
+    if (an <= now) ingest(now);                                           // 3. INGEST-NOW (without a completion at `now`: every arrival up to it)
     // 4. ADMIT. admit() returns with the batch full, the queue empty or (every policy but AGING) `blocked` set, so
     // afterwards something can still be admitted at the next boundary only under AGING (levels change with time)
     bool can_admit = !blocked && b < max_batch && queue_nonempty();

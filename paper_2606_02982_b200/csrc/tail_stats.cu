@@ -260,7 +260,7 @@ __device__ __forceinline__ unsigned match32(const unsigned* pfx32, unsigned s_t,
 
 // kCount: segment counts + AND/OR of all keys. Otherwise: digit-d histogram of the keys matching each (segment, pct) prefix.
 template <bool kCount>
-__global__ void __launch_bounds__(512) lat_pass_kernel(const LatArgs a, int n_pct, int d, Ws* hdr, unsigned long long* counts,
+__global__ void __launch_bounds__(1024) lat_pass_kernel(const LatArgs a, int n_pct, int d, Ws* hdr, unsigned long long* counts,
                                                        const unsigned long long* __restrict__ prefix, unsigned int* hist) {
   extern __shared__ unsigned int sh[];
   const int n_seg = 4 * a.n_groups;
@@ -514,8 +514,10 @@ extern "C" int ds_latency_stats(const ds_traces* tr, const ds_instance* inst, in
   long long per_sm = (long long)(200 * 1024) / (long long)(hsm + 1024);
   if (per_sm > 3) per_sm = 3;
   if (per_sm < 1) per_sm = 1;
+  // when the histograms leave room for one block per SM only (configs[3]/[4]: 160 KB), that block runs 32 warps instead of 16
+  const int threads = per_sm == 1 ? 1024 : 512;
   long long blocks = (long long)num_sms() * per_sm;
-  if (blocks > (n_inst + 15) / 16) blocks = (n_inst + 15) / 16;
+  if (blocks > (n_inst + threads / 32 - 1) / (threads / 32)) blocks = (n_inst + threads / 32 - 1) / (threads / 32);
   if (blocks < 1) blocks = 1;
   for (int metric = 0; metric < 2; ++metric) {
     int64_t* out = metric == 0 ? e2e_out : qdelay_out;
@@ -539,11 +541,11 @@ extern "C" int ds_latency_stats(const ds_traces* tr, const ds_instance* inst, in
       a.skey = (unsigned int*)((char*)workspace + L.total);
       a.scode = (unsigned char*)workspace + L.total + align_up(4 * (size_t)cap, 256);
     }
-    k3::lat_pass_kernel<true><<<(unsigned)blocks, 512, sizeof(unsigned) * (size_t)n_seg, s>>>(a, n_pct, 0, L.hdr, L.counts, L.prefix, L.hist);
+    k3::lat_pass_kernel<true><<<(unsigned)blocks, threads, sizeof(unsigned) * (size_t)n_seg, s>>>(a, n_pct, 0, L.hdr, L.counts, L.prefix, L.hist);
     k3::init_kernel<<<(nsq + 255) / 256, 256, 0, s>>>(L.counts, n_seg, n_pct, pc, L.hdr, L.prefix, L.rank, count_out);
     note_launch(2);
     for (int d = 7; d >= 0; --d) {
-      k3::lat_pass_kernel<false><<<(unsigned)blocks, 512, hsm, s>>>(a, n_pct, d, L.hdr, L.counts, L.prefix, L.hist);
+      k3::lat_pass_kernel<false><<<(unsigned)blocks, threads, hsm, s>>>(a, n_pct, d, L.hdr, L.counts, L.prefix, L.hist);
       k3::select_kernel<<<(nsq + 3) / 4, 128, 0, s>>>(n_seg, n_pct, d, L.hdr, L.counts, L.prefix, L.rank, L.hist, out);
       note_launch(2);
     }

@@ -126,6 +126,25 @@ def test_same_tick_arrivals_and_completions_random(G):
     _assert_same(G.gpu_simulate(c), o, c)
 
 
+def test_many_completions_at_one_boundary(G):
+    # more than 32 requests finishing at the same iteration boundary (equal out_len, admitted together): the retire list's
+    # overflow path, with EMA on so that the ascending-index order of the completions is visible in the factors
+    rng = np.random.default_rng(8)
+    n = 600
+    arr = np.repeat(np.arange(n // 200) * 3_000_000, 200)                     # bursts of 200 simultaneous arrivals
+    req = np.stack([arr, rng.integers(0, 3, n), rng.integers(1, 9, n), rng.integers(1, 12, n), np.where(rng.random(n) < 0.8, 2, 3)], 1)
+    for mb in (48, 64, 128, 256):
+        sv = wl.Server(max_batch=mb, kv_budget=0, aging_step=9000, traj_every=7)
+        c = G.tiny_workload(wl, req, sv, [(p, wl.SPLIT, 0.4) for p in wl.ALL_POLICIES])
+        toff = oracle.traj_offsets(c.trace_off, c.instances, 7)
+        g = G.gpu_simulate(c, traj_off=toff)
+        o = _oracle(c, want_traj=True)
+        _assert_same(g, o, c)
+        assert np.array_equal(g[3].view(np.uint64), o[3].view(np.uint64))
+        per = o[1].reshape(c.n_inst, n)
+        assert max(np.unique(per[0], return_counts=True)[1]) > 32           # the case does put > 32 completions on one tick
+
+
 def test_bad_arguments(G):
     import paper_2606_02982_b200 as ds
     c = wl.config0(oracle.characterize)
