@@ -734,7 +734,11 @@ __global__ void __launch_bounds__(k2::kWarpsPerBlock * 32, DS_K2_MIN_BLOCKS) sim
   constexpr int kFac = kBudget ? 4 : 3;
   __shared__ unsigned long long heap_sm[kWarpsPerBlock][kHeapSmem];
   __shared__ Slots<kSlots> slots_sm[kWarpsPerBlock];
-  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  // lane and warp-in-block through volatile asm: under register pressure the compiler otherwise re-derives them from
+  // SR_TID.X (a 20-cycle S2R plus shifts and the shared-memory address arithmetic) at every use: 27 instructions per request
+  int lane, wib;
+  asm volatile("mov.u32 %0, %%laneid;" : "=r"(lane));
+  asm volatile("{\n.reg .u32 t;\nmov.u32 t, %%tid.x;\nshr.u32 %0, t, 5;\n}" : "=r"(wib));
   // Policy affinity per SM: every warp of an SM starts on the same bucket and, when it is empty, moves to the bucket
   // with the most instances left, so that an SM executes one policy's code at a time (instruction-cache locality).
   // Buckets: SJF, AGING, WEIGHTED, PRIORITY, FIFO, invalid. SMs are split 26/31/35/30/26 (measured relative cost of one
