@@ -347,28 +347,30 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
 #pragma unroll
       for (int s = 0; s < kSlots; ++s) { ri[s] = sl.idx[lane * kSlots + s]; rf[s] = sl.fin[lane * kSlots + s]; }
     }
-    // completions at this boundary (a free slot has idx = kFreeIdx, so its stale fin cannot match)
-    int lm = kFreeIdx, cnt = 0;
+    // completions at this boundary (a free slot has idx = kFreeIdx, so its stale fin cannot match): per lane the smallest
+    // completing request, its slot, and how many of the lane's slots complete
+    int lm = kFreeIdx, ls = 0, cnt = 0;
 #pragma unroll
     for (int s = 0; s < kSlots; ++s) {
       const bool hit = rf[s] == iter && ri[s] != kFreeIdx;
       cnt += hit ? 1 : 0;
-      lm = hit ? min(lm, ri[s]) : lm;
+      if (hit && ri[s] < lm) { lm = ri[s]; ls = s; }
     }
     int left = __reduce_add_sync(kFull, cnt);                 // called with dist == 0: at least one
-    bool freed_any = false;
     while (left > 0) {
-      const int r = __reduce_min_sync(kFull, lm);
+      const int r = __reduce_min_sync(kFull, lm);             // ascending request index (R-ORD)
       if (r == kFreeIdx) break;                               // (defensive: cannot happen; never index with it)
       --left;
-      // owner: clear the slot in registers, push its number on the free stack; then the lane's next candidate
-      lm = kFreeIdx;
-#pragma unroll
-      for (int s = 0; s < kSlots; ++s) {
-        if (ri[s] == r) { ri[s] = kFreeIdx; sl.stack[nfree] = (unsigned short)(lane * kSlots + s); freed_any = true; }
-        if (left > 0) lm = (rf[s] == iter && ri[s] != kFreeIdx) ? min(lm, ri[s]) : lm;
-      }
+      // owner: free the slot in shared memory and push its number on the free stack (registers keep the loaded state: the
+      // completions are told apart from what stays by rf == iter)
+      const bool own = lm == r;
+      if (own) { const int slot = lane * kSlots + ls; sl.idx[slot] = kFreeIdx; sl.stack[nfree] = (unsigned short)slot; --cnt; lm = kFreeIdx; }
       ++nfree;
+      if (kSlots > 1 && __any_sync(kFull, own && cnt > 0)) {  // rare: the owner holds another completion; its next candidate
+#pragma unroll
+        for (int s = 0; s < kSlots; ++s)
+          if (own && rf[s] == iter && ri[s] != kFreeIdx && ri[s] > r && ri[s] < lm) { lm = ri[s]; ls = s; }
+      }
       const Rec rr = rec[r];                                   // one 16-byte load: m, tokens, out_len
       const int Pr = rr.P, Or = max(rr.O, 1);
       dn[r] = now;                                            // every lane, same address and value: one store, no branch
@@ -408,21 +410,10 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       }
       if (traj && done % p.traj_every == 0 && lane < kFac) traj[kFac * (done / p.traj_every - 1) + lane] = Bl;
     }
-    // write the cleared slots back (lanes that freed nothing store what they loaded) and take the distance to the next completion
+    // distance to the next completion: the occupied slots that did not complete now
     unsigned d = 0xffffffffu;
 #pragma unroll
-    for (int s = 0; s < kSlots; ++s) d = ri[s] != kFreeIdx ? min(d, rf[s] - iter) : d;
-    if constexpr (kSlots % 4 == 0) {
-#pragma unroll
-      for (int q = 0; q < kSlots / 4; ++q)
-        *reinterpret_cast<int4*>(&sl.idx[lane * kSlots + 4 * q]) = make_int4(ri[4 * q], ri[4 * q + 1], ri[4 * q + 2], ri[4 * q + 3]);
-    } else if constexpr (kSlots == 2) {
-      *reinterpret_cast<int2*>(&sl.idx[lane * 2]) = make_int2(ri[0], ri[1]);
-    } else {
-#pragma unroll
-      for (int s = 0; s < kSlots; ++s) sl.idx[lane * kSlots + s] = ri[s];
-    }
-    (void)freed_any;
+    for (int s = 0; s < kSlots; ++s) d = (ri[s] != kFreeIdx && rf[s] != iter) ? min(d, rf[s] - iter) : d;
     dist = __reduce_min_sync(kFull, d);
     blocked = false;
     __syncwarp();
