@@ -78,7 +78,7 @@ typedef struct {              /* SoA request records, traces concatenated; HOST 
   const uint8_t* tier;         /* 0 Premium, 1 Standard, 2 Batch */
   const int32_t* words;        /* split() count, >= 0 */
   const int32_t* tokens;       /* pseudo-token count = true prompt length, >= 0 */
-  const int32_t* out_len;      /* decode length, >= 1 */
+  const int32_t* out_len;      /* decode length, in [1, 2^30) */
   int64_t n_requests;          /* HOST copy of trace_off[n_traces]: requests over all traces = length of the five arrays above */
 } ds_traces;
 
@@ -135,7 +135,7 @@ typedef struct {
  *   (touched only by SJF instances with more than 256 requests queued, but always validated), then one packed 16-byte
  *   record per trace request (tokens/words ratio, tokens, out_len; written by a pre-pass of every call).
  * Contract checked on the device (DS_DEV_BAD_TRACE, outputs of that instance unspecified): tier <= 2, words/tokens >= 0,
- *   out_len >= 1, arrival_tick >= 0 and non-decreasing over every pair of neighbouring requests of a trace.
+ *   1 <= out_len < 2^30, arrival_tick >= 0 and non-decreasing over every pair of neighbouring requests of a trace.
  * Launches: 1 memset (work counter) + 3 kernels (policy-major ordering of the instances, request records, simulation). */
 int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
                 const int64_t* out_off, int64_t n_total, int64_t* start_tick, int64_t* done_tick, double* ema_final,

@@ -48,8 +48,10 @@ constexpr long long kInf = 0x7fffffffffffffffLL;
 constexpr unsigned kFull = 0xffffffffu;
 
 // per trace request, written by pack_kernel: m = tokens/words as fp64 (correctly rounded division, the B_measured of Eq. 6
-// under reading A3; -1.0 when words <= 0: no feedback from that request), P = tokens, O = out_len
-struct __align__(16) Rec { double m; int P; int O; };
+// under reading A3; -1.0 when words <= 0: no feedback from that request), P = tokens, O = out_len | tier << 30 (out_len < 2^30
+// is part of the contract, checked by pack_kernel: a completion then needs no second load for the tier)
+struct __align__(16) Rec { double m; int P; unsigned O; };
+constexpr unsigned kRecLenMask = 0x3fffffffu;
 
 struct Params {
   const int64_t* trace_off; const int64_t* arrival; const uint8_t* tier; const int32_t* words; const int32_t* tokens;
@@ -372,7 +374,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
           if (own && rf[s] == iter && ri[s] != kFreeIdx && ri[s] > r && ri[s] < lm) { lm = ri[s]; ls = s; }
       }
       const Rec rr = rec[r];                                   // one 16-byte load: m, tokens, out_len
-      const int Pr = rr.P, Or = max(rr.O, 1);
+      const int Pr = rr.P, Or = max((int)(rr.O & kRecLenMask), 1);
       dn[r] = now;                                            // every lane, same address and value: one store, no branch
       kv_used -= (acc_t)Pr + (acc_t)Or;
       --b;
@@ -389,7 +391,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
           }
         }
       } else if (ema_on) {                                    // Eq. 5-6 (A3): four separately rounded operations; m = P/W came
-        const int tr = min((int)tier[r], 2);                  // rounded from pack_kernel (the same correctly rounded division)
+        const int tr = (int)(rr.O >> 30);                     // rounded from pack_kernel (the same correctly rounded division)
         if (rr.m >= 0.0) {                                    // words > 0
           const double t2 = __dmul_rn(t1, shfl_f64(Bl, tr));
           const double t3 = __dmul_rn(alpha, rr.m);
@@ -560,7 +562,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       }
       const Rec rc = rec[c];                                   // one 16-byte load: tokens, out_len (m unused here)
       const int Pc = rc.P;
-      const int Oc = max(rc.O, 1);                             // (a bad out_len was reported when its window was loaded)
+      const int Oc = max((int)(rc.O & kRecLenMask), 1);        // (a bad out_len was reported when its window was loaded)
       st[c] = now;                                             // every lane, same address and value
       const int slot = sl.stack[--nfree];                      // b < max_batch <= 32*kSlots: a free slot exists
       sl.idx[slot] = c; sl.fin[slot] = iter + (unsigned)Oc;    // (uniform address and value)
@@ -649,13 +651,14 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
 // One 16-byte record per TRACE request (shared by all instances of the trace): the feedback ratio m = tokens/words of Eq. 6
 // (reading A3) as a correctly rounded fp64 division - bit-identical to dividing at every completion - and the two lengths.
 __global__ void __launch_bounds__(256) pack_kernel(const int32_t* __restrict__ W, const int32_t* __restrict__ P, const int32_t* __restrict__ O,
-                                                   long long n, Rec* __restrict__ rec) {
+                                                   const uint8_t* __restrict__ tier, long long n, Rec* __restrict__ rec, unsigned int* status) {
   const long long stride = (long long)gridDim.x * blockDim.x;
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-    const int w = W[i], pt = P[i];
+    const int w = W[i], pt = P[i], o = O[i];
+    if (o > (int)kRecLenMask) atomicOr(status, DS_DEV_BAD_TRACE);     // (out_len < 1, tier > 2: reported when the window is loaded)
     Rec r;
     r.m = w > 0 ? __ddiv_rn((double)pt, (double)w) : -1.0;
-    r.P = pt; r.O = O[i];
+    r.P = pt; r.O = ((unsigned)max(o, 0) & kRecLenMask) | ((unsigned)min((int)tier[i], 2) << 30);
     rec[i] = r;
   }
 }
@@ -849,7 +852,7 @@ static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_
   if (tr->n_requests > 0) {
     long long pb = (tr->n_requests + 255) / 256;
     if (pb > (long long)n_sms * 16) pb = (long long)n_sms * 16;
-    k2::pack_kernel<<<(unsigned)pb, 256, 0, s>>>(tr->words, tr->tokens, tr->out_len, tr->n_requests, recs);
+    k2::pack_kernel<<<(unsigned)pb, 256, 0, s>>>(tr->words, tr->tokens, tr->out_len, tr->tier, tr->n_requests, recs, p.status);
     note_launch();
   }
   note_launch();
