@@ -62,8 +62,8 @@ def test_against_python_split_random_bytes():
     # adversarial alphabet: every whitespace byte incl. 0x0b/0x0c/0x0d, near-misses (0x08,0x0e,0x1c-0x1f,0x85,0xa0),
     # punctuation range edges, letters, digits, high bytes
     alpha = np.frombuffer(b" \t\n\r\x0b\x0c\x08\x0e\x1c\x1f\x7f\x80\x85\xa0\xff!/:@[`{~09AZaz_\x00,.", np.uint8)
-    buf = alpha[rng.integers(0, len(alpha), 400_000)]
-    cuts = np.sort(rng.integers(0, buf.size + 1, 60_000))
+    buf = alpha[rng.integers(0, len(alpha), 6_000_000)]
+    cuts = np.sort(rng.integers(0, buf.size + 1, 1_000_000))      # SURVEY.md §8(c) C.1 pin (1): >= 1 M prompts, WS runs of every length
     off = np.concatenate([[0], cuts, [buf.size]])
     w, t = oracle.characterize(buf, off)
     rw, rt = _py_reference(buf.tobytes(), off.tolist())
