@@ -31,8 +31,8 @@ sys.path.insert(0, ROOT)
 
 METRIC = "simulated requests/sec (policy x trace)"
 UNIT = "req/s"
-K2_COUNTS = os.path.join(ROOT, "profiles", "r02_k2_counts.json")     # ncu-counted instructions per simulated request (see its "how")
-TRAFFIC = os.path.join(ROOT, "profiles", "r02_traffic.json")         # ncu dram bytes per launch of the dominant kernels
+K2_COUNTS = os.path.join(ROOT, "profiles", "r02_k2_counts.json.txt")     # ncu-counted instructions per simulated request (see its "how")
+TRAFFIC = os.path.join(ROOT, "profiles", "r02_traffic.json.txt")         # ncu dram bytes per launch of the dominant kernels
 SIM_CU = os.path.join(ROOT, "paper_2606_02982_b200", "csrc", "simulate.cu")
 
 
@@ -203,7 +203,7 @@ def k2_roofline(kernel_key, n_sim, sim_ms, sm_max):
     cap = _json(K2_COUNTS)
     ent = cap.get(kernel_key)
     if not ent:
-        out["reason"] = "no ncu capture of this instantiation in profiles/r02_k2_counts.json"
+        out["reason"] = "no ncu capture of this instantiation in profiles/r02_k2_counts.json.txt"
         return out
     try:
         sha = hashlib.sha256(open(SIM_CU, "rb").read()).hexdigest()
@@ -211,8 +211,8 @@ def k2_roofline(kernel_key, n_sim, sim_ms, sm_max):
         sha = None
     out["capture"] = {"commit": cap.get("commit"), "simulate_cu_sha256": cap.get("simulate_cu_sha256"),
                       "ncu_issue_active_pct": ent.get("issue_active_pct"), "ncu_achieved_occupancy_pct": ent.get("achieved_occupancy_pct"),
-                      "ncu_inst_per_simreq": ent.get("inst_per_simreq"), "file": "profiles/r02_k2_counts.json"}
-    floor = cap.get("floor_inst_per_simreq")
+                      "ncu_inst_per_simreq": ent.get("inst_per_simreq"), "file": "profiles/r02_k2_counts.json.txt"}
+    floor = ent.get("floor_inst_per_simreq")
     if floor:
         fa = floor * n_sim / (sim_ms * 1e-3) / 1e9
         out["algorithmic"] = {"inst_per_simreq_floor": floor, "achieved": fa, "frac": fa / peak, "source": "DESIGN.md §6.2"}

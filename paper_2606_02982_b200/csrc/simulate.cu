@@ -724,7 +724,8 @@ __global__ void __launch_bounds__(1024) order_kernel(const ds_instance* __restri
 }
 
 template <int kSlots, bool kBudget = false, bool kReest = false>
-__global__ void __launch_bounds__(k2::kWarpsPerBlock * 32, DS_K2_MIN_BLOCKS) simulate_kernel(const __grid_constant__ Params p) {
+__global__ void __launch_bounds__(k2::kWarpsPerBlock * 32, (kSlots == 1 && !kBudget) ? DS_K2_MIN_BLOCKS + 1 : DS_K2_MIN_BLOCKS)
+simulate_kernel(const __grid_constant__ Params p) {   // (one slot per lane: 8 blocks of 64 registers win, configs[1] 11.16 -> 10.51 ms; 4 / 8 slots: 7 blocks)
   constexpr int kFac = kBudget ? 4 : 3;
   __shared__ unsigned long long heap_sm[kWarpsPerBlock][kHeapSmem];
   __shared__ Slots<kSlots> slots_sm[kWarpsPerBlock];
