@@ -32,14 +32,23 @@
 namespace ds {
 namespace k1 {
 
-constexpr int kWarps = 8;                     // warps per CTA (each fully independent)
+#ifndef DS_K1_WARPS
+#define DS_K1_WARPS 8
+#endif
+#ifndef DS_K1_SUB
+#define DS_K1_SUB 2
+#endif
+#ifndef DS_K1_CTAS
+#define DS_K1_CTAS 2
+#endif
+constexpr int kWarps = DS_K1_WARPS;           // warps per CTA (each fully independent)
 constexpr int kThreads = kWarps * 32;
 constexpr int NW = 4;                         // 32-byte groups (= 32-bit mask words) per lane per chunk
 constexpr int kSeg = 32 * NW;                 // 128 bytes per lane per chunk = one TMA box row
 constexpr int kChunk = 32 * kSeg;             // 4 KiB per warp per step
 constexpr int kStages = 2;
-constexpr int kSub = 2;                       // chunks per boundary-attribution pass (amortises the window handling)
-constexpr int kCtasPerSM = 2;
+constexpr int kSub = DS_K1_SUB;               // chunks per boundary-attribution pass (amortises the window handling)
+constexpr int kCtasPerSM = DS_K1_CTAS;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr long long kInfOff = 0x7fffffffffffffffLL;
 constexpr unsigned kNoRel = 0xffffffffu;      // "no boundary" in span-relative 32-bit positions
