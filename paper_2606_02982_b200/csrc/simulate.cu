@@ -179,10 +179,13 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   constexpr bool kPinPtrs = kSlots > 1 && !kBudget && !kReest;
   int64_t* st = p.start_tick + oo;
   int64_t* dn = p.done_tick + oo;
-  if constexpr (kPinPtrs) { asm volatile("mov.b64 %0, %0;" : "+l"(st)); asm volatile("mov.b64 %0, %0;" : "+l"(dn)); }
+  if constexpr (kPinPtrs) {
+    asm volatile("mov.b64 %0, %0;" : "+l"(st)); asm volatile("mov.b64 %0, %0;" : "+l"(dn));
+    __builtin_assume(__isGlobal(st)); __builtin_assume(__isGlobal(dn));     // (the asm hides the address space: keep STG, not generic ST)
+  }
   const int32_t* __restrict__ BASE = split ? W : P;
   const Rec* rec = p.rec + lo;
-  if constexpr (kSlots > 1 && !kBudget && !kReest) asm volatile("mov.b64 %0, %0;" : "+l"(rec));
+  if constexpr (kSlots > 1 && !kBudget && !kReest) { asm volatile("mov.b64 %0, %0;" : "+l"(rec)); __builtin_assume(__isGlobal(rec)); }
   const bool use_kv = p.use_kv != 0;
   int64_t* est_o = p.want_est ? p.est_out + oo : nullptr;
   const bool need_est = use_kv || kPolicy == DS_SJF || est_o != nullptr;
