@@ -199,7 +199,12 @@ def k2_roofline(kernel_key, n_sim, sim_ms, sm_max):
     DESIGN.md §6.2 derives for one request, which does not move with the kernel's own instruction count."""
     peak = 148 * 4 * sm_max * 1e6 / 1e9
     out = {"kernel": "simulate_kernel<%s>" % {"slots1": 1, "slots4": 4, "slots8": 8}[kernel_key], "bound": "alu", "achieved": None,
-           "peak": peak, "unit": "Gwarp-inst/s", "frac": None, "traffic": _json(TRAFFIC).get("simulate_" + kernel_key)}
+           "peak": peak, "unit": "Gwarp-inst/s", "frac": None, "traffic": None}
+    tr = _json(TRAFFIC).get("simulate_" + kernel_key)
+    if tr:   # dram read + write bytes of one launch of this size, from the ncu capture's bytes per simulated request
+        out["traffic"] = tr["dram_bytes_per_simreq"] * n_sim
+        out["traffic_source"] = "profiles/r02_traffic.json.txt: %.1f DRAM bytes per simulated request (ncu --set full, %s) x requests of this launch; algorithmic: 37 B (DESIGN.md §6.2)" % (
+            tr["dram_bytes_per_simreq"], tr["per_launch_of"])
     cap = _json(K2_COUNTS)
     ent = cap.get(kernel_key)
     if not ent:
@@ -328,7 +333,12 @@ def run_ours(args):
         line["characterization_gbs"] = k1_gbs
         line["roofline_scan"] = {"kernel": "characterize_kernel", "bound": "hbm", "achieved": k1_gbs, "peak": hbm_peak, "unit": "GB/s",
                                  "frac": k1_gbs / hbm_peak, "peak_source": which, "frac_of_8TBps": k1_gbs / 8000.0,
-                                 "traffic": _json(TRAFFIC).get("characterize_kernel"), "workload": "text sample of the headline step"}
+                                 "traffic": None, "workload": "text sample of the headline step"}
+        tk = _json(TRAFFIC).get("characterize_kernel")
+        if tk:
+            line["roofline_scan"]["traffic"] = tk["dram_bytes_per_text_byte"] * text_bytes
+            line["roofline_scan"]["traffic_source"] = "profiles/r02_traffic.json.txt: %.4f DRAM bytes per text byte (ncu --set full, %s)" % (
+                tk["dram_bytes_per_text_byte"], tk["per_launch_of"])
     legs = [x for x in args.legs.split(",") if x] if world == 1 else []
     # CPU baseline first (it needs c): the oracle as it stands on a bounded sample (host cores of this box), rank 0, N=1 only
     if world == 1 and not args.no_cpu_baseline:
