@@ -40,6 +40,7 @@ extern "C" {
 #define DS_EINVAL (-1) /* bad argument / host-checkable contract violation */
 #define DS_ECUDA (-2)  /* CUDA runtime error (see ds_last_cuda_error) */
 #define DS_ENOMEM (-3) /* workspace too small */
+#define DS_ELIMIT (-4) /* size beyond the built-in scratch of a *_static entry point (use the workspace form of the call) */
 
 /* bits of the device status word (ds_device_status) */
 #define DS_DEV_BAD_OFFSETS 1u  /* ds_characterize: offsets not in [0,n_bytes] or decreasing */
@@ -239,6 +240,23 @@ int ds_latencies(const ds_traces* tr, const ds_instance* inst, int64_t n_inst, c
  * workspace: ds_workspace_bytes(DS_WS_TAIL_STATS, n_segments, n_pct). Launches: 1 memset + up to 9 x 2 kernels. */
 int ds_tail_stats(const int64_t* values, const int32_t* seg_id, int64_t n, int32_t n_segments, const int32_t* pct,
                   int32_t n_pct, int64_t* out, int64_t* count_out, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ds_tail_stats WITHOUT a caller workspace, for callers that cannot allocate device memory (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): the scratch (header, counts, prefixes, ranks, radix histograms)
+ * is one fixed device array inside the library, DS_TAIL_STATS_STATIC_BYTES (134 400) bytes, present on every GPU that
+ * loads the library until the process exits. The call allocates nothing: no cudaMalloc, cudaFree or allocating library
+ * routine; it enqueues memsets and kernels on `stream` exactly like ds_tail_stats and returns the same results, bit for bit.
+ * Limit: n_segments <= DS_TAIL_STATS_STATIC_MAX_SEGPCT and n_segments * n_pct <= DS_TAIL_STATS_STATIC_MAX_SEGPCT (128);
+ *   anything larger returns DS_ELIMIT ("size beyond the built-in scratch") and launches nothing. n is not limited.
+ * Sharing: every call on a device uses the SAME array, which keeps the last call's contents; each call clears what it
+ *   needs at its start (on `stream`), so calls that follow one another on one stream are independent. Calls that OVERLAP on
+ *   the GPU (two streams, two host threads without ordering between their streams) RACE on the array and give undefined
+ *   results: order them with events, or use ds_tail_stats with one workspace per call in flight.
+ * Everything else (arguments, nearest-rank definition, pct as a HOST array, -1 for an empty segment) as ds_tail_stats. */
+#define DS_TAIL_STATS_STATIC_MAX_SEGPCT 128
+#define DS_TAIL_STATS_STATIC_BYTES 134400
+int ds_tail_stats_static(const int64_t* values, const int32_t* seg_id, int64_t n, int32_t n_segments, const int32_t* pct,
+                         int32_t n_pct, int64_t* out, int64_t* count_out, void* stream);
 
 /* Fused form of ds_latencies + 4 x ds_tail_stats for the report the paper's tables need (Tables VI-VIII: percentiles of
  * end-to-end latency and queue wait per tenant tier and overall): nothing is materialised, every radix pass recomputes

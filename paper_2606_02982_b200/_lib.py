@@ -7,13 +7,14 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdriftsched.so")
 
-DS_OK, DS_EINVAL, DS_ECUDA, DS_ENOMEM = 0, -1, -2, -3
+DS_OK, DS_EINVAL, DS_ECUDA, DS_ENOMEM, DS_ELIMIT = 0, -1, -2, -3, -4
+TAIL_STATS_STATIC_MAX_SEGPCT = 128
 WS_CHARACTERIZE, WS_SIMULATE, WS_TAIL_STATS = 0, 1, 2
 WS_LATENCY_STAGE = 3
 WS_SIMULATE_TRACES = 4
 
 EXPORTS = ["ds_characterize", "ds_simulate", "ds_simulate_est", "ds_simulate_budget", "ds_simulate_closed", "ds_estimation_error", "ds_queue_depth", "ds_latencies", "ds_tail_stats",
-           "ds_latency_stats", "ds_workspace_bytes", "ds_device_status",
+           "ds_tail_stats_static", "ds_latency_stats", "ds_workspace_bytes", "ds_device_status",
            "ds_strerror", "ds_last_cuda_error", "ds_launch_count"]
 
 
@@ -59,6 +60,8 @@ def lib():
         L.ds_queue_depth.argtypes = [C.POINTER(DsTraces), p, i64, p, p, p, i64, i64, i64, p, p]
         L.ds_latencies.argtypes = [C.POINTER(DsTraces), p, i64, p, i64, p, p, p, p, p, p, p, p, p, p]
         L.ds_tail_stats.argtypes = [p, p, i64, i32, C.POINTER(i32), i32, p, p, p, sz, p]
+        L.ds_tail_stats_static.argtypes = [p, p, i64, i32, C.POINTER(i32), i32, p, p, p]
+        L.ds_tail_stats_static.restype = C.c_int
         L.ds_latency_stats.argtypes = [C.POINTER(DsTraces), p, i64, p, p, p, p, p, i32, p, C.POINTER(i32), i32, p, p, p, p, sz, p]
         L.ds_workspace_bytes.argtypes = [C.c_int, i64, i64]
         L.ds_workspace_bytes.restype = sz

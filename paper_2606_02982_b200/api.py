@@ -180,6 +180,18 @@ def tail_stats(values, seg_id, n_segments, pct=(50, 99), out=None, count_out=Non
     return out, count_out
 
 
+def tail_stats_static(values, seg_id, n_segments, out, count_out, pct=(50, 99)):
+    """ds_tail_stats_static: ds_tail_stats on the library's built-in scratch array; the binding allocates nothing either, so
+    `out` int64[n_segments, n_pct] and `count_out` int64[n_segments] (CUDA) must be passed in. Limit: n_segments * n_pct <= 128."""
+    _need_cuda(values, seg_id, out, count_out)
+    assert values.dtype == torch.int64 and seg_id.dtype == torch.int32 and out.dtype == torch.int64 and count_out.dtype == torch.int64
+    n_pct = len(pct)
+    arr = (C.c_int32 * n_pct)(*[int(x) for x in pct])
+    check("ds_tail_stats_static", lib().ds_tail_stats_static(_ptr(values), _ptr(seg_id), values.numel(), n_segments, arr, n_pct,
+                                                             _ptr(out), _ptr(count_out), _stream()))
+    return out, count_out
+
+
 def latency_stats(trace_off, arrival, tier, words, tokens, out_len, inst, out_off, start, done, group, n_groups, t_mid=None,
                   pct=(50, 99), e2e_out=None, qdelay_out=None, count_out=None, workspace=None, stage=True, arrival_override=None):
     """ds_latency_stats -> (e2e_out, qdelay_out, count_out), each laid out [4*G, n_pct] / [4*G] with G = n_groups * phases:

@@ -99,6 +99,7 @@ const char* ds_strerror(int code) {
     case DS_EINVAL: return "invalid argument";
     case DS_ECUDA: return "CUDA runtime error";
     case DS_ENOMEM: return "workspace too small";
+    case DS_ELIMIT: return "size beyond the built-in scratch of a *_static entry point";
     default: return "unknown error";
   }
 }

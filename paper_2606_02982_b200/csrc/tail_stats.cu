@@ -7,6 +7,7 @@
 // atomics otherwise) -> select kernel (one thread per (segment, percentile) walks 256 bins, fixes the digit,
 // reduces the rank). Traffic: 12 B per value per non-skipped digit; only keys matching the prefix are counted.
 #include "common.cuh"
+#include <mutex>
 #include <type_traits>
 
 namespace ds {
@@ -552,4 +553,61 @@ extern "C" int ds_latency_stats(const ds_traces* tr, const ds_instance* inst, in
   }
   DS_CUDA(cudaGetLastError());
   return DS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// ds_tail_stats_static: ds_tail_stats for callers that cannot allocate (code under CUDA graph capture, tight serving
+// loops, harnesses that forbid cudaMalloc). The scratch that ds_tail_stats takes from its caller (header, segment counts,
+// prefixes, ranks, radix histograms) lives in ONE file-scope device array of a fixed, modest size instead; the caller
+// still passes inputs and outputs. The array exists on every GPU that loads the library, until the process exits.
+//
+// In HOST code the array's name is a host-side stand-in, not a device address: a kernel given `g_tail_scratch` itself
+// would fault (or, where the GPU can reach host memory, silently use the wrong memory). The device address is looked up
+// once per device, with that device current, by cudaGetSymbolAddress below, and only that pointer is handed on.
+namespace ds {
+namespace k3 {
+
+constexpr int kStaticMaxSegPct = DS_TAIL_STATS_STATIC_MAX_SEGPCT;   // n_segments * n_pct (and n_segments) at most this
+// the largest Layout (make_layout) any admitted (n_segments, n_pct) needs: header 256 + counts + prefix + rank (each
+// 8 bytes per entry, rounded up to 256) + 256 32-bit bins per (segment, percentile)
+constexpr size_t kStaticRow = (8 * (size_t)kStaticMaxSegPct + 255) / 256 * 256;
+constexpr size_t kStaticBytes = 256 + 3 * kStaticRow + 4 * 256 * (size_t)kStaticMaxSegPct;   // 134 400 bytes at 128
+static_assert(kStaticBytes == DS_TAIL_STATS_STATIC_BYTES, "the header states the size of the built-in scratch");
+static __device__ __align__(256) unsigned char g_tail_scratch[kStaticBytes];
+
+constexpr int kStaticMaxDevices = 64;
+static unsigned char* g_tail_scratch_ptr[kStaticMaxDevices];   // device address of g_tail_scratch, per device (nullptr: not looked up yet)
+static std::mutex g_tail_scratch_mu;
+
+// device address of the scratch array on the calling thread's current device; nullptr (error recorded) on a CUDA error
+static unsigned char* static_scratch() {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) { cuda_fail(e); return nullptr; }
+  if (dev < 0 || dev >= kStaticMaxDevices) { cuda_fail(cudaErrorInvalidDevice); return nullptr; }
+  std::lock_guard<std::mutex> lk(g_tail_scratch_mu);
+  if (!g_tail_scratch_ptr[dev]) {
+    unsigned char* ptr = nullptr;
+    e = cudaGetSymbolAddress((void**)&ptr, g_tail_scratch);       // the set-up step: once per device, that device current
+    if (e != cudaSuccess || !ptr) { cuda_fail(e != cudaSuccess ? e : cudaErrorInvalidSymbol); return nullptr; }
+    g_tail_scratch_ptr[dev] = ptr;
+  }
+  return g_tail_scratch_ptr[dev];
+}
+
+}  // namespace k3
+}  // namespace ds
+
+extern "C" int ds_tail_stats_static(const int64_t* values, const int32_t* seg_id, int64_t n, int32_t n_segments, const int32_t* pct,
+                                    int32_t n_pct, int64_t* out, int64_t* count_out, void* stream) {
+  using namespace ds;
+  if (n_segments < 1 || n_pct < 1 || n_pct > k3::kMaxPct) return DS_EINVAL;
+  // beyond the built-in scratch: refuse, never spill (the caller can use ds_tail_stats with a workspace of its own)
+  if (n_segments > k3::kStaticMaxSegPct || (long long)n_segments * n_pct > k3::kStaticMaxSegPct) return DS_ELIMIT;
+  if (k3::make_layout(nullptr, n_segments, n_pct).total > k3::kStaticBytes) return DS_ELIMIT;   // (implied by the two tests above)
+  unsigned char* ws = k3::static_scratch();
+  if (!ws) return DS_ECUDA;
+  // ds_tail_stats clears the whole layout (cudaMemsetAsync on `stream`) before its first kernel, so what the previous
+  // call left in the shared array is never read. It launches kernels and memsets only: no cudaMalloc / cudaFree.
+  return ds_tail_stats(values, seg_id, n, n_segments, pct, n_pct, out, count_out, ws, k3::kStaticBytes, stream);
 }
