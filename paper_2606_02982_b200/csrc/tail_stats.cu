@@ -88,6 +88,7 @@ __device__ __forceinline__ void agg_add(unsigned int* bins, bool pred, unsigned 
   else if (pred && bin != lead_bin) atomicAdd(&bins[bin], 1u);
 }
 
+constexpr int kSparseLanes = 8;   // digit passes after the first: up to this many matching lanes add with plain shared-memory atomics
 constexpr int kMaxSegPct = 200;   // (segments x percentiles) of the fused pass: 200 KB of shared-memory histograms at most
 constexpr int kUnroll = 4;   // independent 12-byte loads in flight per thread
 
@@ -331,9 +332,19 @@ __global__ void __launch_bounds__(1024) lat_pass_kernel(const LatArgs a, int n_p
             if (!__any_sync(0xffffffffu, hit)) continue;
           }
           const unsigned mm = ok ? match32<NP>(pfx32_s, s_t, s_a, hi, n_pct) : 0u;
-          if (NP != 2 && !__any_sync(0xffffffffu, mm != 0u)) continue;
+          const unsigned hitm = __ballot_sync(0xffffffffu, mm != 0u);
+          if (hitm == 0u) continue;
           const unsigned dig = (kk[u] >> shift) & dmask;
-          for (int q = 0; q < n_pct; ++q) {
+          if (__popc(hitm) <= kSparseLanes) {   // few lanes match (the usual case after the first pass) and their digits are spread:
+            if (mm) {                           // those lanes add on their own; aggregating votes would cost every lane ~10 instructions per histogram
+              for (int q = 0; q < n_pct; ++q) {
+                if ((mm >> q) & 1u) atomicAdd(&sh[(s_t * n_pct + q) * 256 + dig], 1u);
+                if ((mm >> (8 + q)) & 1u) atomicAdd(&sh[(s_a * n_pct + q) * 256 + dig], 1u);
+              }
+            }
+            continue;
+          }
+          for (int q = 0; q < n_pct; ++q) {     // dense (e.g. many equal keys): warp-aggregated adds
             agg_add(sh, (mm >> q) & 1u, (s_t * n_pct + q) * 256 + dig);
             agg_add(sh, (mm >> (8 + q)) & 1u, (s_a * n_pct + q) * 256 + dig);
           }
@@ -394,7 +405,17 @@ __global__ void __launch_bounds__(1024) lat_pass_kernel(const LatArgs a, int n_p
             mm |= (ok && hi == pfx_s[s_t * n_pct + q]) ? (1u << q) : 0u;
             mm |= (ok && hi == pfx_s[s_a * n_pct + q]) ? (256u << q) : 0u;
           }
-          if (!__any_sync(0xffffffffu, mm != 0u)) continue;
+          const unsigned hitm = __ballot_sync(0xffffffffu, mm != 0u);
+          if (hitm == 0u) continue;
+          if (__popc(hitm) <= kSparseLanes) {   // see the staged loop
+            if (mm) {
+              for (int q = 0; q < n_pct; ++q) {
+                if ((mm >> q) & 1u) atomicAdd(&sh[(s_t * n_pct + q) * 256 + dig], 1u);
+                if ((mm >> (8 + q)) & 1u) atomicAdd(&sh[(s_a * n_pct + q) * 256 + dig], 1u);
+              }
+            }
+            continue;
+          }
           for (int q = 0; q < n_pct; ++q) {
             agg_add(sh, (mm >> q) & 1u, (s_t * n_pct + q) * 256 + dig);
             agg_add(sh, (mm >> (8 + q)) & 1u, (s_a * n_pct + q) * 256 + dig);
