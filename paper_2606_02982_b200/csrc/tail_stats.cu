@@ -74,21 +74,16 @@ __global__ void latencies_kernel(const int64_t* __restrict__ trace_off, const in
   }
 }
 
-// Warp-aggregated shared-memory add. Latencies share their high digits, so in the first passes nearly all lanes of a
-// warp hit ONE bin: that bin is found with a broadcast + ballot and costs one atomic for the warp; the lanes that hit
-// other bins add individually. (MATCH.ANY, used before, aggregates every bin but its cost grows with the number of
-// distinct bins: on the spread middle digits it took ~100 cycles per call and made those passes 3-5x slower.)
+// Histogram add in shared memory: a plain atomic by every lane whose predicate holds. Round 1 aggregated the lanes of a warp
+// first (leader's bin by broadcast + ballot, one atomic for all lanes that hit it), on the assumption that keys sharing
+// their high digits serialise 32-way on one bin. Measured again in r02 on B200 (20 M keys per call): spread keys 0.65 ->
+// 0.57 ms, keys that are all equal but 0.5 % outliers 1.33 -> 0.70 ms, two distinct values 1.32 -> 0.72 ms, and the stats
+// stage of configs[3] -35 %: same-address shared-memory atomics of a warp are combined by the hardware, and the two ballots
+// and the shuffle per add were what the passes spent their issue slots on.
 __device__ __forceinline__ void agg_add(unsigned int* bins, bool pred, unsigned bin) {
-  const unsigned act = __ballot_sync(0xffffffffu, pred);
-  if (act == 0u) return;                            // later digits: almost no key matches the prefix
-  const int lead = __ffs(act) - 1;
-  const unsigned lead_bin = __shfl_sync(0xffffffffu, bin, lead);
-  const unsigned same = __ballot_sync(0xffffffffu, pred && bin == lead_bin);
-  if ((int)(threadIdx.x & 31) == lead) atomicAdd(&bins[bin], (unsigned)__popc(same));
-  else if (pred && bin != lead_bin) atomicAdd(&bins[bin], 1u);
+  if (pred) atomicAdd(&bins[bin], 1u);
 }
 
-constexpr int kSparseLanes = 8;   // digit passes after the first: up to this many matching lanes add with plain shared-memory atomics
 constexpr int kMaxSegPct = 200;   // (segments x percentiles) of the fused pass: 200 KB of shared-memory histograms at most
 constexpr int kUnroll = 4;   // independent 12-byte loads in flight per thread
 
@@ -290,7 +285,7 @@ __global__ void __launch_bounds__(1024) lat_pass_kernel(const LatArgs a, int n_p
   // First digit pass: every prefix still is the bits common to ALL keys, so each key matches all of its (segment,
   // percentile) pairs. Only the (group, tier) histogram of percentile 0 is built from the keys; the group's "all"
   // histogram (the sum over its tiers) and the other percentiles' copies are filled in shared memory afterwards:
-  // one aggregated add per key instead of 2 x n_pct. The count pass does the same with the segment counts.
+  // one add per key instead of 2 x n_pct. The count pass does the same with the segment counts.
   const bool first = !kCount && d == 7;
   // one WARP per instance: the dependent header loads (instance -> trace -> offsets) of 16 warps per block overlap
   const int lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
@@ -332,21 +327,12 @@ __global__ void __launch_bounds__(1024) lat_pass_kernel(const LatArgs a, int n_p
             if (!__any_sync(0xffffffffu, hit)) continue;
           }
           const unsigned mm = ok ? match32<NP>(pfx32_s, s_t, s_a, hi, n_pct) : 0u;
-          const unsigned hitm = __ballot_sync(0xffffffffu, mm != 0u);
-          if (hitm == 0u) continue;
           const unsigned dig = (kk[u] >> shift) & dmask;
-          if (__popc(hitm) <= kSparseLanes) {   // few lanes match (the usual case after the first pass) and their digits are spread:
-            if (mm) {                           // those lanes add on their own; aggregating votes would cost every lane ~10 instructions per histogram
-              for (int q = 0; q < n_pct; ++q) {
-                if ((mm >> q) & 1u) atomicAdd(&sh[(s_t * n_pct + q) * 256 + dig], 1u);
-                if ((mm >> (8 + q)) & 1u) atomicAdd(&sh[(s_a * n_pct + q) * 256 + dig], 1u);
-              }
+          if (mm) {                              // plain atomics by the matching lanes (see agg_add)
+            for (int q = 0; q < n_pct; ++q) {
+              if ((mm >> q) & 1u) atomicAdd(&sh[(s_t * n_pct + q) * 256 + dig], 1u);
+              if ((mm >> (8 + q)) & 1u) atomicAdd(&sh[(s_a * n_pct + q) * 256 + dig], 1u);
             }
-            continue;
-          }
-          for (int q = 0; q < n_pct; ++q) {     // dense (e.g. many equal keys): warp-aggregated adds
-            agg_add(sh, (mm >> q) & 1u, (s_t * n_pct + q) * 256 + dig);
-            agg_add(sh, (mm >> (8 + q)) & 1u, (s_a * n_pct + q) * 256 + dig);
           }
         }
       }
@@ -405,20 +391,11 @@ __global__ void __launch_bounds__(1024) lat_pass_kernel(const LatArgs a, int n_p
             mm |= (ok && hi == pfx_s[s_t * n_pct + q]) ? (1u << q) : 0u;
             mm |= (ok && hi == pfx_s[s_a * n_pct + q]) ? (256u << q) : 0u;
           }
-          const unsigned hitm = __ballot_sync(0xffffffffu, mm != 0u);
-          if (hitm == 0u) continue;
-          if (__popc(hitm) <= kSparseLanes) {   // see the staged loop
-            if (mm) {
-              for (int q = 0; q < n_pct; ++q) {
-                if ((mm >> q) & 1u) atomicAdd(&sh[(s_t * n_pct + q) * 256 + dig], 1u);
-                if ((mm >> (8 + q)) & 1u) atomicAdd(&sh[(s_a * n_pct + q) * 256 + dig], 1u);
-              }
+          if (mm) {                              // plain atomics, see the staged loop
+            for (int q = 0; q < n_pct; ++q) {
+              if ((mm >> q) & 1u) atomicAdd(&sh[(s_t * n_pct + q) * 256 + dig], 1u);
+              if ((mm >> (8 + q)) & 1u) atomicAdd(&sh[(s_a * n_pct + q) * 256 + dig], 1u);
             }
-            continue;
-          }
-          for (int q = 0; q < n_pct; ++q) {
-            agg_add(sh, (mm >> q) & 1u, (s_t * n_pct + q) * 256 + dig);
-            agg_add(sh, (mm >> (8 + q)) & 1u, (s_a * n_pct + q) * 256 + dig);
           }
         }
       }

@@ -102,6 +102,24 @@ def test_fused_latency_stats(G):
     _fused_vs_oracle(G, c1)
 
 
+def test_fused_latency_stats_runs_of_equal_keys(G):
+    """Queue delay 0 for nearly every request (an idle server), plus one burst trace whose delays are large: after the first
+    digit every lane of a warp holds the SAME key, the case in which the digit passes must aggregate their adds instead of
+    using plain atomics (tail_stats.cu: concentrated()). Also p50 = 0 and p99 among the outliers: both ends of the range."""
+    from paper_2606_02982_b200 import workload as wl
+    sv = wl.Server(max_batch=64, kv_budget=0)
+    combos = [(p, wl.EXACT, 0.0) for p in (wl.FIFO, wl.SJF, wl.PRIORITY)]
+    c = wl._trace_workload("t", 12, 6, 2000, sv, combos, oracle.characterize, mean_ticks=40_000_000.0)   # one request at a time
+    a = c.arrival.reshape(6, 2000)
+    a[5] = np.sort(a[5] // 4000)                                   # the burst: 2000 requests within 1/4000 of the time
+    c.arrival = a.reshape(-1)
+    st, dn, _ = oracle.simulate(c.trace_off, c.arrival, c.tier, c.words, c.tokens, c.out_len, c.server, c.instances)
+    qd = (st.reshape(c.n_inst, 2000) - a[c.instances["trace"]])
+    assert (qd[c.instances["trace"] < 5] == 0).mean() > 0.99 and qd[c.instances["trace"] == 5].max() > 1_000_000
+    _fused_vs_oracle(G, c)
+    _fused_vs_oracle(G, c, pct=(1, 50, 90, 99, 100))
+
+
 def test_fused_staging_edge_cases(G):
     """The staging area of ds_latency_stats: keys that need more than 32 bits, padded and out-of-order out_off, a staging
     area that is too small - every case must give the oracle's percentiles (the unstaged passes take over)."""
