@@ -7,8 +7,9 @@
 //
 // Mapping to the warp (B200: 148 SMs, persistent warps pulling instances from an atomic counter). The per-instance
 // body is compiled once per (slots, policy) so that each policy's queue logic is straight-line code:
-//  - warp-uniform scalars: clock `now`, cursor `next`, next arrival tick `an`, batch size b, kv_used, B[3] (held by
-//    lanes 0..2);
+//  - warp-uniform scalars: clock `now`, cursor `next`, next arrival tick `an`, batch size b, kv_used; the factors B[3]
+//    and the arrival ticks of the current window sit in shared memory (every lane writes the same factor, so no
+//    synchronisation is needed to read it back; shuffles from an owner lane cost 27 instructions per request with their guards);
 //  - running set: 32*kSlots slots {request index, finishing iteration} in shared memory (max_batch <= 32*kSlots) with a
 //    free-slot stack beside them: an admission is one pop + two stores by uniform address (placing a request into one
 //    lane's register slots cost 35 instructions of divergent, predicated code per request). At a completion boundary
@@ -89,6 +90,15 @@ struct __align__(16) Slots {
   int idx[32 * kSlots];                       // request index, kFreeIdx = free
   unsigned fin[32 * kSlots];                  // iteration at whose boundary the request completes
   unsigned short stack[32 * kSlots];          // free slot numbers, [0, nfree) valid
+  // Warp-uniform values that used to be fetched from their owner lane by shuffles (27 instructions per request with the
+  // convergence guards around every SHFL). B: every lane writes the SAME new factor, so a lane only ever reads what it wrote
+  // itself and no synchronisation is needed. warr / west: lane l's arrival tick and frozen estimate of request wb + l, read
+  // by other lanes after a __syncwarp(). (The cursor policies keep their estimate shuffles: those run only when a queue head
+  // falls inside the ingested range, which is rare; an unconditional store per ingest step cost more: configs[4] +3 %.)
+  double B[4];                                // feedback factors: per tier (3) or per semantic category (4)
+  long long warr[32];                         // arrival ticks of the current 32-request window
+  long long west[32];                         // SJF: estimates of the current ingest step (every heap push ends in a __syncwarp, which
+                                              // orders its reads before the next step's writes)
 };
 
 // ---- SJF heap: implicit 32-ary min-heap, node i has children 32i+1 .. 32i+32 ----
@@ -206,7 +216,8 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   unsigned iter = 0, dist = 0xffffffffu;
   bool blocked = false;
   long long collect = -1;                // batch-wait: tick at which the idle dispatcher started collecting (-1: not collecting)
-  double Bl = 1.0;                       // lane t < 3 holds B[t]
+#pragma unroll
+  for (int k = 0; k < 4; ++k) sl.B[k] = 1.0;   // (every lane, same value)
   // running set: all slots free, the free stack holds every slot number
   int nfree = 32 * kSlots;
 #pragma unroll
@@ -235,7 +246,8 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
   // arrival window: lane holds request wb+lane
   int wb = 0; long long w_arr = kInf; int w_tier = 0, w_base = 0, w_cat = 0;
   auto load_window = [&]() {
-    const long long w_prev_last = wb > 0 ? shfl_i64(w_arr, 31) : 0;   // last arrival of the window being replaced (lane 0's predecessor)
+    const long long w_prev_last = wb > 0 ? sl.warr[31] : 0;   // last arrival of the window being replaced (lane 0's predecessor)
+    __syncwarp();                                              // ... read by every lane before lane 31 overwrites it
     const int i = wb + lane;
     if (i < n) { w_arr = arr_at(i); w_tier = tier[i]; w_base = BASE[i]; } else { w_arr = kInf; w_tier = 0; w_base = 0; }
     if (kBudget) {
@@ -248,9 +260,11 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
     if (bad) atomicOr(p.status, DS_DEV_BAD_TRACE);
     if (w_tier > 2) w_tier = 2;
     if (w_base < 0) w_base = 0;
+    sl.warr[lane] = w_arr;
+    __syncwarp();
   };
   load_window();
-  an = n > 0 ? shfl_i64(w_arr, 0) : kInf;
+  an = n > 0 ? sl.warr[0] : kInf;
 
   auto advance_cursor = [&](TierCursor& c, const int t, bool first) {   // move tier t's head to its next request
     if (!first) c.mask &= c.mask - 1;
@@ -292,14 +306,14 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
           const double sc = w_tier == 0 ? p.bp.s_tenant[0] : w_tier == 1 ? p.bp.s_tenant[1] : p.bp.s_tenant[2];
           double F = __dadd_rn(1.0, __dmul_rn(p.bp.f_slope, (double)w_base));
           if (F > p.bp.f_max) F = p.bp.f_max;
-          double x = __dmul_rn(tb, shfl_f64(Bl, w_cat));
+          double x = __dmul_rn(tb, sl.B[w_cat]);
           x = __dmul_rn(x, sc);
           x = __dmul_rn(x, F);
           est = (long long)w_base + (long long)ceil(x);
         }
       } else if (need_est) {
         if (ema_on) {                                         // Eq. 1-2 reduced (A1), frozen at arrival (A5)
-          const double Bt = shfl_f64(Bl, w_tier);
+          const double Bt = sl.B[w_tier];
           if (w_base > 0) est = (long long)ceil(__dmul_rn(Bt, (double)w_base));
         } else est = w_base;                                  // B == 1.0 exactly
       }
@@ -307,10 +321,12 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       if constexpr (kReest) {
       } else if (kPolicy == DS_SJF) {
         if (pred && est >= (1ll << 39)) atomicOr(p.status, DS_DEV_KEY_RANGE);
+        sl.west[lane] = est;
+        __syncwarp();
         unsigned mm = m;
         while (mm) {
           const int l = __ffs(mm) - 1; mm &= mm - 1;
-          const long long e = shfl_i64(est, l);
+          const long long e = sl.west[l];
           heap.push(((unsigned long long)e << 24) | (unsigned long long)(wb + l), lane);
         }
       } else {
@@ -324,7 +340,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
           for (int t = 0; t < 3; ++t) {
             if (tc[t].head >= next && tc[t].head < last) {   // warp-uniform
               if (use_kv) tc[t].est = shfl_i64(est, tc[t].head - wb);
-              if (kAging) tc[t].arr = shfl_i64(w_arr, tc[t].head - wb);
+              if (kAging) tc[t].arr = sl.warr[tc[t].head - wb];
             }
           }
         }
@@ -334,7 +350,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       if (next == wb + 32 && next < n) { wb += 32; load_window(); continue; }
       break;
     }
-    an = next < n ? shfl_i64(w_arr, next - wb) : kInf;
+    an = next < n ? sl.warr[next - wb] : kInf;
   };
 
   // 2. RETIRE: completions at `now`, ascending request index (R-ORD); then the distance to the next completion.
@@ -394,19 +410,17 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
           const double tb = cr == 0 ? p.bp.t_base[0] : cr == 1 ? p.bp.t_base[1] : cr == 2 ? p.bp.t_base[2] : p.bp.t_base[3];
           if (tb > 0.0) {
             const double m = __ddiv_rn((double)Or, tb);
-            const double t2 = __dmul_rn(t1, shfl_f64(Bl, cr));
+            const double t2 = __dmul_rn(t1, sl.B[cr]);
             const double t3 = __dmul_rn(alpha, m);
-            const double Bn = __dadd_rn(t2, t3);
-            if (lane == cr) Bl = Bn;
+            sl.B[cr] = __dadd_rn(t2, t3);                       // every lane: same address, same value
           }
         }
       } else if (ema_on) {                                    // Eq. 5-6 (A3): four separately rounded operations; m = P/W came
         const int tr = (int)(rr.O >> 30);                     // rounded from pack_kernel (the same correctly rounded division)
         if (rr.m >= 0.0) {                                    // words > 0
-          const double t2 = __dmul_rn(t1, shfl_f64(Bl, tr));
+          const double t2 = __dmul_rn(t1, sl.B[tr]);
           const double t3 = __dmul_rn(alpha, rr.m);
-          const double Bn = __dadd_rn(t2, t3);
-          if (lane == tr) Bl = Bn;
+          sl.B[tr] = __dadd_rn(t2, t3);                         // every lane: same address, same value
         }
       }
       ++done;
@@ -415,12 +429,12 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
         if (t_new < last_rel && lane == 0) atomicOr(p.status, DS_DEV_BAD_TRACE);   // a client's start tick lies after this release
         last_rel = t_new;
         if (lane == 0) __stcg(arr_d + released, t_new);
-        if (lane == released - wb) w_arr = t_new;             // (unsigned compare not needed: released >= next >= wb)
+        if (lane == released - wb) { w_arr = t_new; sl.warr[lane] = t_new; }   // (released >= next >= wb; read back after the __syncwarp below)
         if (released == next) an = t_new;
         ++released;
         __syncwarp();
       }
-      if (traj && done % p.traj_every == 0 && lane < kFac) traj[kFac * (done / p.traj_every - 1) + lane] = Bl;
+      if (traj && done % p.traj_every == 0 && lane < kFac) traj[kFac * (done / p.traj_every - 1) + lane] = sl.B[lane];
     }
     // distance to the next completion: the occupied slots that did not complete now
     unsigned d = 0xffffffffu;
@@ -453,8 +467,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       int qpos = 0;
       if constexpr (kReest) {
         if (qn > 0) {
-          // the factors as they are now, in every lane (Bl lives in lanes 0..2)
-          const double B0 = shfl_f64(Bl, 0), B1 = shfl_f64(Bl, 1), B2 = shfl_f64(Bl, 2);
+          const double B0 = sl.B[0], B1 = sl.B[1], B2 = sl.B[2];   // the factors as they are now
           auto est_now = [&](const int r, const int tr) -> long long {   // Eq. 1-2 reduced (A1) with the current factor (A16)
             const int base = max((int)BASE[r], 0);
             if (!ema_on) return base;                           // B == 1.0 exactly
@@ -654,7 +667,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       }
     }
   }
-  if (lane < kFac) p.ema_final[kFac * (size_t)inst_id + lane] = Bl;
+  if (lane < kFac) p.ema_final[kFac * (size_t)inst_id + lane] = sl.B[lane];
   __syncwarp();
 }
 
