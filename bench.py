@@ -169,6 +169,17 @@ def workload_config(n_traces, text_traces, c, note=None):
     return cfg
 
 
+def pin_workload(c):
+    """Move the per-step input arrays of a workload into pinned host memory ONCE and let the workload's numpy arrays be views
+    of it: the end-to-end leg then copies from these very buffers (Tensor.pin_memory() of an already pinned array is the
+    array itself), so a rank holds its 9.2 GB of inputs once instead of twice (8 ranks on one host: 75 GB, not 150 GB)."""
+    import torch
+    for f in ("text", "offsets", "arrival", "tier", "out_len", "words", "tokens"):
+        a = getattr(c, f)
+        if a is not None:
+            setattr(c, f, torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy())
+
+
 def max_over_ranks(ms, world, device):
     """Timing rule of the bench contract: the job's time is the slowest rank's (all_reduce MAX); identity at N=1."""
     import torch
@@ -247,6 +258,7 @@ def run_ours(args):
 
     # ---- setup (untimed): seeded inputs; W,P of the materialised text come from ds_characterize itself ----
     c = build_cfg3(args.traces, args.text_traces, rank_seed(rank), gpu_characterize_fn(dev))   # weak scaling: every rank its own traces
+    pin_workload(c)
     hp = HotPath(c, dev)
     n_sim = c.sim_requests
     text_bytes = int(c.text.size) if c.text is not None else 0
