@@ -67,7 +67,7 @@ extern "C" {
  * offsets [n_prompts+1]  device, 0 <= offsets[0], non-decreasing, offsets[n_prompts] <= n_bytes
  * words_out, tokens_out [n_prompts] device, overwritten.
  * workspace: ds_workspace_bytes(DS_WS_CHARACTERIZE, n_bytes, n_prompts).
- * Launches: 1 memset + 1 kernel. */
+ * Launches: 2 memsets (the two outputs) + 1 kernel. */
 int ds_characterize(const uint8_t* bytes, int64_t n_bytes, const int64_t* offsets, int64_t n_prompts,
                     int32_t* words_out, int32_t* tokens_out, void* workspace, size_t workspace_bytes, void* stream);
 

@@ -49,3 +49,15 @@ def test_no_oracle_in_product_path():
             if f.endswith((".py", ".cu", ".cuh", ".cpp", ".h")):
                 src = open(os.path.join(dp, f)).read()
                 assert "import oracle" not in src and "from oracle" not in src and "oracle/" not in src.replace("the oracle", ""), f
+
+
+def test_k2_instruction_capture_belongs_to_the_committed_kernel():
+    # bench.py prints roofline.frac only when profiles/r02_k2_counts.json.txt was captured from the simulate.cu in the tree
+    # (it compares sha256); a kernel edit without a new ncu capture must show up here, not as a silently withheld number
+    import hashlib
+    import json
+    cap = json.load(open(os.path.join(ROOT, "profiles", "r02_k2_counts.json.txt")))
+    src = open(os.path.join(ROOT, "paper_2606_02982_b200", "csrc", "simulate.cu"), "rb").read()
+    assert hashlib.sha256(src).hexdigest() == cap["simulate_cu_sha256"], "re-capture profiles/r02_k2_counts.json.txt (see its 'how')"
+    for k in ("slots1", "slots4", "slots8"):
+        assert cap[k]["inst_per_simreq"] > cap[k]["floor_inst_per_simreq"] > 0
