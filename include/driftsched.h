@@ -47,6 +47,7 @@ extern "C" {
 #define DS_DEV_BAD_TRACE 2u    /* ds_simulate: tier > 2, out_len < 1, words/tokens < 0 or arrivals decreasing */
 #define DS_DEV_KEY_RANGE 4u    /* ds_simulate: SJF key overflow (est >= 2^39 or trace longer than 2^24) */
 #define DS_DEV_BAD_INSTANCE 8u /* ds_simulate: instance field out of range; ds_estimation_error: group out of range */
+#define DS_DEV_INTERNAL 32u   /* ds_simulate built with -DDS_K2_CHECK only: an internal invariant of the kernel's bookkeeping failed */
 #define DS_DEV_BAD_OUT_OFF 16u /* ds_simulate: out_off[i] < 0 or out_off[i] + trace length > n_total (instance skipped) */
 
 /* ---------------------------------------------------------------------------------------------- (a)

@@ -45,6 +45,13 @@ constexpr int kWarpsPerBlock = 4;
                              // shared memory: 6 / 7 / 8 blocks = configs[3] at 4096 traces 384.0 / 381.3 / 396.8 ms, configs[1] 12.92 / 12.47 / 13.29 ms)
 #endif
 constexpr int kHeapSmem = 256;  // heap entries cached in shared memory per warp
+// Build with -DDS_K2_CHECK to verify the bookkeeping of the shared-memory structures on the device (compute-sanitizer is not
+// available on this pool): a violated invariant sets DS_DEV_INTERNAL in the status word. Off in the product build.
+#ifdef DS_K2_CHECK
+#define DS_K2_INVARIANT(cond) do { if (!(cond)) atomicOr(p.status, DS_DEV_INTERNAL); } while (0)
+#else
+#define DS_K2_INVARIANT(cond) do { } while (0)
+#endif
 constexpr long long kInf = 0x7fffffffffffffffLL;
 constexpr unsigned kFull = 0xffffffffu;
 
@@ -391,6 +398,7 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       // owner: free the slot in shared memory and push its number on the free stack (registers keep the loaded state: the
       // completions are told apart from what stays by rf == iter)
       const bool own = lm == r;
+      DS_K2_INVARIANT(nfree >= 0 && nfree < 32 * kSlots && __popc(__ballot_sync(kFull, own)) == 1 && r >= 0 && r < next);
       if (own) { const int slot = lane * kSlots + ls; sl.idx[slot] = kFreeIdx; sl.stack[nfree] = (unsigned short)slot; --cnt; lm = kFreeIdx; }
       ++nfree;
       if (kSlots > 1 && __any_sync(kFull, own && cnt > 0)) {  // rare: the owner holds another completion; its next candidate
@@ -586,7 +594,9 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
       const int Pc = rc.P;
       const int Oc = max((int)(rc.O & kRecLenMask), 1);        // (a bad out_len was reported when its window was loaded)
       st[c] = now;                                             // every lane, same address and value
+      DS_K2_INVARIANT(nfree >= 1 && nfree <= 32 * kSlots && c >= 0 && c < next);
       const int slot = sl.stack[--nfree];                      // b < max_batch <= 32*kSlots: a free slot exists
+      DS_K2_INVARIANT(slot >= 0 && slot < 32 * kSlots && sl.idx[slot] == kFreeIdx);
       sl.idx[slot] = c; sl.fin[slot] = iter + (unsigned)Oc;    // (uniform address and value)
       kv_used += (acc_t)Pc; prefill_new += (acc_t)Pc; ++b;
       dist = min(dist, (unsigned)Oc);
@@ -595,6 +605,10 @@ __device__ __forceinline__ void run_instance(const Params& p, const unsigned ins
 
   // ---- main loop: one pass per iteration boundary that has an event; event-free boundaries are jumped over ----
   for (;;) {
+    DS_K2_INVARIANT(b >= 0 && b <= max_batch && max_batch <= 32 * kSlots && nfree + b == 32 * kSlots);   // one slot per running request
+    DS_K2_INVARIANT(next >= 0 && next <= n && done >= 0 && done <= next && wb >= 0 && wb <= next && next - wb <= 32);
+    DS_K2_INVARIANT(kPolicy != DS_SJF || kReest || (heap.size >= 0 && heap.size <= next - done));
+    DS_K2_INVARIANT(!kReest || (qn >= 0 && qn <= next - done));
     // 1.-3. Two inlined copies of ingest() instead of one in a two-trip loop: the loop's carried state cost ~35 instructions
     // per request in register moves (measured: configs[3] -4.8 %, configs[1] -6.7 % simulate time).
     if (dist == 0) {
