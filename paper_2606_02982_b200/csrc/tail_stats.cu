@@ -80,7 +80,7 @@ __global__ void latencies_kernel(const int64_t* __restrict__ trace_off, const in
 // 0.57 ms, keys that are all equal but 0.5 % outliers 1.33 -> 0.70 ms, two distinct values 1.32 -> 0.72 ms, and the stats
 // stage of configs[3] -35 %: same-address shared-memory atomics of a warp are combined by the hardware, and the two ballots
 // and the shuffle per add were what the passes spent their issue slots on.
-__device__ __forceinline__ void agg_add(unsigned int* bins, bool pred, unsigned bin) {
+__device__ __forceinline__ void hist_add(unsigned int* bins, bool pred, unsigned bin) {
   if (pred) atomicAdd(&bins[bin], 1u);
 }
 
@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(512) count_kernel(const int64_t* __restrict__ 
     for (int u = 0; u < kUnroll; ++u) {
       const bool ok = sv[u] >= 0 && sv[u] < n_seg;
       if (ok) { a &= kv[u]; o |= kv[u]; any = true; }
-      if (priv) agg_add(sc, ok, (unsigned)sv[u]);
+      if (priv) hist_add(sc, ok, (unsigned)sv[u]);
       else if (ok) atomicAdd(&counts[sv[u]], 1ull);
     }
   }
@@ -160,7 +160,7 @@ __global__ void __launch_bounds__(512) hist_kernel(const int64_t* __restrict__ v
       const unsigned long long hi = hshift >= 64 ? 0ull : (kv[u] >> hshift);
       const unsigned dig = (unsigned)(kv[u] >> shift) & dmask;
       for (int q = 0; q < n_pct; ++q)
-        agg_add(bins, ok && hi == prefix[s * n_pct + q], (unsigned)((s * n_pct + q) * 256) + dig);
+        hist_add(bins, ok && hi == prefix[s * n_pct + q], (unsigned)((s * n_pct + q) * 256) + dig);
     }
   }
   if (kPriv) { __syncthreads(); for (int i = threadIdx.x; i < nb; i += blockDim.x) if (sh[i]) atomicAdd(&hist[i], sh[i]); }
@@ -316,7 +316,7 @@ __global__ void __launch_bounds__(1024) lat_pass_kernel(const LatArgs a, int n_p
           const bool ok = cc[u] != 255u;
           const unsigned s_t = ok ? cc[u] : 0u;
           if (kFirst) {    // every key matches every prefix of its segments: one add, the other histograms follow from it
-            agg_add(sh, ok, (s_t * n_pct) * 256 + ((kk[u] >> shift) & dmask));
+            hist_add(sh, ok, (s_t * n_pct) * 256 + ((kk[u] >> shift) & dmask));
             continue;
           }
           const unsigned hi = __funnelshift_r(kk[u], 0u, hshift);                     // kk >> hshift, 0 when hshift = 32
@@ -328,7 +328,7 @@ __global__ void __launch_bounds__(1024) lat_pass_kernel(const LatArgs a, int n_p
           }
           const unsigned mm = ok ? match32<NP>(pfx32_s, s_t, s_a, hi, n_pct) : 0u;
           const unsigned dig = (kk[u] >> shift) & dmask;
-          if (mm) {                              // plain atomics by the matching lanes (see agg_add)
+          if (mm) {                              // plain atomics by the matching lanes (see hist_add)
             for (int q = 0; q < n_pct; ++q) {
               if ((mm >> q) & 1u) atomicAdd(&sh[(s_t * n_pct + q) * 256 + dig], 1u);
               if ((mm >> (8 + q)) & 1u) atomicAdd(&sh[(s_a * n_pct + q) * 256 + dig], 1u);
@@ -377,13 +377,13 @@ __global__ void __launch_bounds__(1024) lat_pass_kernel(const LatArgs a, int n_p
         const unsigned s_t = (unsigned)(3 * g + (ok ? tr[u] : 0)), s_a = (unsigned)(3 * a.n_groups + g);
         if (kCount) {
           if (ok) { kand &= k; kor |= k; any = true; }
-          agg_add(sh, ok, s_t);                   // (s_a's count is the sum over the group's tiers: added after the loop)
+          hist_add(sh, ok, s_t);                   // (s_a's count is the sum over the group's tiers: added after the loop)
           const long long r = base + u * 32 + lane;
           if (stage && r < n) { a.skey[oo + r] = (unsigned)k; a.scode[oo + r] = ok ? (unsigned char)s_t : (unsigned char)255; }
         } else {
           const unsigned long long hi = hshift >= 64 ? 0ull : (k >> hshift);
           const unsigned dig = (unsigned)(k >> shift) & dmask;
-          if (first) { agg_add(sh, ok, (s_t * n_pct) * 256 + dig); continue; }
+          if (first) { hist_add(sh, ok, (s_t * n_pct) * 256 + dig); continue; }
           // which of the key's (segment, percentile) prefixes it matches: bit q = tier segment, bit 8+q = "all" segment.
           // After the first pass almost no key matches anything: one vote rejects the whole warp.
           unsigned mm = 0;
