@@ -293,7 +293,7 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
   // shared-window addresses of the stages and their barriers, computed once (the generic->shared conversion per use costs
   // a dozen instructions in the loop)
   const uint32_t stage_a0 = smem_u32(stage[0]), mbar_a0 = smem_u32(&mbar[0]);
-  auto issue = [&](unsigned it, int s) {  // lane 0 only
+  auto issue = [&](unsigned it, int s) {  // one lane only
     if (it < it_tma) {
       const uint32_t bar = mbar_a0 + 8u * (unsigned)s, dst = stage_a0 + (unsigned)kChunk * (unsigned)s;
       asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"((unsigned)kChunk) : "memory");
@@ -440,7 +440,13 @@ characterize_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t* __r
 
     // the stage's bytes are all in registers now: refill it with the chunk kStages ahead
     __syncwarp();
-    if (lane == 0 && it + kStages < it_tma) issue(it + kStages, s);
+    // One lane chosen by elect.sync issues the refill. With a `lane == 0` test the compiler wraps the (uniform-datapath) TMA
+    // instruction in a vote-and-retry loop, 15 instructions per chunk; an elected lane needs none.
+    if (it + kStages < it_tma) {
+      unsigned elected;
+      asm volatile("{\n.reg .pred p;\nelect.sync _|p, 0xffffffff;\nselp.u32 %0, 1, 0, p;\n}" : "=r"(elected));
+      if (elected) issue(it + kStages, s);
+    }
     const uint4 S4 = reinterpret_cast<const uint4*>(sb)[h * 32 + lane];
     reinterpret_cast<uint4*>(sb)[h * 32 + lane] = make_uint4(0u, 0u, 0u, 0u);
     const uint32_t S[NW] = {S4.x, S4.y, S4.z, S4.w};
