@@ -10,6 +10,12 @@
 // brute force; the absolute latencies of the synthetic server model are this build's reading of
 // BASELINE.json:configs[0] (DESIGN.md §4 A6-A10): "parity unpinned" beyond those pins.
 // tail_stats — pinned (hand values, numpy partition).
+// simulate_budget / simulate_closed (Eq. 1-2 in full, closed loop, batch wait) — pinned (tests/test_oracle_simulate_budget.py,
+// tests/test_oracle_simulate_closed.py: hand traces, order-statistics identity of the releases, conservation, gate property).
+// reestimate mode (reading A16) — pinned (tests/test_oracle_reestimate.py: hand traces H11/H12, reductions to the frozen run).
+// estimation_error, queue_depth, latencies incl. their arrival_override form — pinned (tests/test_oracle_estimation_error.py,
+// tests/test_oracle_queue_depth.py, tests/test_oracle_closed_loop_reporting.py: Eq. 4 thresholds, numpy one-liners, hand-worked
+// closed-loop trace, queue-wait conservation, discrete Little's law). No function of this file is "parity unpinned".
 #include "oracle.h"
 
 #include <algorithm>
