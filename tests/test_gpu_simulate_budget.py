@@ -175,6 +175,21 @@ def test_closed_loop(G, n_clients, think, max_batch, kv):
     assert np.array_equal(traj.cpu().numpy().view(np.uint64), otraj.view(np.uint64))
 
 
+def test_order_of_the_three_products_of_eq2(G):
+    # reading B3: ((T_base * B) * S_tenant) * F_input, each product rounded; parameters for which the swapped order lands on
+    # the other side of an integer (expected values derived by exact rationals in tests/test_oracle_simulate_budget.py)
+    import paper_2606_02982_b200 as ds
+    for t_base, s_ten, f_in, expect in ((75.0, 1.1, 1.2, 99), (200.0, 1.25, 1.1, 275), (189.0, 0.8, 1.25, 190)):
+        bp = wl.Budget(t_base=(t_base, 1.0, 1.0, 1.0), s_tenant=(s_ten, 1.0, 1.0), f_slope=1.0, f_max=f_in)
+        c = G.tiny_workload(wl, [[0, 0, 7, 9, 1]], wl.Server(max_batch=1, kv_budget=0), [(wl.FIFO, wl.BUDGET_SPLIT, 0.0), (wl.FIFO, wl.BUDGET_EXACT, 0.0)])
+        d = G.upload(c)
+        est = torch.full((2,), -1, dtype=torch.int64, device=G.DEV)
+        ds.simulate_budget(d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"], torch.zeros(1, dtype=torch.uint8, device=G.DEV),
+                           bp, c.server, d["inst"], d["out_off"], 2, est_out=est)
+        assert ds.device_status() == 0
+        assert est.tolist() == [7 + expect, 9 + expect], (t_base, s_ten, f_in)
+
+
 def test_closed_loop_hand_trace_and_contract(G):
     import paper_2606_02982_b200 as ds
     req = [[0, 1, 1, 9, 1], [0, 1, 1, 5, 1], [0, 1, 1, 3, 1], [0, 1, 1, 1, 1]]

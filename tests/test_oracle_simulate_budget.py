@@ -146,3 +146,29 @@ def test_contract_violations():
         _run(req, [0], wl.Budget(s_tenant=(1.0, 0.0, 1.0)), server(), [(wl.FIFO, wl.BUDGET_EXACT, 0.0)])
     with pytest.raises(ValueError):
         _run(req, [0], wl.Budget(f_max=0.5), server(), [(wl.FIFO, wl.BUDGET_EXACT, 0.0)])
+
+
+def test_order_of_the_three_products_of_eq2():
+    # Reading B3: T_budget = T_input + ceil(((T_base * B) * S_tenant) * F_input), each product rounded to fp64 in that
+    # order. Products of doubles do not associate, so the order is part of the definition. Parameters chosen (by a search over
+    # two-digit decimals) so that the prescribed order and the swapped one, ((T_base * B) * F_input) * S_tenant, land on different
+    # sides of an integer. Expected values: exact rational arithmetic with a correct rounding to the nearest double after every
+    # product (float(Fraction) rounds correctly), i.e. IEEE-754 applied by hand, not this formula in floating point.
+    from fractions import Fraction as Fr
+    import math
+
+    def rounded_product_chain(*factors):
+        x = Fr(factors[0])
+        for f in factors[1:]:
+            x = Fr(float(x * Fr(f)))
+        return x
+
+    for t_base, s_ten, f_in, expect, swapped in ((75.0, 1.1, 1.2, 99, 100), (200.0, 1.25, 1.1, 275, 276), (189.0, 0.8, 1.25, 190, 189)):
+        assert math.ceil(rounded_product_chain(t_base, 1.0, s_ten, f_in)) == expect          # the prescribed order, by hand
+        assert math.ceil(rounded_product_chain(t_base, 1.0, f_in, s_ten)) == swapped         # the other order differs: the case discriminates
+        # F_input = min(f_max, 1 + f_slope * T_input) = f_max exactly once 1 + T_input >= f_max; alpha = 0 keeps B = 1.0
+        bp = wl.Budget(t_base=(t_base, 1.0, 1.0, 1.0), s_tenant=(s_ten, 1.0, 1.0), f_slope=1.0, f_max=f_in)
+        req = [[0, 0, 7, 9, 1]]                                           # tier 0 (-> s_ten), words 7, tokens 9
+        for estimator, t_input in ((wl.BUDGET_SPLIT, 7), (wl.BUDGET_EXACT, 9)):
+            out = _run(req, np.zeros(1, np.uint8), bp, server(), [(wl.FIFO, estimator, 0.0)])
+            assert out[-1].tolist() == [t_input + expect], (t_base, s_ten, f_in, estimator)
