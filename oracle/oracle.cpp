@@ -87,17 +87,8 @@ struct Sim {
   // arrival (A5) but recomputed from the factors current at every scheduling decision; est[r] ends as the value in force
   // when r was admitted to the batch.
   bool reest() const { return sv->reestimate != 0; }
-  int64_t estimate_now(int64_t r) const {
+  int64_t estimate_now(int64_t r) const {          // reduced estimator (A1) only: re-estimation is not defined for the budget estimators
     int64_t b = base(r);
-    if (budget()) {
-      int c = cat[r];
-      double F = 1.0 + bp->f_slope * (double)b;
-      if (F > bp->f_max) F = bp->f_max;
-      double x = bp->t_base[c] * B[c];
-      x = x * bp->s_tenant[tier[r]];
-      x = x * F;
-      return b + (int64_t)std::ceil(x);
-    }
     return b > 0 ? (int64_t)std::ceil(B[tier[r]] * (double)b) : 0;
   }
   int64_t queued_est(int64_t r) const { return reest() ? estimate_now(r) : est[r]; }
@@ -198,6 +189,7 @@ static int simulate_impl(const oracle_traces* tr, const uint8_t* category, const
   if (sv->weight[0] < 1 || sv->weight[1] < 1 || sv->weight[2] < 1) return -1;
   if (sv->aging_step < 1) return -1;
   if (sv->reestimate != 0 && sv->reestimate != 1) return -1;
+  if (sv->reestimate && bp) return -1;   // A16 is a reading for ds_simulate / ds_simulate_est only (the library returns DS_EINVAL)
   for (int64_t ii = 0; ii < n_inst; ++ii) {
     const oracle_instance& in = inst[ii];
     if (in.trace < 0 || in.trace >= tr->n_traces || in.policy < 0 || in.policy > AGING_UNCLAMPED || !(in.ema_alpha >= 0.0 && in.ema_alpha <= 1.0))

@@ -92,3 +92,20 @@ def test_feedback_lowers_estimation_error_like_tables_iv_x():
     assert 1.30 < bias[0] < 1.50                                   # closed form 1.3977 (SURVEY.md §8(c) C.1 pin 3)
     assert abs(bias[1] - 1.0) < 0.03                               # Table IV: mean bias 0.999 with feedback on
     assert mae[2] == 0 and mae[3] == 0 and bias[2] == 1.0 and bias[3] == 1.0   # tokenizer-aware: nothing to correct
+
+
+def test_budget_estimators_are_scored_against_input_plus_output_tokens():
+    # Eq. 1 predicts T_input + the output budget, so for the DS_BUDGET_* estimators the observed length is tokens + out_len
+    # (driftsched.h); the sums are numpy one-liners over the oracle's own estimates
+    sv = wl.Server(max_batch=8, kv_budget=3000)
+    c = wl._trace_workload("t", 19, 2, 300, sv, [(wl.FIFO, wl.BUDGET_SPLIT, 0.1), (wl.SJF, wl.BUDGET_EXACT, 0.1)], oracle.characterize, rho=0.9)
+    cat, out_len = wl.assign_categories(19, c.out_len)
+    tr = (c.trace_off, c.arrival, c.tier, c.words, c.tokens, out_len)
+    st, dn, ema, est = oracle.simulate_budget(*tr, cat, wl.Budget(), sv, c.instances, want_est=True)
+    sums = oracle.estimation_error(*tr, c.instances, c.out_off, est, st, c.group, c.n_groups)
+    obs = (c.tokens.astype(np.int64) + out_len.astype(np.int64)).reshape(c.n_traces, c.n_req)[c.instances["trace"]].reshape(-1)
+    for g in range(c.n_groups):
+        sel = np.repeat(c.group == g, c.n_req)
+        err = est[sel] - obs[sel]
+        assert sums[g, :5].tolist() == [int(sel.sum()), int(np.abs(err).sum()), int((err * err).sum()), int(est[sel].sum()), int(obs[sel].sum())]
+    assert (sums[:, 4] > c.tokens.sum() // 2).all()                    # the output tokens are in the observed length

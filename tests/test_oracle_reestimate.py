@@ -85,3 +85,12 @@ def test_dispatch_time_estimates_track_a_drift_better():
 def test_contract():
     with pytest.raises(ValueError):
         run_oracle([[0, 0, 1, 1, 1]], server(reestimate=2), wl.FIFO)
+
+
+def test_not_defined_for_the_budget_estimators():
+    # A16 is a reading for the reduced estimator; with the full Eq. 1-2 estimator the oracle refuses (as the library does: DS_EINVAL)
+    req = np.asarray([[0, 1, 4, 2, 1]], np.int64)
+    inst = np.zeros(1, wl.INSTANCE_DTYPE); inst[0] = (0, wl.FIFO, wl.BUDGET_SPLIT, 0, 0.1)
+    tr = ([0, 1], req[:, 0], req[:, 1], req[:, 2], req[:, 3], req[:, 4])
+    with pytest.raises(ValueError):
+        oracle.simulate_budget(*tr, np.zeros(1, np.uint8), wl.Budget(), server(reestimate=1), inst)

@@ -43,3 +43,13 @@ def test_latencies_definition():
     a = np.tile(cfg.arrival, 2)
     assert np.array_equal(e2e, dn - a) and np.array_equal(qd, st - a)
     assert np.array_equal(seg_a, np.repeat([0, 1], 200)) and np.array_equal(seg_t, seg_a * 3 + np.tile(cfg.tier, 2))
+
+
+def test_segment_ids_outside_the_range_are_skipped():
+    # SURVEY.md §8(c) C.3 / driftsched.h: seg_id outside [0, n_segments) is skipped, negative or too large alike (by hand)
+    vals = np.array([5, 1, 9, 3, 100, 200, 7], np.int64)
+    seg = np.array([0, 0, 0, 0, -1, 2, 1], np.int32)          # 200 has id 2 = n_segments: not segment 0 (2 % 2), not counted at all
+    out, cnt = oracle.tail_stats(vals, seg, 2, (50, 99))
+    assert out.tolist() == [[3, 9], [7, 7]] and cnt.tolist() == [4, 1]
+    out, cnt = oracle.tail_stats(vals, np.full(7, 9, np.int32), 2, (50,))
+    assert out.tolist() == [[-1], [-1]] and cnt.tolist() == [0, 0]
