@@ -6,7 +6,7 @@
 //
 // Pin status (tests/test_oracle_*.py): characterize — pinned (Python bytes.split(), independent
 // per-byte reference, closed-form token/word ratio, hand cases). simulate — pinned to the hand-worked
-// traces H1-H10 (H7-H10: R-ORD, A8 blocking, A8 progress, KV release), closed forms (service time, M/M/1, M/D/1, EMA geometric form), invariants I1-I9 (I2/A8 reconstructed from outputs) and
+// traces H1-H14 (H7-H10: R-ORD, A8 blocking, A8 progress, KV release; H11/H12: A16; H13: A9 wrap; H14: R-ORD completion order), closed forms (service time, M/M/1, M/D/1, EMA geometric form), invariants I1-I9 (I2/A8 reconstructed from outputs) and
 // brute force; the absolute latencies of the synthetic server model are this build's reading of
 // BASELINE.json:configs[0] (DESIGN.md §4 A6-A10): "parity unpinned" beyond those pins.
 // tail_stats — pinned (hand values, numpy partition).

@@ -38,6 +38,8 @@ def test_hand_traces(G, golden_dir):
         c = G.tiny_workload(wl, case["req"], sv, [(case["policy"], case["estimator"], case["alpha"])])
         st, dn, ema = G.gpu_simulate(c)
         assert st.tolist() == case["start"] and dn.tolist() == case["done"], case["name"]
+        if "ema" in case:                                   # H14: completions at one tick applied in ascending request index
+            assert ema[0].tolist() == case["ema"], case["name"]
         if "est" in case:                                   # frozen admission-time estimates (H7: R-ORD) through ds_simulate_est
             import paper_2606_02982_b200 as ds
             d = G.upload(c)

@@ -190,6 +190,20 @@ def test_order_of_the_three_products_of_eq2(G):
         assert est.tolist() == [7 + expect, 9 + expect], (t_base, s_ten, f_in)
 
 
+def test_the_factor_of_eq2_is_the_categorys_not_the_tiers(G):
+    # reading B4 ("one factor per workload category"); hand derivation in tests/test_oracle_simulate_budget.py
+    import paper_2606_02982_b200 as ds
+    bp = wl.Budget(t_base=(100.0, 100.0, 100.0, 100.0), s_tenant=(1.0, 1.0, 1.0), f_slope=0.0, f_max=1.0)
+    req = [[0, 2, 5, 5, 50], [50_000_000, 2, 5, 5, 1], [60_000_000, 0, 5, 5, 1]]
+    c = G.tiny_workload(wl, req, wl.Server(max_batch=1, kv_budget=0), [(wl.FIFO, wl.BUDGET_SPLIT, 0.5)])
+    d = G.upload(c)
+    est = torch.full((3,), -1, dtype=torch.int64, device=G.DEV)
+    ds.simulate_budget(d["trace_off"], d["arrival"], d["tier"], d["words"], d["tokens"], d["out_len"],
+                       torch.tensor([0, 0, 2], dtype=torch.uint8, device=G.DEV), bp, c.server, d["inst"], d["out_off"], 3, est_out=est)
+    assert ds.device_status() == 0
+    assert est.tolist() == [105, 80, 105]
+
+
 def test_closed_loop_hand_trace_and_contract(G):
     import paper_2606_02982_b200 as ds
     req = [[0, 1, 1, 9, 1], [0, 1, 1, 5, 1], [0, 1, 1, 3, 1], [0, 1, 1, 1, 1]]

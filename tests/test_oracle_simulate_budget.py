@@ -172,3 +172,14 @@ def test_order_of_the_three_products_of_eq2():
         for estimator, t_input in ((wl.BUDGET_SPLIT, 7), (wl.BUDGET_EXACT, 9)):
             out = _run(req, np.zeros(1, np.uint8), bp, server(), [(wl.FIFO, estimator, 0.0)])
             assert out[-1].tolist() == [t_input + expect], (t_base, s_ten, f_in, estimator)
+
+
+def test_the_factor_of_eq2_is_the_categorys_not_the_tiers():
+    # PAPER.md:276 "one factor per workload category" (reading B4). alpha = 0.5, t_base = 100 for every category.
+    # r0 (Batch = tier 2, category 0, O 50) completes first: B[category 0] = 0.5 * 1 + 0.5 * (50 / 100) = 0.75, the others stay 1.
+    # r1 arrives long after: tier 2, category 0 -> T_budget = 5 + ceil(100 * 0.75) = 80 (with the tier's factor B[2] = 1: 105).
+    # r2: tier 0, category 2 -> 5 + ceil(100 * 1.0) = 105 (with the tier's factor B[0] = 0.75: 80).
+    bp = wl.Budget(t_base=(100.0, 100.0, 100.0, 100.0), s_tenant=(1.0, 1.0, 1.0), f_slope=0.0, f_max=1.0)
+    req = [[0, 2, 5, 5, 50], [50_000_000, 2, 5, 5, 1], [60_000_000, 0, 5, 5, 1]]
+    out = _run(req, np.array([0, 0, 2], np.uint8), bp, server(), [(wl.FIFO, wl.BUDGET_SPLIT, 0.5)])
+    assert out[-1].tolist() == [105, 80, 105]

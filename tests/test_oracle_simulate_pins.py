@@ -20,7 +20,7 @@ def _golden(golden_dir):
 
 def test_hand_traces(golden_dir):
     g = _golden(golden_dir)
-    assert len(g["cases"]) == 19
+    assert len(g["cases"]) == 21
     for c in g["cases"]:
         sv = server(**c["server"])
         if "weight" in c["server"]:
@@ -30,6 +30,8 @@ def test_hand_traces(golden_dir):
         assert dn.tolist() == c["done"], c["name"]
         if "est" in c:
             assert est.tolist() == c["est"], c["name"]
+        if "ema" in c:
+            assert ema[0].tolist() == c["ema"], c["name"]
 
 
 def test_h7_factor_after_same_tick_completion():
@@ -172,3 +174,37 @@ def test_ema_converges_to_token_word_ratio():
     assert traj.shape == (4000, 3)
     assert np.abs(traj[1000:].mean(axis=0) - 1.3977).max() < 0.02
     assert np.abs(ema[0] - 1.3977).max() < 0.08
+
+
+def test_h13_weighted_cursor_wraps_after_the_last_slot():
+    # H13 (A9; derivation in DESIGN.md §4.4). Weights 4:2:1 = slots PPPPSSB, max_batch 1, all O = 1, P = 1: S = 2150 + 6 = 2156.
+    # t=0: only r0 (Batch) is queued, cur = 0: slots 0-5 (P, S) are empty, slot 6 serves r0 and the cursor wraps to 0.
+    # r1..r4 Premium, r5 Standard, r6 Premium arrive while r0 runs. From cur = 0: four Premium slots -> r1, r2, r3, r4; slot 4 is
+    # a Standard slot -> r5; slot 5: Standard and Batch empty, wrap to slot 0 -> r6. A scan that never reaches the last slot
+    # serves r0 by accident but leaves cur = 1: then only three Premium slots remain and r5 overtakes r4.
+    req = [[0, 2, 1, 1, 1], [10, 0, 1, 1, 1], [20, 0, 1, 1, 1], [30, 0, 1, 1, 1], [40, 0, 1, 1, 1], [50, 1, 1, 1, 1], [60, 0, 1, 1, 1]]
+    st, dn, _ = run_oracle(req, server(weight=(4, 2, 1)), wl.WEIGHTED)
+    assert st.tolist() == [0, 2156, 4312, 6468, 8624, 10780, 12936]
+    assert dn.tolist() == [2156, 4312, 6468, 8624, 10780, 12936, 15092]
+
+
+def test_h14_completions_at_one_tick_update_the_factor_in_ascending_index():
+    # H14 (R-ORD: "multiple completions at one tick: ascending request index"; derivation in DESIGN.md §4.4). max_batch 2, FIFO, SPLIT,
+    # alpha = 0.5. r0 = (0, Std, W 4, P 2, O 1) and r1 = (0, Std, W 2, P 3, O 1) are admitted together and both complete at
+    # 2000 + 300 + 5 + 25 = 2330. r0 first: m = 0.5 -> B = 0.5 + 0.25 = 0.75; then r1: m = 1.5 -> B = 0.375 + 0.75 = 1.125.
+    # (The other order gives 1.25, then 0.875.) All values are exact in binary.
+    req = [[0, 1, 4, 2, 1], [0, 1, 2, 3, 1]]
+    st, dn, ema, traj = run_oracle(req, server(max_batch=2, traj_every=1), wl.FIFO, wl.SPLIT, 0.5, want_traj=True)
+    assert st.tolist() == [0, 0] and dn.tolist() == [2330, 2330]
+    assert traj.tolist() == [[1.0, 0.75, 1.0], [1.0, 1.125, 1.0]] and ema[0].tolist() == [1.0, 1.125, 1.0]
+
+
+def test_trajectory_stride():
+    # traj_every = 3: sample j holds the factors after 3 (j + 1) completions; constant ratio m = 1.5 -> closed form (iv)
+    k = 10
+    req = [[i * 10_000_000, 1, 4, 6, 1] for i in range(k)]
+    st, dn, ema, traj = run_oracle(req, server(traj_every=3), wl.FIFO, wl.SPLIT, 0.1, want_traj=True)
+    assert traj.shape == (3, 3)                                    # floor(10 / 3) samples
+    for j in range(3):
+        expect = 1.5 + (1 - 1.5) * 0.9 ** (3 * (j + 1))
+        assert abs(traj[j, 1] / expect - 1) < 1e-14 and traj[j, 0] == 1.0 and traj[j, 2] == 1.0

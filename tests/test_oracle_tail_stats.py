@@ -53,3 +53,9 @@ def test_segment_ids_outside_the_range_are_skipped():
     assert out.tolist() == [[3, 9], [7, 7]] and cnt.tolist() == [4, 1]
     out, cnt = oracle.tail_stats(vals, np.full(7, 9, np.int32), 2, (50,))
     assert out.tolist() == [[-1], [-1]] and cnt.tolist() == [0, 0]
+
+
+def test_percentile_0_and_100_are_the_extremes():
+    # nearest rank (A13): rank = max(1, ceil(p n / 100)): p = 0 -> the smallest element, p = 100 -> the largest (by hand)
+    out, cnt = oracle.tail_stats(np.array([5, 1, 9, 3], np.int64), np.zeros(4, np.int32), 1, (0, 100))
+    assert out.tolist() == [[1, 9]] and cnt.tolist() == [4]
