@@ -139,3 +139,55 @@ def one_case(seed):
             assert nm == "traj" and (b is None or np.asarray(b).size == 0), desc
             continue
         _same(nm, a, b, desc)
+
+
+def one_case_k1(seed):
+    """ds_characterize on a random buffer: alphabet, size, prompt cuts (empty prompts, bytes outside every prompt) and base
+    misalignment all drawn from the seed."""
+    rng = np.random.default_rng([seed, 1])
+    alphabets = (b" \t\n\r\x0b\x0c\x08\x0e\x1c\x1f\x7f\x80\x85\xa0\xff!/:@[`{~09AZaz_\x00,.", b"  ab", b"a", b" ", b"a,. \n",
+                 bytes(range(256)), b"abcdefghijklmnopqrstuvwxyz      .,;")
+    alpha = np.frombuffer(alphabets[int(rng.integers(0, len(alphabets)))], np.uint8)
+    n = int(rng.choice([0, 1, 7, 4095, 4096, 4097, 8192, 12289, 50_000, 300_001, int(rng.integers(1, 400_000))]))
+    mis = int(rng.choice([0, 0, 1, 5, 8, 15]))
+    big = alpha[rng.integers(0, len(alpha), n + mis)] if rng.random() < 0.7 else np.repeat(
+        alpha[rng.integers(0, len(alpha), (n + mis) // 37 + 1)], 37)[:n + mis]          # long runs of one byte
+    buf = big[mis:mis + n]
+    k = int(rng.choice([0, 1, 3, 50, max(1, n // 3), max(1, n)]))
+    cuts = np.sort(rng.integers(0, n + 1, k)).astype(np.int64)
+    lo, hi = (0, n) if rng.random() < 0.7 or k == 0 else (int(cuts[0]), int(cuts[-1]))
+    off = np.concatenate([[lo], cuts, [hi]]).astype(np.int64)
+    ow, ot = oracle.characterize(buf, off)
+    t = torch.from_numpy(np.ascontiguousarray(big)).to(DEV)
+    w, tk = ds.characterize(t[mis:mis + n], torch.from_numpy(off).to(DEV))
+    assert ds.device_status() == 0, (seed, n, mis, k)
+    assert np.array_equal(w.cpu().numpy(), ow) and np.array_equal(tk.cpu().numpy(), ot), (seed, n, mis, k)
+
+
+def one_case_k3(seed):
+    """ds_tail_stats (and the static entry point when the sizes fit) on random values / segments / percentiles."""
+    rng = np.random.default_rng([seed, 3])
+    n = int(rng.choice([0, 1, 2, 33, 1000, 70_000, int(rng.integers(1, 300_000))]))
+    nseg = int(rng.choice([1, 2, 3, 16, 60, 128, 1000]))
+    mode = int(rng.integers(0, 6))
+    if mode == 0:   v = rng.integers(-10, 10, n)
+    elif mode == 1: v = rng.integers(0, 1 << 25, n)
+    elif mode == 2: v = (rng.pareto(1.2, n) * 1e4).astype(np.int64)
+    elif mode == 3: v = rng.integers(np.iinfo(np.int64).min, np.iinfo(np.int64).max, n, dtype=np.int64, endpoint=True)
+    elif mode == 4: v = np.full(n, int(rng.integers(-5, 5)) << int(rng.integers(0, 60)))
+    else:           v = (1 << 40) + rng.integers(0, 3, n) * (1 << int(rng.integers(0, 30)))
+    v = np.asarray(v, np.int64)
+    seg = (rng.integers(0, nseg, n) if rng.random() < 0.6 else np.minimum(rng.geometric(0.3, n) - 1, nseg - 1)).astype(np.int32)
+    if n:
+        seg[rng.random(n) < rng.choice([0.0, 0.05, 0.9])] = int(rng.choice([-1, nseg, nseg + 7]))   # skipped values
+    pct = tuple(int(x) for x in rng.choice([0, 1, 25, 50, 90, 95, 99, 100], int(rng.integers(1, 9)), replace=True))
+    o, oc = oracle.tail_stats(v, seg, nseg, pct)
+    dv, dseg = torch.from_numpy(v).to(DEV), torch.from_numpy(seg).to(DEV)
+    g, gc = ds.tail_stats(dv, dseg, nseg, pct)
+    assert ds.device_status() == 0
+    assert np.array_equal(g.cpu().numpy(), o) and np.array_equal(gc.cpu().numpy(), oc), (seed, n, nseg, mode, pct)
+    if nseg * len(pct) <= 128 and nseg <= 128:
+        out = torch.full((nseg, len(pct)), -777, dtype=torch.int64, device=DEV)
+        cnt = torch.full((nseg,), -777, dtype=torch.int64, device=DEV)
+        ds.tail_stats_static(dv, dseg, nseg, out, cnt, pct)
+        assert np.array_equal(out.cpu().numpy(), o) and np.array_equal(cnt.cpu().numpy(), oc), (seed, n, nseg, mode, pct, "static")

@@ -11,3 +11,10 @@ def test_randomised_differential_cases():
         _fuzz.one_case(seed)
     s = _fuzz.stats
     assert s["cases"] == 600 and min(s["kind"]) > 100 and s["requests"] > 1_500_000 and s["deferrals_possible"] > 200
+
+
+def test_randomised_characterize_and_tail_stats():
+    import _fuzz
+    for seed in range(500):
+        _fuzz.one_case_k1(seed)
+        _fuzz.one_case_k3(seed)
