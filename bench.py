@@ -159,7 +159,8 @@ def workload_config(n_traces, text_traces, c, note=None):
                        "KV 65536, Pareto outputs, rho 0.95, aging 250 ms; whole hot path per step: ds_characterize over the materialised "
                        "prompt text of the first %d traces (the other traces' (W,P) are drawn numerically, SURVEY.md §8(d)) -> "
                        "ds_simulate -> ds_latency_stats" % (n_traces, text_traces),
-           "l2": "inputs_exceed_l2 (3.4 GB of trace records + 5.7 GB of text re-read every step)",
+           "l2": "inputs_exceed_l2 (%.2f GB of trace records + %.1f GB of text re-read every step)"
+                 % (n_traces * 10000 * 21 / 1e9, c.text.size / 1e9 if c is not None and c.text is not None else 5.5 * text_traces / 1000.0),
            "per_rank": "own traces (seed 3 + 1000*rank)"}
     if c is not None:
         cfg.update({"instances": c.n_inst, "sim_requests_per_step": c.sim_requests,

@@ -10,9 +10,10 @@
 //
 // Design (v3, B200). The v2 kernel was bound by the ALU pipe (LOP3/SHF at half rate), not by HBM: 731 warp
 // instructions per 2 KiB. v3 cuts that to about a third:
-//  * every WARP is its own pipeline: it owns one contiguous span of 4 KiB chunks and a private ring of stages filled
-//    by 2-D TMA tile copies (32 rows x 128 B, SWIZZLE_128B, one mbarrier per stage, issued by lane 0): no block-wide
-//    barrier anywhere, and a lane reads its own 128-byte row with eight conflict-free LDS.128;
+//  * every WARP is its own pipeline: it owns one contiguous span of 4 KiB chunks and a private stage (kStages = 1 since
+//    r02: the refill is issued the moment the stage's bytes are in registers) filled by 2-D TMA tile copies (32 rows x
+//    128 B, SWIZZLE_128B, one mbarrier per stage, issued by an elected lane): no block-wide barrier anywhere, and a lane
+//    reads its own 128-byte row with eight conflict-free LDS.128;
 //  * byte classification is BIT-SLICED: each 32-byte group (8 registers) is transposed into its 8 bit planes
 //    (2 PRMT stages + 3 masked-shift stages, shifts issued as IMAD/IMAD.HI on the FMA pipe), after which WS and LETTER
 //    are a ~20-LOP3 boolean network evaluated for 32 bytes at a time, and the results already are position masks;
@@ -23,7 +24,7 @@
 //    chunks live in warp-uniform registers;
 //  * prompt boundaries come from a 32-entry register window over offsets[], held as 32-bit positions relative to the
 //    warp's span; the counts at a boundary are read back from a per-32-byte table {wordstart mask, token mask,
-//    running count} that the owning lanes leave in the already consumed stage buffer. A prompt that closes inside
+//    running count} that the owning lanes leave in the warp's shared-memory table `att`. A prompt that closes inside
 //    the warp's span is a plain store, the (at most two) prompts cut by the span's edges are integer atomicAdds.
 #include <cuda.h>
 
@@ -32,21 +33,29 @@
 namespace ds {
 namespace k1 {
 
+// Launch shape (r02, measured on configs[2] at 8 GiB): ONE CTA of 24 warps per SM, one 4 KiB TMA stage per warp.
+// The stage is refilled as soon as its bytes are in registers and a chunk's arithmetic (~575 warp instructions at 6 warps per
+// scheduler) outlasts the refill's latency, so a second stage only costs shared memory: 9 KB per warp instead of 13 KB is what lets
+// 24 warps (80 registers each, no spills) share an SM instead of 16. 8 warps x 2 CTAs x 2 stages: 4.61 TB/s; 16 x 1 x 2: 5.04;
+// 12 x 2 x 1: 4.90; 20 x 1 x 1 (96 registers): 5.17; 24 x 1 x 1: 5.25; 25 x 1 x 1 (72 registers): 4.73; 32 x 1 x 1 with kSub = 1: 4.97.
 #ifndef DS_K1_WARPS
-#define DS_K1_WARPS 8
+#define DS_K1_WARPS 24
+#endif
+#ifndef DS_K1_STAGES
+#define DS_K1_STAGES 1
 #endif
 #ifndef DS_K1_SUB
 #define DS_K1_SUB 2
 #endif
 #ifndef DS_K1_CTAS
-#define DS_K1_CTAS 2
+#define DS_K1_CTAS 1
 #endif
 constexpr int kWarps = DS_K1_WARPS;           // warps per CTA (each fully independent)
 constexpr int kThreads = kWarps * 32;
 constexpr int NW = 4;                         // 32-byte groups (= 32-bit mask words) per lane per chunk
 constexpr int kSeg = 32 * NW;                 // 128 bytes per lane per chunk = one TMA box row
 constexpr int kChunk = 32 * kSeg;             // 4 KiB per warp per step
-constexpr int kStages = 2;
+constexpr int kStages = DS_K1_STAGES;         // TMA stages per warp
 constexpr int kSub = DS_K1_SUB;               // chunks per boundary-attribution pass (amortises the window handling)
 constexpr int kCtasPerSM = DS_K1_CTAS;
 constexpr unsigned kFull = 0xffffffffu;
@@ -613,7 +622,10 @@ extern "C" int ds_characterize(const uint8_t* bytes, int64_t n_bytes, const int6
   if (attr_needed(DS_ATTR_K1))
     DS_CUDA(cudaFuncSetAttribute(k1::characterize_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(k1::Smem)));
   long long grid = (long long)num_sms() * k1::kCtasPerSM;
-  const long long need = (n_chunks + k1::kWarps - 1) / k1::kWarps;
+  // small inputs: spread the chunks over CTAs as 8 per CTA rather than filling every warp of a few CTAs (a warp whose span is
+  // empty returns at once), so that 1184 chunks (4.6 MiB) already reach every SM
+  constexpr int kFill = k1::kWarps < 8 ? k1::kWarps : 8;
+  const long long need = (n_chunks + kFill - 1) / kFill;
   if (grid > need) grid = need;
   const k1::Mul mu = {2u, 4u, 16u, 1u << 31, 1u << 30, 1u << 28, 1u << 16, 0u - (1u << 16)};
   k1::characterize_kernel<<<(unsigned)grid, k1::kThreads, sizeof(k1::Smem), st>>>(tmap, bytes, n_bytes, offsets, n_prompts, words_out,
