@@ -39,11 +39,33 @@
 namespace ds {
 namespace k2 {
 
-constexpr int kWarpsPerBlock = 4;
-#ifndef DS_K2_MIN_BLOCKS
-#define DS_K2_MIN_BLOCKS 7   // resident 128-thread blocks per SM the register allocation is bounded for (r02, with the running set in
-                             // shared memory: 6 / 7 / 8 blocks = configs[3] at 4096 traces 384.0 / 381.3 / 396.8 ms, configs[1] 12.92 / 12.47 / 13.29 ms)
+// Launch shape per instantiation (warps per block x resident blocks per SM the register allocation is bounded for), r02. With the
+// running set in shared memory the 4-slot body runs best at 28 warps of 72 registers (6 / 7 / 8 blocks of 4 warps = configs[3] at
+// 4096 traces 384.0 / 381.3 / 396.8 ms; 7 x 4, 2 x 14 and 1 x 28 are the same within 0.1 %, 24 warps of 80 registers +7 %). The
+// one-slot body fits 64 registers (32 warps) and the 8-slot body spills least at 80 (24 warps); both gain another 3-4 % from
+// 8-warp blocks (configs[1] 10.15 -> 9.75 ms, configs[4] at 1024 traces 319.7 -> 309.1 ms; 4 x 8 / 8 x 3 / 6 x 5 / 7 x 4 for the
+// former: 10.15 / 11.04 / 10.23 / 10.75, 4 x 7 / 4 x 6 / 6 x 4 / 5 x 5 for the latter: 319.7 / 321.6 / 325.1 / 321.8).
+#ifndef DS_K2_WARPS
+#define DS_K2_WARPS 4
 #endif
+#ifndef DS_K2_MIN_BLOCKS
+#define DS_K2_MIN_BLOCKS 7
+#endif
+#ifndef DS_K2_WARPS_1
+#define DS_K2_WARPS_1 8
+#endif
+#ifndef DS_K2_MIN_BLOCKS_1
+#define DS_K2_MIN_BLOCKS_1 4
+#endif
+#ifndef DS_K2_WARPS_8
+#define DS_K2_WARPS_8 8
+#endif
+#ifndef DS_K2_MIN_BLOCKS_8
+#define DS_K2_MIN_BLOCKS_8 3
+#endif
+template <int kSlots, bool kBudget, bool kReest> struct Shape { static constexpr int kWarps = DS_K2_WARPS, kBlocks = DS_K2_MIN_BLOCKS; };
+template <> struct Shape<1, false, false> { static constexpr int kWarps = DS_K2_WARPS_1, kBlocks = DS_K2_MIN_BLOCKS_1; };
+template <> struct Shape<8, false, false> { static constexpr int kWarps = DS_K2_WARPS_8, kBlocks = DS_K2_MIN_BLOCKS_8; };
 constexpr int kHeapSmem = 256;  // heap entries cached in shared memory per warp
 // Build with -DDS_K2_CHECK to verify the bookkeeping of the shared-memory structures on the device (compute-sanitizer is not
 // available on this pool): a violated invariant sets DS_DEV_INTERNAL in the status word. Off in the product build.
@@ -775,9 +797,10 @@ __global__ void __launch_bounds__(1024) order_kernel(const ds_instance* __restri
 }
 
 template <int kSlots, bool kBudget = false, bool kReest = false>
-__global__ void __launch_bounds__(k2::kWarpsPerBlock * 32, (kSlots == 1 && !kBudget) ? DS_K2_MIN_BLOCKS + 1 : DS_K2_MIN_BLOCKS)
-simulate_kernel(const __grid_constant__ Params p) {   // (one slot per lane: 8 blocks of 64 registers win, configs[1] 11.16 -> 10.51 ms; 4 / 8 slots: 7 blocks)
+__global__ void __launch_bounds__(k2::Shape<kSlots, kBudget, kReest>::kWarps * 32, k2::Shape<kSlots, kBudget, kReest>::kBlocks)
+simulate_kernel(const __grid_constant__ Params p) {   // (launch shape per instantiation: k2::Shape above)
   constexpr int kFac = kBudget ? 4 : 3;
+  constexpr int kWarpsPerBlock = Shape<kSlots, kBudget, kReest>::kWarps;
   __shared__ unsigned long long heap_sm[kWarpsPerBlock][kHeapSmem];
   __shared__ Slots<kSlots> slots_sm[kWarpsPerBlock];
   // lane and warp-in-block through volatile asm: under register pressure the compiler otherwise re-derives them from
@@ -908,30 +931,30 @@ static int simulate_impl(const ds_traces* tr, const uint8_t* category, const ds_
     note_launch();
   }
   note_launch();
-  const int threads = k2::kWarpsPerBlock * 32;
   int per_sm = 0;
-  auto launch = [&](auto kern) -> int {
+  auto launch = [&](auto kern, int warps) -> int {
+    const int threads = warps * 32;
     DS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, 0));
     if (per_sm < 1) per_sm = 1;
     long long blocks = (long long)n_sms * per_sm;
-    const long long need = (n_inst + k2::kWarpsPerBlock - 1) / k2::kWarpsPerBlock;
+    const long long need = (n_inst + warps - 1) / warps;
     if (blocks > need) blocks = need;
     kern<<<(unsigned)blocks, threads, 0, s>>>(p);
     note_launch();
     DS_CUDA(cudaGetLastError());
     return DS_OK;
   };
-  if (sv->reestimate) return launch(k2::simulate_kernel<8, false, true>);   // the variant's one instantiation serves every max_batch <= 256
+  if (sv->reestimate) return launch(k2::simulate_kernel<8, false, true>, k2::Shape<8, false, true>::kWarps);   // the variant's one instantiation serves every max_batch <= 256
   if (bp) {
-    if (sv->max_batch <= 32) return launch(k2::simulate_kernel<1, true>);
-    if (sv->max_batch <= 64) return launch(k2::simulate_kernel<2, true>);
-    if (sv->max_batch <= 128) return launch(k2::simulate_kernel<4, true>);
-    return launch(k2::simulate_kernel<8, true>);
+    if (sv->max_batch <= 32) return launch(k2::simulate_kernel<1, true>, k2::Shape<1, true, false>::kWarps);
+    if (sv->max_batch <= 64) return launch(k2::simulate_kernel<2, true>, k2::Shape<2, true, false>::kWarps);
+    if (sv->max_batch <= 128) return launch(k2::simulate_kernel<4, true>, k2::Shape<4, true, false>::kWarps);
+    return launch(k2::simulate_kernel<8, true>, k2::Shape<8, true, false>::kWarps);
   }
-  if (sv->max_batch <= 32) return launch(k2::simulate_kernel<1>);
-  if (sv->max_batch <= 64) return launch(k2::simulate_kernel<2>);
-  if (sv->max_batch <= 128) return launch(k2::simulate_kernel<4>);
-  return launch(k2::simulate_kernel<8>);
+  if (sv->max_batch <= 32) return launch(k2::simulate_kernel<1>, k2::Shape<1, false, false>::kWarps);
+  if (sv->max_batch <= 64) return launch(k2::simulate_kernel<2>, k2::Shape<2, false, false>::kWarps);
+  if (sv->max_batch <= 128) return launch(k2::simulate_kernel<4>, k2::Shape<4, false, false>::kWarps);
+  return launch(k2::simulate_kernel<8>, k2::Shape<8, false, false>::kWarps);
 }
 
 extern "C" int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
