@@ -40,11 +40,12 @@ namespace ds {
 namespace k2 {
 
 // Launch shape per instantiation (warps per block x resident blocks per SM the register allocation is bounded for), r02. With the
-// running set in shared memory the 4-slot body runs best at 28 warps of 72 registers (6 / 7 / 8 blocks of 4 warps = configs[3] at
-// 4096 traces 384.0 / 381.3 / 396.8 ms; 7 x 4, 2 x 14 and 1 x 28 are the same within 0.1 %, 24 warps of 80 registers +7 %). The
-// one-slot body fits 64 registers (32 warps) and the 8-slot body spills least at 80 (24 warps); both gain another 3-4 % from
-// 8-warp blocks (configs[1] 10.15 -> 9.75 ms, configs[4] at 1024 traces 319.7 -> 309.1 ms; 4 x 8 / 8 x 3 / 6 x 5 / 7 x 4 for the
-// former: 10.15 / 11.04 / 10.23 / 10.75, 4 x 7 / 4 x 6 / 6 x 4 / 5 x 5 for the latter: 319.7 / 321.6 / 325.1 / 321.8).
+// running set in shared memory the 4- and 8-slot bodies run best at 28 warps of 72 registers (6 / 7 / 8 blocks of 4 warps =
+// configs[3] at 4096 traces 384.0 / 381.3 / 396.8 ms; 7 x 4, 2 x 14 and 1 x 28 are the same within 0.1 %, 24 warps of 80
+// registers +7 %). The one-slot body fits 64 registers (32 warps) and gains 4 % from 8-warp blocks (configs[1] 10.15 -> 9.72 ms;
+// 4 x 8 / 8 x 3 / 6 x 5 / 7 x 4 / 16 x 2: 10.15 / 11.04 / 10.23 / 10.75 / 10.22). For the 8-slot body 8 x 3 at 80 registers looked
+// 3.5 % faster on configs[4] cut to 1024 traces (10 240 instances fill a third round of 24 warps per SM better than one of 28)
+// and is 3.9 % slower at full size (40 960 instances: 1131.9 against 1089.7 ms): it stays at 4 x 7.
 #ifndef DS_K2_WARPS
 #define DS_K2_WARPS 4
 #endif
@@ -57,15 +58,8 @@ namespace k2 {
 #ifndef DS_K2_MIN_BLOCKS_1
 #define DS_K2_MIN_BLOCKS_1 4
 #endif
-#ifndef DS_K2_WARPS_8
-#define DS_K2_WARPS_8 8
-#endif
-#ifndef DS_K2_MIN_BLOCKS_8
-#define DS_K2_MIN_BLOCKS_8 3
-#endif
 template <int kSlots, bool kBudget, bool kReest> struct Shape { static constexpr int kWarps = DS_K2_WARPS, kBlocks = DS_K2_MIN_BLOCKS; };
 template <> struct Shape<1, false, false> { static constexpr int kWarps = DS_K2_WARPS_1, kBlocks = DS_K2_MIN_BLOCKS_1; };
-template <> struct Shape<8, false, false> { static constexpr int kWarps = DS_K2_WARPS_8, kBlocks = DS_K2_MIN_BLOCKS_8; };
 constexpr int kHeapSmem = 256;  // heap entries cached in shared memory per warp
 // Build with -DDS_K2_CHECK to verify the bookkeeping of the shared-memory structures on the device (compute-sanitizer is not
 // available on this pool): a violated invariant sets DS_DEV_INTERNAL in the status word. Off in the product build.
