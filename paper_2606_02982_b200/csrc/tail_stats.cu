@@ -13,6 +13,11 @@
 namespace ds {
 namespace k3 {
 
+#ifndef DS_K3_KEYS
+#define DS_K3_KEYS 16    // staged keys per thread and trip of the digit passes: 4 / 8 / 16 = configs[3] stats at 4096 traces 16.05 / 13.94 / 13.57 ms
+#endif
+static_assert(DS_K3_KEYS % 4 == 0, "16-byte key loads");
+
 constexpr int kMaxPct = 8;
 constexpr unsigned long long kSign = 0x8000000000000000ull;
 
@@ -294,25 +299,31 @@ __global__ void __launch_bounds__(1024) lat_pass_kernel(const LatArgs a, int n_p
     // staged pass, all in 32 bits (measured: the 64-bit form of this loop - variable 64-bit shifts, 8-byte prefix compares -
     // executed 120 instructions per key and was issue-bound at 80-110 us for 102 MB). Every key agrees with every prefix
     // on bits 32..63 (they are common to all keys), so only bits [hshift, 32) are compared.
-    // 4 consecutive requests per thread (one 16-byte + one 4-byte load), the grid strides over the requests.
+    // kKeys consecutive requests per thread and trip (16-byte key loads + 4-byte code loads, all issued before the first use:
+    // the bytes in flight per SM, not the arithmetic, set the speed of these passes), the grid strides over the requests.
     const long long n = a.out_off[a.n_inst];
     const unsigned segall0 = 3u * (unsigned)a.n_groups;
-    const long long gstride = (long long)gridDim.x * blockDim.x * 4, nr = (n + 127) & ~127ll;   // warp-uniform trips
+    constexpr int kKeys = DS_K3_KEYS;
+    const long long gstride = (long long)gridDim.x * blockDim.x * kKeys, nr = (n + 32 * kKeys - 1) / (32 * kKeys) * (32 * kKeys);   // warp-uniform trips
     auto run = [&](auto np_tag, auto first_tag) {
       constexpr int NP = decltype(np_tag)::value;
       constexpr bool kFirst = decltype(first_tag)::value;
-      for (long long i4 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 4; i4 < nr; i4 += gstride) {
-        unsigned kk[4], cc[4];
-        if (i4 + 3 < n) {
-          const uint4 kv = *reinterpret_cast<const uint4*>(a.skey + i4);
-          const uchar4 cv = *reinterpret_cast<const uchar4*>(a.scode + i4);
-          kk[0] = kv.x; kk[1] = kv.y; kk[2] = kv.z; kk[3] = kv.w; cc[0] = cv.x; cc[1] = cv.y; cc[2] = cv.z; cc[3] = cv.w;
+      for (long long i4 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * kKeys; i4 < nr; i4 += gstride) {
+        unsigned kk[kKeys], cc[kKeys];
+        if (i4 + kKeys - 1 < n) {
+#pragma unroll
+          for (int v = 0; v < kKeys / 4; ++v) {
+            const uint4 kv = *reinterpret_cast<const uint4*>(a.skey + i4 + 4 * v);
+            const uchar4 cv = *reinterpret_cast<const uchar4*>(a.scode + i4 + 4 * v);
+            kk[4 * v] = kv.x; kk[4 * v + 1] = kv.y; kk[4 * v + 2] = kv.z; kk[4 * v + 3] = kv.w;
+            cc[4 * v] = cv.x; cc[4 * v + 1] = cv.y; cc[4 * v + 2] = cv.z; cc[4 * v + 3] = cv.w;
+          }
         } else {
 #pragma unroll
-          for (int u = 0; u < 4; ++u) { const bool in = i4 + u < n; kk[u] = in ? a.skey[i4 + u] : 0u; cc[u] = in ? a.scode[i4 + u] : 255u; }
+          for (int u = 0; u < kKeys; ++u) { const bool in = i4 + u < n; kk[u] = in ? a.skey[i4 + u] : 0u; cc[u] = in ? a.scode[i4 + u] : 255u; }
         }
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < kKeys; ++u) {
           const bool ok = cc[u] != 255u;
           const unsigned s_t = ok ? cc[u] : 0u;
           if (kFirst) {    // every key matches every prefix of its segments: one add, the other histograms follow from it
