@@ -50,10 +50,11 @@ def _same(name, g, o, desc):
     assert bad.size == 0, (name, desc, bad[:5], g[bad[:5]], o[bad[:5]])
 
 
-def one_case(seed):
+def one_case(seed, long_traces=False):
     rng = np.random.default_rng(seed)
     n_tr = int(rng.integers(1, 5))
-    lens = [int(rng.choice([1, 2, 5, 31, 32, 33, 64, 100, 257, 700])) for _ in range(n_tr)]
+    # long_traces: queues deeper than the 256 heap entries SJF keeps in shared memory, many 32-request windows, long clocks
+    lens = [int(rng.choice([1500, 3000, 5000] if long_traces else [1, 2, 5, 31, 32, 33, 64, 100, 257, 700])) for _ in range(n_tr)]
     parts = [gen_trace(rng, n) for n in lens]
     trace_off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
     arrival, tier, words, tokens, out_len = (np.concatenate([p[k] for p in parts]) for k in range(5))

@@ -9,8 +9,10 @@ def test_randomised_differential_cases():
     import _fuzz
     for seed in range(20261105, 20261105 + 600):
         _fuzz.one_case(seed)
+    for seed in range(77000, 77012):                     # (the oracle steps every boundary: a deep-queue case takes it seconds)
+        _fuzz.one_case(seed, long_traces=True)
     s = _fuzz.stats
-    assert s["cases"] == 600 and min(s["kind"]) > 100 and s["requests"] > 1_500_000 and s["deferrals_possible"] > 200
+    assert s["cases"] == 612 and min(s["kind"]) > 100 and s["requests"] > 1_500_000 and s["deferrals_possible"] > 200
 
 
 def test_randomised_characterize_and_tail_stats():
