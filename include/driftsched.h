@@ -138,6 +138,13 @@ typedef struct {
  *   record per trace request (tokens/words ratio, tokens, out_len; written by a pre-pass of every call).
  * Contract checked on the device (DS_DEV_BAD_TRACE, outputs of that instance unspecified): tier <= 2, words/tokens >= 0,
  *   1 <= out_len < 2^30, arrival_tick >= 0 and non-decreasing over every pair of neighbouring requests of a trace.
+ *   The check REPORTS, it does not stop the instance: with decreasing arrivals a request may be queued ahead of its turn or
+ *   twice. What was verified on such inputs (randomised closed-loop cases under the -DDS_K2_CHECK build): every
+ *   request index the kernel uses stays inside the trace, so start_tick / done_tick / est_out writes stay inside the
+ *   instance's own ranges, and the running-set bookkeeping stays intact. What is NOT guaranteed: the SJF heap / re-estimation
+ *   queue scratch and the trajectory samples of such an instance may run up to a few entries past its own share of the
+ *   workspace / ema_traj. When DS_DEV_BAD_TRACE is set, treat every output of the CALL as invalid and validate the traces
+ *   (sorted arrivals; for ds_simulate_closed: every client start tick <= the first release) before calling again.
  * Launches: 1 memset (work counter) + 3 kernels (policy-major ordering of the instances, request records, simulation). */
 int ds_simulate(const ds_traces* tr, const ds_server* sv, const ds_instance* inst, int64_t n_inst,
                 const int64_t* out_off, int64_t n_total, int64_t* start_tick, int64_t* done_tick, double* ema_final,
